@@ -1,0 +1,340 @@
+"""Pins P1-P13: the oracle against what the paper and the mathematics fix.
+
+None of these retype the oracle's formulas: they use explicit many-body matrices
+(tests/fock.py), brute-force four-index sums, closed forms, scipy's matrix exponential,
+Gauss-Hermite quadrature, and invariances.  CPU only.
+"""
+import numpy as np
+import pytest
+import scipy.linalg as sla
+
+from oracle.afqmc_oracle import AFQMCOracle
+from tests.fock import Fock
+
+
+def small_problem(M, na, nb, ng, kind, seed, lscale=0.3, noise=0.2, nw=3):
+    r = np.random.default_rng(seed)
+    h = r.standard_normal((M, M)); h = 0.5 * (h + h.T)
+    L = r.standard_normal((ng, M, M)) * lscale
+    L = 0.5 * (L + L.transpose(0, 2, 1))
+    if kind == 0:
+        trial = np.linalg.qr(r.standard_normal((M, na)))[0]
+        Nt = na
+    else:
+        trial = np.concatenate([np.linalg.qr(r.standard_normal((M, na)))[0],
+                                np.linalg.qr(r.standard_normal((M, nb)))[0]], axis=1)
+        Nt = na + nb
+    walkers = trial[None] + noise * (r.standard_normal((nw, M, Nt)) + 1j * r.standard_normal((nw, M, Nt)))
+    return h, L, trial, walkers.astype(np.complex128)
+
+
+def spin_blocks(o, mat):
+    """(alpha, beta) column blocks of a [M, Nt] array under the oracle's walker kind."""
+    if o.walker_kind == 0:
+        return mat[:, :o.n_alpha], mat[:, :o.n_alpha]
+    return mat[:, :o.n_alpha], mat[:, o.n_alpha:o.n_alpha + o.n_beta]
+
+
+# --------------------------------------------------------------------------- P1
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P1_walker_equals_trial(kind):
+    h, L, trial, _ = small_problem(8, 3, 2 if kind else 3, 5, kind, 1)
+    o = AFQMCOracle(h, L, trial, 3, 2 if kind else 3, kind)
+    w = trial[None].astype(np.complex128)
+    assert abs(o.overlap(w)[0] - 1) < 1e-13
+    for G, p in zip(o.greens_function(w), o.psi):
+        assert np.abs(G[0] - (p @ p.T).T).max() < 1e-13          # G = P^T
+    X = o.force_bias_X(o.theta(w))
+    assert np.abs(X[0] - o.m).max() < 1e-12                       # X = m  =>  xbar = 0
+    _, info = o.propagate(w, np.zeros((1, 5)), 0.01)
+    assert np.abs(info["xbar"]).max() < 1e-12
+
+
+# --------------------------------------------------------------------------- P2
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P2_hartree_fock_closed_form(kind):
+    na, nb = (3, 3) if kind == 0 else (3, 2)
+    h, L, trial, _ = small_problem(9, na, nb, 7, kind, 2)
+    o = AFQMCOracle(h, L, trial, na, nb, kind)
+    pa = trial[:, :na]
+    pb = pa if kind == 0 else trial[:, na:]
+    Pa, Pb = pa @ pa.T, pb @ pb.T
+    e1 = np.trace(h @ Pa) + np.trace(h @ Pb)
+    ec = 0.5 * sum((np.trace(Lg @ Pa) + np.trace(Lg @ Pb)) ** 2 for Lg in L)
+    ex = -0.5 * sum(np.trace(Lg @ Pa @ Lg @ Pa) + np.trace(Lg @ Pb @ Lg @ Pb) for Lg in L)
+    E = o.local_energy(trial[None].astype(np.complex128))[0]
+    assert abs(E[0] - (e1 + ec + ex)) < 1e-12 * abs(e1 + ec + ex) + 1e-12
+    assert abs(E[1] - e1) < 1e-12
+    assert abs(E[2] - (ec + ex)) < 1e-12
+    assert abs(o.e_shift - (e1 + ec + ex)) < 1e-11                # auto shift = trial energy
+
+
+# --------------------------------------------------------------------------- P3
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P3_bruteforce_four_index(kind):
+    na, nb = (3, 3) if kind == 0 else (4, 2)
+    h, L, trial, walkers = small_problem(10, na, nb, 6, kind, 3)
+    o = AFQMCOracle(h, L, trial, na, nb, kind)
+    eri = np.einsum("gps,gqr->psqr", L, L)                        # (ps|qr), Eq. (3)
+    Gs = o.greens_function(walkers)
+    if kind == 0:
+        Gs = [Gs[0], Gs[0]]
+    E = o.local_energy(walkers)
+    for w in range(walkers.shape[0]):
+        Ga, Gb = Gs[0][w], Gs[1][w]
+        Gt = Ga + Gb
+        e1 = np.sum(h * Gt)
+        # <a+_p a+_q a_r a_s> = G_ps G_qr - delta_spin G_pr G_qs  (Wick)
+        e2 = 0.5 * (np.einsum("psqr,ps,qr->", eri, Gt, Gt)
+                    - np.einsum("psqr,pr,qs->", eri, Ga, Ga)
+                    - np.einsum("psqr,pr,qs->", eri, Gb, Gb))
+        assert abs(E[w, 1] - e1) < 1e-12 * max(1, abs(e1))
+        assert abs(E[w, 2] - e2) < 1e-11 * max(1, abs(e2))
+        assert abs(E[w, 0] - (e1 + e2)) < 1e-11 * max(1, abs(e1 + e2))
+
+
+# --------------------------------------------------------------------------- P4
+@pytest.mark.parametrize("kind,na,nb", [(1, 2, 1), (0, 2, 2)])
+def test_P4_fock_space(kind, na, nb):
+    M, ng = 4, 3
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, 4)
+    o = AFQMCOracle(h, L, trial, na, nb, kind)
+    F = Fock(M)
+    H = F.hamiltonian(h, L)
+    ta, tb = spin_blocks(o, trial)
+    bra = F.det_state(ta.astype(complex), tb.astype(complex)).conj()
+    ov = o.overlap(walkers)
+    E = o.local_energy(walkers)
+    X = o.force_bias_X(o.theta(walkers))
+    Gs = o.greens_function(walkers)
+    for w in range(walkers.shape[0]):
+        wa, wb = spin_blocks(o, walkers[w])
+        ket = F.det_state(wa, wb)
+        ov_mb = bra @ ket
+        assert abs(ov[w] - ov_mb) < 1e-12
+        assert abs(E[w, 0] - (bra @ H @ ket) / ov_mb) < 1e-11
+        for g in range(ng):
+            assert abs(X[w, g] - (bra @ F.one_body(L[g]) @ ket) / ov_mb) < 1e-12
+        for p in range(M):
+            for q in range(M):                                   # alpha Green's function
+                g_mb = (bra @ F.cd[p] @ F.c[q] @ ket) / ov_mb
+                assert abs(Gs[0][w][p, q] - g_mb) < 1e-12
+    # Thouless: e^{A_hat}|phi> = |e^{A} phi> for a complex symmetric one-body A
+    A = -1j * 0.1 * np.einsum("g,gpq->pq", np.array([0.3, -1.1, 0.7]), L)
+    wa, wb = spin_blocks(o, walkers[0])
+    lhs = sla.expm(F.one_body(A)) @ F.det_state(wa, wb)
+    rhs = F.det_state(sla.expm(A) @ wa, sla.expm(A) @ wb)
+    assert np.abs(lhs - rhs).max() < 1e-12
+
+
+# --------------------------------------------------------------------------- P5
+@pytest.mark.parametrize("seed", [5, 6])
+def test_P5_mean_field_shift_identity(seed):
+    """H = H1[h_mod] + E_const + 1/2 sum_g (L_g - m_g)^2 for the oracle's h_mod, E_const, m,
+    whatever trial (hence whatever m) it was built from (Eqs. 4-6)."""
+    M, ng = 3, 3
+    h, L, trial, _ = small_problem(M, 2, 1, ng, 1, seed)
+    o = AFQMCOracle(h, L, trial, 2, 1, 1)
+    F = Fock(M)
+    H = F.hamiltonian(h, L)
+    I = np.eye(2 ** F.n)
+    rhs = F.one_body(o.h_mod) + o.E_const * I
+    for g in range(ng):
+        d = F.one_body(L[g]) - o.m[g] * I
+        rhs = rhs + 0.5 * d @ d
+    assert np.abs(H - rhs).max() < 1e-12
+    assert np.abs(o.m).max() > 1e-2
+
+
+# --------------------------------------------------------------------------- P6
+def _quadrature_error(dt, mode, kind=1):
+    M, ng, na, nb = 3, 2, 2, 1
+    if kind == 0:
+        nb = na
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, 7, lscale=0.5, noise=0.15, nw=1)
+    o = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24)
+    F = Fock(M)
+    H = F.hamiltonian(h, L)
+    wa, wb = spin_blocks(o, walkers[0])
+    exact = sla.expm(-dt * H) @ F.det_state(wa, wb)
+    nodes, wts = np.polynomial.hermite_e.hermegauss(28)
+    wts = wts / wts.sum()
+    xs = np.array([[a, b] for a in nodes for b in nodes])
+    ws = np.array([u * v for u in wts for v in wts])
+    batch = np.repeat(walkers, xs.shape[0], axis=0)
+    override = {"fb": None, "zero": np.zeros(ng), "arb": np.array([0.11 - 0.07j, -0.05 + 0.13j])}[mode]
+    new, info = o.propagate(batch, xs, dt, xbar_override=override)
+    # exp(c_fb + c_mf - dt E_const) = I * ovlp_old/ovlp_new * exp(-dt E_shift)
+    scal = info["I"] * info["ovlp_old"] / info["ovlp_new"] * np.exp(-dt * o.e_shift)
+    acc = np.zeros_like(exact)
+    for k in range(xs.shape[0]):
+        a, b = spin_blocks(o, new[k])
+        acc = acc + ws[k] * scal[k] * F.det_state(a, b)
+    return np.linalg.norm(acc - exact) / np.linalg.norm(exact)
+
+
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P6_hubbard_stratonovich_quadrature(kind):
+    """int dx p(x) e^{x.xbar - xbar.xbar/2} B(x - xbar)|phi> = e^{-dt H}|phi> + O(dt^2)
+    (Eqs. 8, 9, 12, 16) for the force bias, for xbar = 0 and for an arbitrary complex xbar."""
+    e1 = {m: _quadrature_error(0.02, m, kind) for m in ("fb", "zero", "arb")}
+    e2 = {m: _quadrature_error(0.01, m, kind) for m in ("fb", "zero", "arb")}
+    for m in e1:
+        assert e1[m] < 5e-3
+        assert 3.3 < e1[m] / e2[m] < 4.7, (m, e1[m], e2[m])
+    # independent of xbar to quadrature accuracy
+    assert abs(e1["fb"] - e1["zero"]) < 1e-6 and abs(e1["arb"] - e1["zero"]) < 1e-6
+
+
+# --------------------------------------------------------------------------- P7
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P7_reorthonormalisation(kind):
+    na, nb = (3, 3) if kind == 0 else (3, 2)
+    h, L, trial, walkers = small_problem(8, na, nb, 5, kind, 8, noise=0.4)
+    o = AFQMCOracle(h, L, trial, na, nb, kind)
+    q, detR = o.reorthonormalise(walkers)
+    for a, b in o.blocks:
+        for w in range(walkers.shape[0]):
+            Q = q[w, :, a:b]
+            assert np.abs(Q.conj().T @ Q - np.eye(b - a)).max() < 1e-13
+            R = Q.conj().T @ walkers[w, :, a:b]
+            assert np.abs(np.tril(R, -1)).max() < 1e-13          # upper triangular
+            assert np.all(np.diagonal(R).real > 0) and np.abs(np.diagonal(R).imag).max() < 1e-13
+    assert np.abs(o.local_energy(q) - o.local_energy(walkers)).max() < 1e-11
+    assert np.abs(o.force_bias_X(o.theta(q)) - o.force_bias_X(o.theta(walkers))).max() < 1e-11
+    assert np.abs(o.overlap(walkers) / detR - o.overlap(q)).max() < 1e-12
+    # and through step(): ortho_every=1 returns orthonormal walkers and the matching overlap
+    o1 = AFQMCOracle(h, L, trial, na, nb, kind, ortho_every=1)
+    x = np.random.default_rng(0).standard_normal((walkers.shape[0], 5))
+    nwk, wts, ov = o1.step(walkers, np.ones(walkers.shape[0]), x, 0.01)
+    assert np.abs(o1.overlap(nwk) - ov).max() < 1e-12
+    o0 = AFQMCOracle(h, L, trial, na, nb, kind, ortho_every=0)
+    nwk0, wts0, ov0 = o0.step(walkers, np.ones(walkers.shape[0]), x, 0.01)
+    assert np.abs(wts - wts0).max() < 1e-14                       # weights untouched by QR
+    assert np.abs(o0.local_energy(nwk0) - o0.local_energy(nwk)).max() < 1e-10
+
+
+# --------------------------------------------------------------------------- P8
+def _std_log_I(dt, flip):
+    h, L, trial, walkers = small_problem(6, 2, 2, 8, 0, 9, lscale=0.4, noise=0.25, nw=1)
+    o = AFQMCOracle(h, L, trial, 2, 2, 0, taylor_order=12)
+    r = np.random.default_rng(11)
+    x = r.standard_normal((300, 8))
+    batch = np.repeat(walkers, 300, axis=0)
+    override = None
+    if flip:
+        _, info0 = o.propagate(walkers, x[:1], dt)
+        override = -info0["xbar"][0]
+    _, info = o.propagate(batch, x, dt, xbar_override=override)
+    return np.std(np.log(info["I"]))
+
+
+def test_P8_force_bias_sign():
+    """With xbar = +i sqrt(dt)(X - m) the O(sqrt dt) fluctuation of log I cancels:
+    std(log I) ~ dt; with Eq. (14)'s printed sign it stays ~ sqrt(dt) (reading S1)."""
+    r_good = _std_log_I(0.02, False) / _std_log_I(0.005, False)
+    r_bad = _std_log_I(0.02, True) / _std_log_I(0.005, True)
+    assert r_good > 3.0, r_good
+    assert r_bad < 2.6, r_bad
+    assert _std_log_I(0.005, False) < 0.5 * _std_log_I(0.005, True)
+
+
+# --------------------------------------------------------------------------- P9
+def test_P9_rhf_equals_uhf_on_duplicated_blocks():
+    h, L, trial, walkers = small_problem(8, 3, 3, 6, 0, 10)
+    o_r = AFQMCOracle(h, L, trial, 3, 3, 0)
+    o_u = AFQMCOracle(h, L, np.concatenate([trial, trial], axis=1), 3, 3, 1)
+    wu = np.concatenate([walkers, walkers], axis=2)
+    assert np.abs(o_r.local_energy(walkers) - o_u.local_energy(wu)).max() < 1e-12
+    assert abs(o_r.e_shift - o_u.e_shift) < 1e-12
+    x = np.random.default_rng(1).standard_normal((3, 6))
+    a, wa, ova = o_r.step(walkers, np.ones(3), x, 0.01)
+    b, wb, ovb = o_u.step(wu, np.ones(3), x, 0.01)
+    assert np.abs(a - b[:, :, :3]).max() < 1e-13 and np.abs(a - b[:, :, 3:]).max() < 1e-13
+    assert np.abs(wa - wb).max() < 1e-13 and np.abs(ova - ovb).max() < 1e-12
+
+
+# --------------------------------------------------------------------------- P10
+def test_P10_taylor_vs_expm():
+    h, L, trial, walkers = small_problem(8, 3, 3, 6, 0, 12, lscale=0.15)
+    dt = 0.01
+    x = np.random.default_rng(2).standard_normal((3, 6))
+    for K, tol_fn in ((6, lambda a: a ** 7 / 5040 * np.exp(a)), (24, lambda a: 1e-13)):
+        o = AFQMCOracle(h, L, trial, 3, 3, 0, taylor_order=K)
+        new, info = o.propagate(walkers, x, dt)
+        E1 = sla.expm(-0.5 * dt * o.h_mod)
+        for w in range(3):
+            A = info["A"][w]
+            nA = np.linalg.norm(A, 2)
+            assert nA <= 0.3
+            mid = E1 @ walkers[w]
+            exact = E1 @ (sla.expm(A) @ mid)
+            err = np.linalg.norm(new[w] - exact, 2)
+            scale = np.linalg.norm(mid, 2) * np.linalg.norm(E1, 2)
+            assert err <= 1.05 * tol_fn(nA) * scale + 1e-14
+            if K == 6:
+                assert err > 1e-3 * tol_fn(nA) * scale             # the bound is not vacuous
+            # A = -i sqrt(dt) sum xs_g L_g, complex symmetric
+            assert np.abs(A - A.T).max() < 1e-15
+            ref = -1j * np.sqrt(dt) * np.einsum("g,gpq->pq", info["xs"][w], L)
+            assert np.abs(A - ref).max() < 1e-14
+
+
+# --------------------------------------------------------------------------- P11
+def test_P11_one_body_limit():
+    M, na = 7, 3
+    h, _, trial, walkers = small_problem(M, na, na, 4, 0, 13)
+    L0 = np.zeros((4, M, M))
+    dt = 0.05
+    o = AFQMCOracle(h, L0, trial, na, na, 0, ortho_every=1)
+    x = np.random.default_rng(3).standard_normal((3, 4))
+    new, info = o.propagate(walkers, x, dt)
+    assert np.abs(info["X"]).max() == 0 and np.abs(info["xbar"]).max() == 0 and np.abs(info["A"]).max() == 0
+    ref = np.einsum("pq,wqi->wpi", sla.expm(-dt * h), walkers)
+    assert np.abs(new - ref).max() < 1e-12
+    r = o.overlap(ref) / o.overlap(walkers)
+    _, wts, _ = o.step(walkers, np.ones(3), x, dt)
+    expect = np.abs(r) * np.exp(dt * o.e_shift) * np.maximum(0, np.cos(np.angle(r)))
+    assert np.abs(wts - expect).max() < 1e-12
+    # long projection converges to the sum of the lowest na eigenvalues (x2 for RHF)
+    wk, w = walkers, np.ones(3)
+    for _ in range(1500):
+        wk, w, _ = o.step(wk, w, x, dt)
+    e0 = 2 * np.sort(np.linalg.eigvalsh(h))[:na].sum()
+    assert np.abs(o.local_energy(wk)[:, 0] - e0).max() < 1e-8
+
+
+# --------------------------------------------------------------------------- P12
+def test_P12_conjugation_symmetry():
+    h, L, trial, walkers = small_problem(8, 3, 2, 6, 1, 14)
+    o = AFQMCOracle(h, L, trial, 3, 2, 1)
+    x = np.random.default_rng(4).standard_normal((3, 6))
+    a, wa, ova = o.step(walkers, np.ones(3), x, 0.01)
+    b, wb, ovb = o.step(walkers.conj(), np.ones(3), -x, 0.01)
+    assert np.abs(a.conj() - b).max() < 1e-13
+    assert np.abs(wa - wb).max() < 1e-13 and np.abs(ova.conj() - ovb).max() < 1e-13
+    assert np.abs(o.local_energy(walkers).conj() - o.local_energy(walkers.conj())).max() < 1e-12
+
+
+# --------------------------------------------------------------------------- P13
+def test_P13_weights_real_nonnegative_and_phaseless_cut():
+    h, L, trial, walkers = small_problem(8, 3, 3, 6, 0, 15, lscale=0.8, noise=0.6, nw=40)
+    o = AFQMCOracle(h, L, trial, 3, 3, 0)
+    r = np.random.default_rng(5)
+    wk, w = walkers, np.ones(40)
+    killed = 0
+    for s in range(6):
+        x = r.standard_normal((40, 6))
+        _, info = o.propagate(wk, x, 0.05)
+        wk, w, _ = o.step(wk, w, x, 0.05)
+        assert w.dtype == np.float64 and np.all(w >= 0) and np.all(np.isfinite(w))
+        neg = info["S"].real <= 0
+        assert np.all(w[neg] == 0)                                # max[0, cos theta], Eq. (15)
+        killed += int(neg.sum())
+    assert killed > 0                                             # the cut was exercised
+    E = o.local_energy(wk)
+    assert np.isfinite(np.sum(w * E[:, 0]) / np.sum(w))
+    # a zero-overlap walker gets weight 0, not an error (reading S10)
+    bad = walkers[:1].copy(); bad[:] = 0
+    _, wb, _ = o.step(bad, np.ones(1), r.standard_normal((1, 6)), 0.05)
+    assert wb[0] == 0.0
