@@ -96,13 +96,13 @@ class AFQMCOracle:
         hprime = h1.copy()                       # D2 / Eq. (5): h' = h - 1/2 sum_g L_g L_g
         mL = np.zeros((M, M))                    # sum_g m_g L_g
         for g0, Ls in _as_slab_iter(L):
-            ms = np.einsum("gpq,pq->g", Ls, P_tot)
+            ms = Ls.reshape(Ls.shape[0], -1) @ P_tot.ravel()
             m_list.append(ms)
             for g in range(Ls.shape[0]):
                 hprime -= 0.5 * (Ls[g] @ Ls[g])
                 mL += ms[g] * Ls[g]
             for s, p in enumerate(self.psi):     # S4 half rotation: Lrot^g_sigma = psi^T L_g
-                lrot[s].append(np.einsum("pi,gpq->giq", p, Ls))
+                lrot[s].append(p.T @ Ls)                 # [g, Ns, M]
         self.m = np.concatenate(m_list)
         self.n_chol = self.m.shape[0]
         if n_chol is not None and n_chol != self.n_chol:
