@@ -1,0 +1,132 @@
+/* afqmc.h - C ABI of libafqmc: one batched phaseless-AFQMC walker step and the local energy,
+ * single-determinant RHF/UHF trial, Cholesky-factorised Hamiltonian, on one B200 (sm_100a).
+ *
+ * The operations are those of /root/reference/PAPER.md (arXiv 2406.16238) Sec. II,
+ * Eqs. (2)-(18); the working formulas derived from them are listed in
+ * DESIGN.md ("Readings") and follow SURVEY.md 8(c).
+ *
+ * Conventions
+ *   - All matrices are row-major.  complex128 = two consecutive doubles (re, im).
+ *   - H = sum_pq h1[p][q] a+_p a_q + 1/2 sum (ps|qr) a+_p a+_q a_r a_s with
+ *     (ps|qr) = sum_g L[g][p][s] L[g][q][r]            (Eqs. 2-3)
+ *   - v_g = i L_g (Eq. 6); B(x) = e^{-dt/2 v0} e^{-sqrt(dt) x.v} e^{-dt/2 v0} (Eq. 9),
+ *     so the two-body propagator is exp(A), A = -i sqrt(dt) sum_g (x_g - xbar_g) L_g, applied
+ *     by a Taylor series of order `taylor_order`.  The force bias is
+ *     xbar_g = +i sqrt(dt) (X_g - m_g), X_g = <Psi_T|L_g|phi>/<Psi_T|phi>, m_g = <L_g>_T
+ *     (Eq. 14 with the sign that is consistent with Eq. 9: DESIGN.md reading S1).
+ *   - Trial columns are [alpha | beta], real, orthonormal per spin block.
+ *   - walker_kind 0 (RHF): restricted walkers, ONE block [M][n_alpha] per walker used for
+ *     both spins, Nt = n_alpha.  walker_kind 1 (UHF): Nt = n_alpha + n_beta, alpha first.
+ *
+ * Pointers: every pointer argument says HOST, DEVICE or EITHER.  EITHER pointers are
+ * classified with cudaPointerGetAttributes; host buffers are staged through the handle's
+ * stream inside the call (and, for outputs, the call returns after the copy back).
+ * Calls on device buffers are asynchronous on the handle's stream.
+ *
+ * Errors: every int32_t entry point returns AFQMC_OK or a negative code; nothing throws or
+ * aborts across the ABI.  afqmc_last_error() gives a message for the last failure on that
+ * handle (or for a failed afqmc_create when passed NULL).  A walker whose overlap with the
+ * trial is zero or non-finite is NOT an error: its weight becomes exactly 0 (Eq. 15,
+ * reading S10).  One handle per host thread; no global mutable state besides the create
+ * error string.
+ */
+#ifndef AFQMC_H_
+#define AFQMC_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define AFQMC_OK 0
+#define AFQMC_ERR_INVALID (-1)     /* null pointer / bad struct_size / bad value          */
+#define AFQMC_ERR_DIMS (-2)        /* nw > max_walkers, RHF with n_alpha != n_beta, ...   */
+#define AFQMC_ERR_ALLOC (-3)       /* device or host allocation failed                    */
+#define AFQMC_ERR_CUDA (-4)        /* CUDA runtime error, see afqmc_last_error            */
+#define AFQMC_ERR_TRIAL (-5)       /* trial columns not orthonormal to 1e-10              */
+#define AFQMC_ERR_UNSUPPORTED (-6) /* taylor_order > 16, occupied block > 64 columns, ... */
+
+typedef struct afqmc_handle afqmc_handle; /* opaque, library-owned */
+
+typedef struct {
+  int32_t struct_size;  /* = sizeof(afqmc_params) */
+  int32_t M;            /* orbitals (the paper's N)                          */
+  int32_t n_alpha;      /* occupied alpha                                                 */
+  int32_t n_beta;       /* occupied beta                                                  */
+  int32_t n_chol;       /* Cholesky vectors N_gamma                         */
+  int32_t max_walkers;  /* workspaces are sized for this many walkers per call            */
+  int32_t walker_kind;  /* 0 RHF restricted walkers, 1 UHF [alpha|beta]                   */
+  int32_t taylor_order; /* 0 -> 6; at most 16                                             */
+  int32_t ortho_every;  /* 0 never; n: QR after every n-th afqmc_step on this handle      */
+  int32_t e_shift_auto; /* 1: E_shift = local energy of the trial; 0: use e_shift         */
+  double e_shift;       /* energy shift in the weight, exp(-dt (E_const - E_shift))       */
+  void* stream;         /* cudaStream_t to run on; NULL = the library creates its own     */
+} afqmc_params;
+
+/* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;
+ * "half rotation").  Computes m_g = tr(L_g P), h' = h1 - 1/2 sum_g L_g L_g,
+ * h_mod = h' + sum_g m_g L_g, E_const = -1/2 sum_g m_g^2, Lrot^g = trial^T L_g,
+ * hrot = trial^T h1 and (if e_shift_auto) the trial's local energy, all on the device.
+ *   h1     EITHER [M][M] symmetric, COPIED.
+ *   L_chol DEVICE [n_chol][M][M], each L_g symmetric; BORROWED read-only until afqmc_destroy
+ *          (it is the dominant resident array, 55 GB in the largest configuration).
+ *   trial  EITHER [M][Nt] real, COPIED.
+ *   out    receives the handle; NULL on failure. */
+int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial,
+                     const afqmc_params* p, afqmc_handle** out);
+
+/* One walker step for nw walkers (Eqs. 12-18):
+ * overlap and Theta = phi O^-1, force bias, field shift, A = V_HS build, phi <- E1 e^A E1 phi
+ * with E1 = expm(-dt/2 h_mod) (cached per dt), new overlap, w <- w |I| max(0, cos arg S),
+ * and, every ortho_every-th call, thin QR with R_ii > 0 (weights unchanged).
+ *   walkers    EITHER complex128 [nw][M][Nt], in/out.
+ *   weights    EITHER double [nw], in/out.
+ *   aux_fields EITHER double [nw][n_chol], standard normal draws x (Eq. 8), read-only.
+ * The overlap of the walkers as returned is kept in the handle (afqmc_get_overlaps). */
+int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields,
+                   double dt, int32_t nw);
+
+/* Local energy E_loc = <Psi_T|H|phi>/<Psi_T|phi> (Eq. 11):
+ * one-body, Coulomb 1/2 sum_g X_g^2 and exchange -1/2 sum_g sum_spin tr(T_g T_g),
+ * T_g = Lrot^g Theta.
+ *   walkers EITHER complex128 [nw][M][Nt], read-only.
+ *   E_out   EITHER complex128 [nw][3] = (E, E_1body, E_2body) per walker, as
+ *           energy[:, 0..2] of the paper's Code Snippet 9. */
+int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, int32_t nw);
+
+/* Overlaps <Psi_T|phi_w> of the walkers as left by the last afqmc_step.
+ *   ovlp_out EITHER complex128 [nw of that step]. */
+int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out);
+
+/* Scalars fixed at create: out[0] = E_const, out[1] = E_shift in use, out[2] = trial energy
+ * (NaN if never computed).  HOST pointer. */
+int32_t afqmc_get_constants(afqmc_handle* h, double* out3);
+
+/* Diagnostics for stage-by-stage parity tests: copies an internal device array of the last
+ * step / energy call to `out` (EITHER).  which: 0 = X [nw][2][n_chol] (re plane, im plane;
+ * the force-bias expectation <L_g> of the last step, spin summed), 1 = A = V_HS
+ * [nw][2][M][M] (re plane, im plane), 2 = E1 [M][M], 3 = h_mod [M][M], 4 = m [n_chol],
+ * 5 = Lrot [n_chol][Nt][M].  Returns the number of doubles written, or a negative code;
+ * with out == NULL only returns the count. */
+int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out);
+
+/* Number of kernel launches issued by this handle since create (for bench.py). */
+int64_t afqmc_launch_count(const afqmc_handle* h);
+
+/* Stream synchronise and surface any deferred CUDA error. */
+int32_t afqmc_sync(afqmc_handle* h);
+
+const char* afqmc_last_error(const afqmc_handle* h);
+
+void afqmc_destroy(afqmc_handle* h);
+
+/* Measurement helper (not part of the method): register-only issue loops on all SMs for
+ * `ms` milliseconds each.  out[0] = FP64 mma.sync m8n8k4 (DMMA) TFLOP/s, out[1] = FP64 FMA
+ * (DFMA) TFLOP/s, out[2] = SM clock seen (MHz, from clock64/elapsed).  HOST pointer. */
+int32_t afqmc_measure_fp64_peak(double ms, double* out3);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AFQMC_H_ */

@@ -1,0 +1,162 @@
+"""ctypes binding of libafqmc.so (include/afqmc.h).  Argument marshalling only: every step
+of the path runs in the library's CUDA kernels.  There is no CPU fallback: if the library is
+missing or cannot be loaded, importing this module raises.
+
+Arrays may be torch CUDA tensors (device pointers) or NumPy arrays / CPU tensors (host
+pointers, staged inside the library call).
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libafqmc.so")
+
+EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overlaps",
+           "afqmc_get_constants", "afqmc_debug_read", "afqmc_launch_count", "afqmc_sync",
+           "afqmc_last_error", "afqmc_destroy", "afqmc_measure_fp64_peak"]
+
+
+class AfqmcParams(C.Structure):
+    _fields_ = [("struct_size", C.c_int32), ("M", C.c_int32), ("n_alpha", C.c_int32),
+                ("n_beta", C.c_int32), ("n_chol", C.c_int32), ("max_walkers", C.c_int32),
+                ("walker_kind", C.c_int32), ("taylor_order", C.c_int32),
+                ("ortho_every", C.c_int32), ("e_shift_auto", C.c_int32),
+                ("e_shift", C.c_double), ("stream", C.c_void_p)]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_2406_16238_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64, dbl = C.c_void_p, C.c_int32, C.c_int64, C.c_double
+    lib.afqmc_create.argtypes = [vp, vp, vp, C.POINTER(AfqmcParams), C.POINTER(vp)]
+    lib.afqmc_create.restype = i32
+    lib.afqmc_step.argtypes = [vp, vp, vp, vp, dbl, i32]
+    lib.afqmc_step.restype = i32
+    lib.afqmc_local_energy.argtypes = [vp, vp, vp, i32]
+    lib.afqmc_local_energy.restype = i32
+    lib.afqmc_get_overlaps.argtypes = [vp, vp]
+    lib.afqmc_get_overlaps.restype = i32
+    lib.afqmc_get_constants.argtypes = [vp, vp]
+    lib.afqmc_get_constants.restype = i32
+    lib.afqmc_debug_read.argtypes = [vp, i32, vp]
+    lib.afqmc_debug_read.restype = i64
+    lib.afqmc_launch_count.argtypes = [vp]
+    lib.afqmc_launch_count.restype = i64
+    lib.afqmc_sync.argtypes = [vp]
+    lib.afqmc_sync.restype = i32
+    lib.afqmc_last_error.argtypes = [vp]
+    lib.afqmc_last_error.restype = C.c_char_p
+    lib.afqmc_destroy.argtypes = [vp]
+    lib.afqmc_destroy.restype = None
+    lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
+    lib.afqmc_measure_fp64_peak.restype = i32
+    return lib
+
+
+lib = _load()
+
+
+class AfqmcError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"libafqmc error {code}: {msg}")
+        self.code = code
+
+
+def _ptr(a):
+    """Raw address of a torch tensor or a NumPy array (must be contiguous)."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        if not a.flags["C_CONTIGUOUS"]:
+            raise ValueError("array must be C-contiguous")
+        return a.ctypes.data
+    if hasattr(a, "data_ptr"):
+        if not a.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return a.data_ptr()
+    raise TypeError(f"unsupported array type {type(a)}")
+
+
+def measure_fp64_peak(ms=200.0):
+    """(DMMA TFLOP/s, DFMA TFLOP/s, SM MHz) from register-only issue loops."""
+    out = np.zeros(3)
+    rc = lib.afqmc_measure_fp64_peak(float(ms), out.ctypes.data)
+    if rc != 0:
+        raise AfqmcError(rc, "afqmc_measure_fp64_peak")
+    return tuple(out)
+
+
+class AFQMC:
+    """Handle wrapper with the same calls as the C ABI."""
+
+    def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
+                 walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None):
+        p = AfqmcParams()
+        p.struct_size = C.sizeof(AfqmcParams)
+        p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
+        p.max_walkers, p.walker_kind = max_walkers, walker_kind
+        p.taylor_order, p.ortho_every = taylor_order, ortho_every
+        p.e_shift_auto = 1 if e_shift is None else 0
+        p.e_shift = 0.0 if e_shift is None else float(e_shift)
+        p.stream = stream
+        self._keep = (h1, L_chol, trial)     # L_chol is borrowed by the library
+        self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers
+        self.Nt = n_alpha if walker_kind == 0 else n_alpha + n_beta
+        h = C.c_void_p()
+        rc = lib.afqmc_create(_ptr(h1), _ptr(L_chol), _ptr(trial), C.byref(p), C.byref(h))
+        if rc != 0:
+            raise AfqmcError(rc, lib.afqmc_last_error(None).decode())
+        self._h = h
+
+    def _check(self, rc):
+        if rc != 0:
+            raise AfqmcError(rc, lib.afqmc_last_error(self._h).decode())
+
+    def step(self, walkers, weights, aux_fields, dt, nw=None):
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_step(self._h, _ptr(walkers), _ptr(weights), _ptr(aux_fields), float(dt), nw))
+
+    def local_energy(self, walkers, E_out, nw=None):
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_local_energy(self._h, _ptr(walkers), _ptr(E_out), nw))
+
+    def get_overlaps(self, out):
+        self._check(lib.afqmc_get_overlaps(self._h, _ptr(out)))
+
+    def constants(self):
+        out = np.zeros(3)
+        self._check(lib.afqmc_get_constants(self._h, out.ctypes.data))
+        return dict(E_const=out[0], e_shift=out[1], e_trial=out[2])
+
+    def debug_read(self, which):
+        n = lib.afqmc_debug_read(self._h, which, None)
+        if n < 0:
+            self._check(int(n))
+        out = np.empty(int(n))
+        r = lib.afqmc_debug_read(self._h, which, out.ctypes.data)
+        if r < 0:
+            self._check(int(r))
+        return out
+
+    def launch_count(self):
+        return int(lib.afqmc_launch_count(self._h))
+
+    def sync(self):
+        self._check(lib.afqmc_sync(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.afqmc_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,519 @@
+// api.cu - the C ABI of libafqmc (include/afqmc.h): handle, setup, and the stream-ordered
+// sequence of kernels that makes one walker step / one local-energy evaluation.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "internal.h"
+
+using namespace afq;
+
+struct afqmc_handle {
+  afqmc_params p;
+  int M = 0, Nt = 0, nblk = 1, off[2] = {0, 0}, ns[2] = {0, 0};
+  int n_chol = 0, maxw = 0, K = 6, rhf = 1;
+  double sf = 2.0;
+  cudaStream_t st = nullptr;
+  bool own_stream = false;
+  const double* L = nullptr;
+  std::vector<void*> allocs;
+  // constants
+  double *h1 = nullptr, *trial = nullptr, *trialT = nullptr, *Lrot = nullptr, *hrot = nullptr;
+  double *m = nullptr, *hmod = nullptr, *E1 = nullptr, *Xs = nullptr, *Pa = nullptr, *Pb = nullptr;
+  double E_const = 0.0, e_shift = 0.0, e_trial = NAN, hmod_norm1 = 0.0, dt_cached = NAN;
+  // per-step workspaces
+  double *det_old = nullptr, *det_new = nullptr, *ThT = nullptr, *Xp = nullptr, *X = nullptr, *Cf = nullptr;
+  double *cfb = nullptr, *cmf = nullptr, *A = nullptr, *T0 = nullptr, *T1 = nullptr, *Acc = nullptr;
+  double *ovlp = nullptr, *detR = nullptr;
+  double *expart[2] = {nullptr, nullptr}, *Xe = nullptr, *e1 = nullptr;
+  int exgroups[2] = {0, 0};
+  // staging for host-pointer calls
+  double *stW = nullptr, *stWt = nullptr, *stX = nullptr, *stE = nullptr;
+  int fb_split = 1;
+  long step_count = 0;
+  int last_nw = 0;
+  int64_t launches = 0;
+  std::string err;
+};
+
+static std::string g_create_err;
+
+namespace {
+
+bool is_device_ptr(const void* p) {
+  cudaPointerAttributes at;
+  cudaError_t e = cudaPointerGetAttributes(&at, p);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  return at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged;
+}
+
+int fail(afqmc_handle* h, int code, const std::string& msg) {
+  if (h) h->err = msg; else g_create_err = msg;
+  return code;
+}
+
+int check_cuda(afqmc_handle* h, const char* where) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, AFQMC_ERR_CUDA, std::string(where) + ": " + cudaGetErrorString(e));
+  return AFQMC_OK;
+}
+
+double* dalloc(afqmc_handle* h, size_t n_doubles) {
+  void* p = nullptr;
+  if (n_doubles == 0) n_doubles = 2;
+  if (cudaMalloc(&p, n_doubles * sizeof(double)) != cudaSuccess) {
+    cudaGetLastError();
+    return nullptr;
+  }
+  h->allocs.push_back(p);
+  return (double*)p;
+}
+
+void dfree_one(afqmc_handle* h, double* p) {
+  for (auto& q : h->allocs)
+    if (q == p) { cudaFree(q); q = nullptr; }
+}
+
+// copy `n` doubles from a host-or-device pointer to a device buffer on the stream
+void to_device(afqmc_handle* h, double* dst, const void* src, size_t n) {
+  cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDefault, h->st);
+}
+
+GemmArgs gemm_args() {
+  GemmArgs a;
+  memset(&a, 0, sizeof(a));
+  a.batch = 1;
+  a.splitK = 1;
+  a.alpha = 1.0;
+  return a;
+}
+
+// E1 = expm(-dt/2 h_mod) by scaling and squaring of a degree-16 Taylor polynomial (Horner),
+// every product on the DMMA GEMM.  (The oracle uses an eigendecomposition instead: reading S6.)
+void build_E1(afqmc_handle* h, double dt) {
+  const int M = h->M;
+  const long MM = (long)M * M;
+  double nrm = 0.5 * fabs(dt) * h->hmod_norm1;
+  int s = 0;
+  while (nrm > 0.25 && s < 40) { nrm *= 0.5; ++s; }
+  h->launches += run_scale_copy(h->Xs, h->hmod, -0.5 * dt / std::ldexp(1.0, s), MM, h->st);
+  h->launches += run_fill(h->Pa, 0.0, MM, h->st);
+  h->launches += run_axpby_identity(h->Pa, 0.0, 1.0, M, h->st);
+  double *P = h->Pa, *Q = h->Pb;
+  for (int k = 16; k >= 1; --k) {
+    GemmArgs g = gemm_args();
+    g.A = h->Xs; g.lda = M; g.B = P; g.ldb = M; g.C = Q; g.ldc = M;
+    g.M = M; g.N = M; g.K = M; g.alpha = 1.0 / k;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+    h->launches += run_axpby_identity(Q, 1.0, 1.0, M, h->st);
+    std::swap(P, Q);
+  }
+  for (int i = 0; i < s; ++i) {
+    GemmArgs g = gemm_args();
+    g.A = P; g.lda = M; g.B = P; g.ldb = M; g.C = Q; g.ldc = M;
+    g.M = M; g.N = M; g.K = M;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+    std::swap(P, Q);
+  }
+  h->launches += run_scale_copy(h->E1, P, 1.0, MM, h->st);
+  h->dt_cached = dt;
+}
+
+OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, int want_e1) {
+  OTArgs a;
+  a.W = W; a.trial = h->trial; a.hrot = h->hrot; a.det = det; a.ThT = h->ThT; a.e1 = h->e1;
+  a.M = h->M; a.Nt = h->Nt; a.nblk = h->nblk;
+  for (int b = 0; b < 2; ++b) { a.off[b] = h->off[b]; a.ns[b] = h->ns[b]; }
+  a.want_theta = want_theta; a.want_e1 = want_e1;
+  return a;
+}
+
+int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
+  h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
+  for (int b = 0; b < h->nblk; ++b) {
+    ExArgs e;
+    e.Lrot = h->Lrot; e.ThT = h->ThT; e.expart = h->expart[b]; e.X = h->Xe;
+    e.M = h->M; e.Nt = h->Nt; e.n_chol = h->n_chol; e.nw = nw;
+    e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
+    h->launches += run_exchange(e, h->st);
+  }
+  EnergyArgs r;
+  r.expart = h->expart[0]; r.ngroups = h->exgroups[0];
+  r.X = h->Xe; r.e1 = h->e1; r.E_out = E_out;
+  r.n_chol = h->n_chol; r.nw = nw; r.nblk = h->nblk; r.spin_factor = h->sf;
+  h->launches += run_energy_reduce2(r, h->nblk > 1 ? h->expart[1] : nullptr, h->exgroups[1], h->st);
+  return AFQMC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* afqmc_last_error(const afqmc_handle* h) { return h ? h->err.c_str() : g_create_err.c_str(); }
+
+void afqmc_destroy(afqmc_handle* h) {
+  if (!h) return;
+  cudaStreamSynchronize(h->st);
+  for (void* p : h->allocs)
+    if (p) cudaFree(p);
+  if (h->own_stream) cudaStreamDestroy(h->st);
+  delete h;
+}
+
+int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial, const afqmc_params* p,
+                     afqmc_handle** out) {
+  if (out) *out = nullptr;
+  if (!h1 || !L_chol || !trial || !p || !out) return fail(nullptr, AFQMC_ERR_INVALID, "null argument");
+  if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
+  if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
+      p->ortho_every < 0 || p->taylor_order < 0 || (p->walker_kind != 0 && p->walker_kind != 1))
+    return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
+  if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
+  if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
+  if (p->n_alpha > p->M || p->n_beta > p->M) return fail(nullptr, AFQMC_ERR_DIMS, "more occupied orbitals than basis functions");
+  if (p->taylor_order > kMaxTaylor) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "taylor_order > 16");
+  if (p->n_alpha > kMaxOcc || p->n_beta > kMaxOcc) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "occupied block > 64 columns");
+  if ((long)p->n_chol * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
+  if (!is_device_ptr(L_chol)) return fail(nullptr, AFQMC_ERR_INVALID, "L_chol must be a device pointer");
+
+  afqmc_handle* h = new (std::nothrow) afqmc_handle();
+  if (!h) return fail(nullptr, AFQMC_ERR_ALLOC, "host allocation failed");
+  h->p = *p;
+  h->M = p->M; h->n_chol = p->n_chol; h->maxw = p->max_walkers;
+  h->K = p->taylor_order ? p->taylor_order : 6;
+  h->rhf = p->walker_kind == 0;
+  h->sf = h->rhf ? 2.0 : 1.0;
+  h->nblk = h->rhf ? 1 : 2;
+  h->off[0] = 0; h->ns[0] = p->n_alpha;
+  h->off[1] = p->n_alpha; h->ns[1] = h->rhf ? 0 : p->n_beta;
+  h->Nt = h->rhf ? p->n_alpha : p->n_alpha + p->n_beta;
+  h->L = L_chol;
+  if (p->stream) {
+    h->st = (cudaStream_t)p->stream;
+  } else {
+    if (cudaStreamCreateWithFlags(&h->st, cudaStreamNonBlocking) != cudaSuccess) {
+      delete h;
+      return fail(nullptr, AFQMC_ERR_CUDA, "cudaStreamCreate failed");
+    }
+    h->own_stream = true;
+  }
+  const int M = h->M, Nt = h->Nt, nc = h->n_chol, mw = h->maxw;
+  const long MM = (long)M * M;
+  auto bail = [&](int code, const std::string& msg) {
+    std::string m2 = msg;
+    afqmc_destroy(h);
+    return fail(nullptr, code, m2);
+  };
+
+  // ---- host copies of the small inputs, checks, P_tot ------------------------------------
+  std::vector<double> th((size_t)M * Nt), hh((size_t)MM);
+  if (cudaMemcpy(th.data(), trial, th.size() * 8, cudaMemcpyDefault) != cudaSuccess ||
+      cudaMemcpy(hh.data(), h1, hh.size() * 8, cudaMemcpyDefault) != cudaSuccess)
+    return bail(AFQMC_ERR_CUDA, "copy of h1/trial failed");
+  for (int b = 0; b < h->nblk; ++b)
+    for (int i = 0; i < h->ns[b]; ++i)
+      for (int j = i; j < h->ns[b]; ++j) {
+        double s = 0.0;
+        for (int q = 0; q < M; ++q) s += th[(size_t)q * Nt + h->off[b] + i] * th[(size_t)q * Nt + h->off[b] + j];
+        if (!(fabs(s - (i == j ? 1.0 : 0.0)) <= 1e-10)) return bail(AFQMC_ERR_TRIAL, "trial columns are not orthonormal to 1e-10");
+      }
+  std::vector<double> P((size_t)MM, 0.0), tT((size_t)Nt * M);
+  for (int q = 0; q < M; ++q)
+    for (int i = 0; i < Nt; ++i) tT[(size_t)i * M + q] = th[(size_t)q * Nt + i];
+  for (int i = 0; i < Nt; ++i)
+    for (int a = 0; a < M; ++a) {
+      const double f = h->sf * tT[(size_t)i * M + a];
+      if (f == 0.0) continue;
+      for (int c = 0; c < M; ++c) P[(size_t)a * M + c] += f * tT[(size_t)i * M + c];
+    }
+
+  // ---- device constants ---------------------------------------------------------------
+  h->h1 = dalloc(h, MM); h->trial = dalloc(h, (size_t)M * Nt); h->trialT = dalloc(h, (size_t)Nt * M);
+  h->Lrot = dalloc(h, (size_t)nc * Nt * M); h->hrot = dalloc(h, (size_t)Nt * M); h->m = dalloc(h, nc);
+  h->hmod = dalloc(h, MM); h->E1 = dalloc(h, MM); h->Xs = dalloc(h, MM); h->Pa = dalloc(h, MM); h->Pb = dalloc(h, MM);
+  double* dP = dalloc(h, MM);
+  double* mL = dalloc(h, MM);
+  if (!h->h1 || !h->trial || !h->trialT || !h->Lrot || !h->hrot || !h->m || !h->hmod || !h->E1 || !h->Xs ||
+      !h->Pa || !h->Pb || !dP || !mL)
+    return bail(AFQMC_ERR_ALLOC, "device allocation failed (constants)");
+  cudaMemcpyAsync(h->h1, hh.data(), MM * 8, cudaMemcpyHostToDevice, h->st);
+  cudaMemcpyAsync(h->trial, th.data(), th.size() * 8, cudaMemcpyHostToDevice, h->st);
+  cudaMemcpyAsync(h->trialT, tT.data(), tT.size() * 8, cudaMemcpyHostToDevice, h->st);
+  cudaMemcpyAsync(dP, P.data(), MM * 8, cudaMemcpyHostToDevice, h->st);
+
+  // m_g = tr(L_g P_tot); mL = sum_g m_g L_g
+  h->launches += run_mean_field(h->L, dP, h->m, M, nc, h->st);
+  h->launches += run_sum_mL(h->L, h->m, mL, M, nc, h->st);
+  // sum_g L_g L_g = L2d^T L2d with L2d = L viewed as [(g,k)][M] (L_g symmetric), split over K
+  {
+    const int tiles = ((M + 127) / 128) * ((M + 127) / 128);
+    int split = (296 + tiles - 1) / tiles;
+    if (split > 32) split = 32;
+    if (split < 1) split = 1;
+    double* part = dalloc(h, (size_t)split * MM);
+    if (!part) return bail(AFQMC_ERR_ALLOC, "device allocation failed (setup)");
+    GemmArgs g = gemm_args();
+    g.A = h->L; g.lda = M; g.B = h->L; g.ldb = M; g.C = part; g.ldc = M;
+    g.M = M; g.N = M; g.K = nc * M; g.splitK = split; g.sCsplit = MM;
+    h->launches += run_gemm(GEMM_KMKN, g, h->st);
+    h->launches += run_hmod(h->h1, part, split, mL, h->hmod, M, h->st);
+    cudaStreamSynchronize(h->st);
+    dfree_one(h, part);
+  }
+  // half rotation: Lrot[g] = trial^T L_g ; hrot = trial^T h1
+  {
+    GemmArgs g = gemm_args();
+    g.A = h->trialT; g.lda = M; g.sA = 0; g.B = h->L; g.ldb = M; g.sB = MM;
+    g.C = h->Lrot; g.ldc = M; g.sC = (long)Nt * M; g.M = Nt; g.N = M; g.K = M; g.batch = nc;
+    // grid.z limit: batch in chunks of 32768
+    for (int b0 = 0; b0 < nc; b0 += 32768) {
+      GemmArgs gg = g;
+      gg.B = g.B + (size_t)b0 * MM; gg.C = g.C + (size_t)b0 * Nt * M; gg.batch = std::min(32768, nc - b0);
+      h->launches += run_gemm(GEMM_KN, gg, h->st);
+    }
+    GemmArgs g2 = gemm_args();
+    g2.A = h->trialT; g2.lda = M; g2.B = h->h1; g2.ldb = M; g2.C = h->hrot; g2.ldc = M;
+    g2.M = Nt; g2.N = M; g2.K = M;
+    h->launches += run_gemm(GEMM_KN, g2, h->st);
+  }
+  // E_const and the 1-norm of h_mod on the host
+  {
+    std::vector<double> mh(nc), hm((size_t)MM);
+    cudaMemcpyAsync(mh.data(), h->m, nc * 8, cudaMemcpyDeviceToHost, h->st);
+    cudaMemcpyAsync(hm.data(), h->hmod, MM * 8, cudaMemcpyDeviceToHost, h->st);
+    if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, std::string("setup kernels failed: ") + cudaGetErrorString(cudaPeekAtLastError()));
+    double s = 0.0;
+    for (int g = 0; g < nc; ++g) s += mh[g] * mh[g];
+    h->E_const = -0.5 * s;
+    double n1 = 0.0;
+    for (int c = 0; c < M; ++c) {
+      double cs = 0.0;
+      for (int r = 0; r < M; ++r) cs += fabs(hm[(size_t)r * M + c]);
+      if (cs > n1) n1 = cs;
+    }
+    h->hmod_norm1 = n1;
+  }
+  dfree_one(h, dP);
+  dfree_one(h, mL);
+
+  // ---- workspaces ----------------------------------------------------------------------
+  {
+    const int tiles = ((2 * mw + 127) / 128) * ((nc + 127) / 128);
+    int split = (296 + tiles - 1) / tiles;
+    const int kmax = std::max(1, (Nt * M) / 512);
+    if (split > kmax) split = kmax;
+    if (split > 16) split = 16;
+    if (split < 1) split = 1;
+    h->fb_split = split;
+  }
+  const size_t wsz = (size_t)mw * M * 2 * Nt;
+  h->det_old = dalloc(h, (size_t)mw * 2 * 2); h->det_new = dalloc(h, (size_t)mw * 2 * 2);
+  h->ThT = dalloc(h, wsz); h->Xp = dalloc(h, (size_t)h->fb_split * 2 * mw * nc);
+  h->X = dalloc(h, (size_t)2 * mw * nc); h->Cf = dalloc(h, (size_t)2 * mw * nc);
+  h->cfb = dalloc(h, 2 * mw); h->cmf = dalloc(h, 2 * mw);
+  h->A = dalloc(h, (size_t)mw * 2 * MM);
+  h->T0 = dalloc(h, wsz); h->T1 = dalloc(h, wsz); h->Acc = dalloc(h, wsz);
+  h->ovlp = dalloc(h, 2 * mw); h->detR = dalloc(h, 2 * mw);
+  for (int b = 0; b < h->nblk; ++b) {
+    const int G = exchange_group_size(h->ns[b]);
+    h->exgroups[b] = (nc + G - 1) / G;
+    h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mw * 2);
+  }
+  h->Xe = dalloc(h, (size_t)nc * mw * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
+  h->stW = dalloc(h, wsz); h->stWt = dalloc(h, mw); h->stX = dalloc(h, (size_t)mw * nc); h->stE = dalloc(h, (size_t)mw * 6);
+  if (!h->det_old || !h->det_new || !h->ThT || !h->Xp || !h->X || !h->Cf || !h->cfb || !h->cmf || !h->A ||
+      !h->T0 || !h->T1 || !h->Acc || !h->ovlp || !h->detR || !h->expart[0] || (h->nblk > 1 && !h->expart[1]) ||
+      !h->Xe || !h->e1 || !h->stW || !h->stWt || !h->stX || !h->stE)
+    return bail(AFQMC_ERR_ALLOC, "device allocation failed (workspaces)");
+
+  // ---- E_shift = trial energy ---------------------------------------------------------------
+  {
+    std::vector<double> wt((size_t)M * Nt * 2, 0.0);
+    for (size_t i = 0; i < th.size(); ++i) wt[2 * i] = th[i];
+    cudaMemcpyAsync(h->stW, wt.data(), wt.size() * 8, cudaMemcpyHostToDevice, h->st);
+    local_energy_device(h, h->stW, h->stE, 1);
+    double e[6];
+    cudaMemcpyAsync(e, h->stE, 48, cudaMemcpyDeviceToHost, h->st);
+    if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, std::string("trial energy failed: ") + cudaGetErrorString(cudaPeekAtLastError()));
+    h->e_trial = e[0];
+  }
+  h->e_shift = p->e_shift_auto ? h->e_trial : p->e_shift;
+  *out = h;
+  return AFQMC_OK;
+}
+
+int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
+  const int M = h->M, Nt = h->Nt, nc = h->n_chol;
+  const long MM = (long)M * M;
+  const size_t wlen = (size_t)nw * M * 2 * Nt;
+  const bool hostW = !is_device_ptr(walkers), hostWt = !is_device_ptr(weights), hostX = !is_device_ptr(aux_fields);
+  double* W = (double*)walkers;
+  double* wt = weights;
+  const double* x = aux_fields;
+  if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
+  if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
+  if (hostX) { to_device(h, h->stX, aux_fields, (size_t)nw * nc); x = h->stX; }
+
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
+
+  // a1/a2: overlap, Theta
+  h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+  // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
+  {
+    GemmArgs g = gemm_args();
+    g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
+    g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
+    g.splitK = h->fb_split; g.sCsplit = (long)2 * h->maxw * nc;
+    h->launches += run_gemm(GEMM_NK, g, h->st);
+  }
+  // a4: shifted fields, scalars, V_HS coefficients
+  {
+    ShiftArgs s;
+    s.Xp = h->Xp; s.sXp = (long)2 * h->maxw * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
+    s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
+    s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
+    h->launches += run_field_shift(s, nw, h->st);
+  }
+  // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
+  {
+    GemmArgs g = gemm_args();
+    g.A = h->Cf; g.lda = nc; g.B = h->L; g.ldb = MM; g.C = h->A; g.ldc = MM;
+    g.M = 2 * nw; g.N = (int)MM; g.K = nc;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+  }
+  // a6: T0 = Acc = E1 phi
+  const long wstride = (long)M * 2 * Nt;
+  {
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
+    g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+  }
+  // a7: T_n = A T_{n-1} / n, Acc += T_n
+  {
+    double *Tp = h->T0, *Tn = h->T1;
+    for (int n = 1; n <= h->K; ++n) {
+      GemmArgs g = gemm_args();
+      g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
+      g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
+      g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
+      h->launches += run_gemm(GEMM_CPLX_KN, g, h->st);
+      std::swap(Tp, Tn);
+    }
+  }
+  // a8: phi = E1 Acc, written into the caller's walkers
+  {
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+  }
+  // a9: new overlap and weights
+  h->launches += run_overlap_theta(ot_args(h, W, h->det_new, 0, 0), nw, h->st);
+  {
+    WeightArgs a;
+    a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = h->cfb; a.cmf = h->cmf;
+    a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
+    a.expo = -dt * (h->E_const - h->e_shift);
+    h->launches += run_weight_update(a, nw, h->st);
+  }
+  // a10: re-orthonormalisation
+  h->step_count += 1;
+  h->last_nw = nw;
+  if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) {
+    QRArgs q;
+    q.W = W; q.detR = h->detR; q.M = M; q.Nt = Nt; q.nblk = h->nblk;
+    for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
+    h->launches += run_fill(h->detR, 1.0, (long)nw * h->nblk, h->st);
+    h->launches += run_cholqr_pass(q, nw, h->st);
+    h->launches += run_cholqr_pass(q, nw, h->st);
+    h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
+  }
+  if (hostW) cudaMemcpyAsync(walkers, W, wlen * 8, cudaMemcpyDeviceToHost, h->st);
+  if (hostWt) cudaMemcpyAsync(weights, wt, (size_t)nw * 8, cudaMemcpyDeviceToHost, h->st);
+  if (hostW || hostWt) {
+    if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_step");
+  }
+  return check_cuda(h, "afqmc_step");
+}
+
+int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, int32_t nw) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!walkers || !E_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
+  const bool hostW = !is_device_ptr(walkers), hostE = !is_device_ptr(E_out);
+  const double* W = (const double*)walkers;
+  double* E = (double*)E_out;
+  if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
+  if (hostE) E = h->stE;
+  local_energy_device(h, W, E, nw);
+  if (hostE) {
+    cudaMemcpyAsync(E_out, E, (size_t)nw * 48, cudaMemcpyDeviceToHost, h->st);
+    if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_local_energy");
+  }
+  return check_cuda(h, "afqmc_local_energy");
+}
+
+int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!ovlp_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (h->last_nw <= 0) return fail(h, AFQMC_ERR_INVALID, "no step has been taken");
+  const bool host = !is_device_ptr(ovlp_out);
+  cudaMemcpyAsync(ovlp_out, h->ovlp, (size_t)h->last_nw * 16, cudaMemcpyDefault, h->st);
+  if (host && cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_get_overlaps");
+  return check_cuda(h, "afqmc_get_overlaps");
+}
+
+int32_t afqmc_get_constants(afqmc_handle* h, double* out3) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!out3) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  out3[0] = h->E_const; out3[1] = h->e_shift; out3[2] = h->e_trial;
+  return AFQMC_OK;
+}
+
+int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
+  if (!h) return AFQMC_ERR_INVALID;
+  const double* src = nullptr;
+  int64_t n = 0;
+  const long MM = (long)h->M * h->M;
+  const int nw = h->last_nw;
+  switch (which) {
+    case 0: src = h->X; n = (int64_t)2 * nw * h->n_chol; break;
+    case 1: src = h->A; n = (int64_t)2 * nw * MM; break;
+    case 2: src = h->E1; n = MM; break;
+    case 3: src = h->hmod; n = MM; break;
+    case 4: src = h->m; n = h->n_chol; break;
+    case 5: src = h->Lrot; n = (int64_t)h->n_chol * h->Nt * h->M; break;
+    default: return fail(h, AFQMC_ERR_INVALID, "unknown debug array");
+  }
+  if (!out) return n;
+  cudaMemcpyAsync(out, src, (size_t)n * 8, cudaMemcpyDefault, h->st);
+  if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_debug_read");
+  int rc = check_cuda(h, "afqmc_debug_read");
+  return rc == AFQMC_OK ? n : rc;
+}
+
+int64_t afqmc_launch_count(const afqmc_handle* h) { return h ? h->launches : -1; }
+
+int32_t afqmc_sync(afqmc_handle* h) {
+  if (!h) return AFQMC_ERR_INVALID;
+  cudaError_t e = cudaStreamSynchronize(h->st);
+  if (e != cudaSuccess) return fail(h, AFQMC_ERR_CUDA, std::string("sync: ") + cudaGetErrorString(e));
+  return check_cuda(h, "afqmc_sync");
+}
+
+}  // extern "C"

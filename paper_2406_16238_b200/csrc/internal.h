@@ -1,0 +1,106 @@
+// internal.h - declarations shared by the translation units of libafqmc (not installed).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+
+#include "../../include/afqmc.h"
+#include "gemm.cuh"
+
+namespace afq {
+
+constexpr int kMaxOcc = 64;     // largest occupied block (columns per spin) supported
+constexpr int kMaxTaylor = 16;
+
+enum GemmKind { GEMM_KN = 0, GEMM_NK = 1, GEMM_KMKN = 2, GEMM_CPLX_KN = 3 };
+
+// gemm.cu
+// Fills the vec* fields, picks a tile configuration and launches.  Returns launches issued.
+int run_gemm(GemmKind kind, GemmArgs a, cudaStream_t st);
+
+// small.cu ---------------------------------------------------------------------------------
+struct OTArgs {                 // overlap / Theta / one-body energy, one CTA per (block, walker)
+  const double* W;              // walkers as doubles [nw][M][2*Nt]
+  const double* trial;          // [M][Nt]
+  const double* hrot;           // [Nt][M] (only with want_e1)
+  double* det;                  // [nw][nblk] complex: det(psi_s^T phi_s)
+  double* ThT;                  // [nw][2][Nt][M] planar transpose of Theta (want_theta)
+  double* e1;                   // [nw][nblk] complex partial one-body energy (want_e1)
+  int M, Nt, nblk;
+  int off[2], ns[2];
+  int want_theta, want_e1;
+};
+int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st);
+
+struct ShiftArgs {              // a4: force bias -> shifted fields and scalars, one CTA per walker
+  const double* Xp;             // [splitK][2*nw][n_chol] partial sums of X (planar re/im rows)
+  long sXp;                     // stride between partial slices
+  int nsplit;
+  const double* m;              // [n_chol]
+  const double* x;              // [nw][n_chol] aux fields
+  double* X;                    // [nw][2][n_chol] summed X incl. spin factor (kept for diagnostics)
+  double* Cf;                   // [nw][2][n_chol]: rows of the V_HS GEMM: (sqrt(dt) Im xs, -sqrt(dt) Re xs)
+  double* cfb;                  // [nw] complex
+  double* cmf;                  // [nw] complex
+  int n_chol;
+  double spin_factor, sqrt_dt;
+};
+int run_field_shift(const ShiftArgs& a, int nw, cudaStream_t st);
+
+struct WeightArgs {
+  const double* det_old;        // [nw][nblk] complex
+  const double* det_new;        // [nw][nblk] complex
+  const double* cfb;
+  const double* cmf;
+  double* weights;              // [nw] in/out
+  double* ovlp;                 // [nw] complex out: overlap of the new walkers
+  int nblk, rhf;
+  double expo;                  // -dt (E_const - E_shift)
+};
+int run_weight_update(const WeightArgs& a, int nw, cudaStream_t st);
+
+struct QRArgs {                 // one Cholesky-QR pass per (block, walker), in place
+  double* W;                    // [nw][M][2*Nt]
+  double* detR;                 // [nw][nblk] real: multiplied by prod diag(R) of this pass
+  int M, Nt, nblk;
+  int off[2], ns[2];
+};
+int run_cholqr_pass(const QRArgs& a, int nw, cudaStream_t st);
+int run_ovlp_div_detR(double* ovlp, const double* detR, int nblk, int rhf, int nw, cudaStream_t st);
+int run_fill(double* p, double v, long n, cudaStream_t st);
+
+// exchange.cu ------------------------------------------------------------------------------
+struct ExArgs {
+  const double* Lrot;           // [n_chol][Nt][M]
+  const double* ThT;            // [nw][2][Nt][M]
+  double* expart;               // [ngroups][nw] complex: sum over the group's g of tr(T T)
+  double* X;                    // [n_chol][nw] complex: tr(T_g) (accumulated over spin blocks)
+  int M, Nt, n_chol, nw;
+  int off, ns;                  // spin block
+  int accumulate;               // 1: add to expart / X (second spin block)
+};
+int exchange_group_size(int ns);            // gamma per CTA tile for this block size
+int run_exchange(const ExArgs& a, cudaStream_t st);
+
+struct EnergyArgs {
+  const double* expart; int ngroups;
+  const double* X;              // [n_chol][nw] complex
+  const double* e1;             // [nw][nblk] complex
+  double* E_out;                // [nw][3] complex
+  int n_chol, nw, nblk;
+  double spin_factor;
+};
+int run_energy_reduce(const EnergyArgs& a, cudaStream_t st);
+int run_energy_reduce2(const EnergyArgs& a, const double* expart2, int ngroups2, cudaStream_t st);
+
+// setup.cu ---------------------------------------------------------------------------------
+int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);
+int run_sum_mL(const double* L, const double* m, double* out, int M, int n_chol, cudaStream_t st);
+// hmod = h1 - 0.5 * sum_s part[s] + mL
+int run_hmod(const double* h1, const double* part, int nsplit, const double* mL, double* hmod, int M,
+             cudaStream_t st);
+int run_axpby_identity(double* P, double a, double idval, int M, cudaStream_t st);  // P = a P + idval I
+int run_scale_copy(double* dst, const double* src, double a, long n, cudaStream_t st);
+
+}  // namespace afq
