@@ -1,0 +1,344 @@
+"""bench.py - walker-steps/s of the ph-AFQMC hot path (one step = afqmc_step + afqmc_local_energy
+over one batch of Nw synthetic walkers) on B200, with the roofline of the dominant kernel and
+the CPU oracle timed beside it.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c5] [--impl reference]
+
+Multi-GPU (torchrun, one rank per GPU): replicas only - every rank holds its own copy of the
+Hamiltonian and its own Nw walkers, no data-path collective; the value
+is N * Nw * K / max-over-ranks time, scaling "weak".
+
+Timed region of `value`: inputs resident in HBM (walkers, weights, all aux fields pre-staged),
+K x (afqmc_step, afqmc_local_energy) on one stream, CUDA events on that stream.  `e2e`: the
+same K steps through the same C-ABI calls with pinned HOST buffers (the library stages H2D /
+D2H inside each call).  The Cholesky tensor (13.7 GB at c4, 55 GB at c5) is far larger than the
+126 MB L2, so no explicit L2 flush is needed between iterations (config.l2: "inputs > L2").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "walker-steps/s (propagate + local energy)"
+UNIT = "walker-steps/s"
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
+# `ncu --set full` captures summarised under profiles/ (file named beside each number).
+NCU_TRAFFIC = {}
+
+
+def flops_model(cfg, nw):
+    """Algorithmic real FP64 flops per launch of each contraction stage."""
+    M, ng, K = cfg.M, cfg.n_chol, cfg.taylor_order
+    blocks = [cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta]
+    Nt = sum(blocks)
+    return {
+        "exchange": nw * sum(4.0 * ng * ns * ns * M + 8.0 * ng * ns * ns for ns in blocks),
+        "vhs": nw * 4.0 * ng * M * M,
+        "taylor": nw * 8.0 * K * M * M * Nt,
+        "force_bias": nw * 4.0 * ng * Nt * M,
+        "one_body": 2 * nw * 4.0 * M * M * Nt,
+    }
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "200"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            pass
+
+    def stop(self):
+        out = {"sm_mhz": None, "sm_max_mhz": None, "reasons": []}
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush()
+        self.f.seek(0)
+        rows = [r.split(",") for r in self.f.read().strip().splitlines() if r.count(",") >= 6]
+        self.f.close()
+        os.unlink(self.f.name)
+        if not rows:
+            return out
+        sm = [float(r[0]) for r in rows]
+        out["sm_mhz"] = float(np.median(sm))
+        out["sm_max_mhz"] = float(rows[0][1])
+        out["power_w_max"] = max(float(r[2]) for r in rows)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        out["reasons"] = [n for i, n in enumerate(names) if any("Not" not in r[3 + i] for r in rows)]
+        out["samples"] = len(rows)
+        return out
+
+
+def oracle_sample(cfg, h1, L_host, trial, nw_s, steps, warmup, seed=0):
+    """Times the oracle as it stands on `nw_s` walkers: `steps` x (step + local energy).
+    Returns (walker-steps/s, seconds per sample step, threads)."""
+    from oracle.afqmc_oracle import AFQMCOracle
+    from paper_2406_16238_b200 import inputs
+    o = AFQMCOracle(h1, L_host, trial, cfg.n_alpha, cfg.n_beta, cfg.walker_kind,
+                    taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every)
+    W = inputs.make_walkers(cfg, trial, seed, nw_s)
+    wt = np.ones(nw_s)
+    ts = []
+    for s in range(warmup + steps):
+        x = inputs.make_aux_fields(cfg, seed, s, nw_s)
+        t0 = time.perf_counter()
+        W, wt, _ = o.step(W, wt, x, cfg.dt)
+        o.local_energy(W)
+        ts.append(time.perf_counter() - t0)
+    t = float(np.sum(ts[warmup:]))
+    try:
+        import threadpoolctl
+        thr = max([p["num_threads"] for p in threadpoolctl.threadpool_info()] + [1])
+    except Exception:
+        thr = os.cpu_count()
+    return nw_s * steps / t, t / steps, thr
+
+
+def sample_walkers(cfg):
+    """Bounded oracle sample: about 10-30 s of CPU work per bench run."""
+    return {"c1": 16, "c2": 64, "c3": 8, "c4": 4, "c5": 4}.get(cfg.name, 4)
+
+
+def make_L(cfg, seed, want_host, want_dev):
+    """(L_dev or None, L_host or None): host recipe for small configs, device recipe beyond 1 GB."""
+    import torch
+    from paper_2406_16238_b200 import inputs
+    big = cfg.n_chol * cfg.M * cfg.M * 8 > (1 << 30)
+    if big and torch.cuda.is_available():
+        Ld = inputs.make_L_device(cfg, seed)
+        Lh = Ld.cpu().numpy() if want_host else None
+        return (Ld if want_dev else None), Lh
+    Lh = inputs.make_L_host(cfg, seed)
+    Ld = torch.from_numpy(Lh).cuda() if want_dev else None
+    return Ld, (Lh if want_host else None)
+
+
+def run_reference(args, cfg, rank):
+    """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload."""
+    if rank != 0:
+        return
+    from paper_2406_16238_b200 import inputs
+    h1 = inputs.make_h1(cfg, 0)
+    trial = inputs.make_trial(cfg, h1, 0)
+    _, Lh = make_L(cfg, 0, True, False)
+    nw_s = sample_walkers(cfg)
+    v, sec, thr = oracle_sample(cfg, h1, Lh, trial, nw_s, args.steps, args.warmup)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic",
+        "config": {"workload": cfg.name, "M": cfg.M, "n_alpha": cfg.n_alpha, "n_beta": cfg.n_beta,
+                   "n_chol": cfg.n_chol, "n_walkers": nw_s, "dt": cfg.dt,
+                   "taylor_order": cfg.taylor_order},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+                         "sample": f"{nw_s} of {cfg.nw} walkers x {args.steps} steps (step + local energy)"},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+
+    import torch
+    from paper_2406_16238_b200 import inputs
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = inputs.get_config(args.workload)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+
+    from paper_2406_16238_b200 import afqmc
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+
+    K, Wm, nw = args.steps, args.warmup, cfg.nw
+    seed = rank           # every replica draws its own walkers / fields; same Hamiltonian shape
+    h1 = inputs.make_h1(cfg, 0)
+    trial = inputs.make_trial(cfg, h1, 0)
+    want_cpu = (rank == 0 and world == 1 and not args.no_cpu_baseline)
+    Ld, _ = make_L(cfg, 0, False, True)
+    stream = torch.cuda.Stream()
+    g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta,
+                    n_chol=cfg.n_chol, max_walkers=nw, walker_kind=cfg.walker_kind,
+                    taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every,
+                    stream=stream.cuda_stream)
+    peak_dmma, peak_dfma, _ = afqmc.measure_fp64_peak(200.0)
+
+    walkers_h = inputs.make_walkers(cfg, trial, seed, nw)
+    xs_h = np.stack([inputs.make_aux_fields(cfg, seed, s, nw) for s in range(Wm + K)])
+    with torch.cuda.stream(stream):
+        W = torch.from_numpy(walkers_h).cuda()
+        wt = torch.ones(nw, dtype=torch.float64, device="cuda")
+        xs = torch.from_numpy(xs_h).cuda()
+        E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+
+        def one(s):
+            g.step(W, wt, xs[s], cfg.dt)
+            g.local_energy(W, E)
+
+        for s in range(Wm):
+            one(s)
+        g.sync()
+        g.set_profiling(True)
+        g.stage_times(reset=True)
+        l0 = g.launch_count()
+        barrier()
+        torch.cuda.synchronize()
+        clk = ClockSampler(local)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for s in range(Wm, Wm + K):
+            one(s)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        barrier()
+        clocks = clk.stop()
+        ms = e0.elapsed_time(e1)
+        launches = g.launch_count() - l0
+        stages = g.stage_times(reset=True)
+        g.set_profiling(False)
+        E_last = E.cpu().numpy()
+        wt_last = wt.cpu().numpy()
+
+    tmax = ms
+    if dist is not None:
+        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        tmax = float(t.item())
+    value = world * nw * K / (tmax * 1e-3)
+
+    # ---- end to end through the C ABI with pinned host buffers ---------------------------------
+    e2e = None
+    if not args.no_e2e:
+        Wp = torch.from_numpy(walkers_h.copy()).pin_memory()
+        wp = torch.ones(nw, dtype=torch.float64).pin_memory()
+        xp = torch.from_numpy(xs_h).pin_memory()
+        Ep = torch.empty((nw, 3), dtype=torch.complex128).pin_memory()
+        Wn, wn, En = Wp.numpy(), wp.numpy(), Ep.numpy()
+
+        def one_host(s):
+            g.step(Wn, wn, xp[s].numpy(), cfg.dt)
+            g.local_energy(Wn, En)
+
+        for s in range(min(Wm, 2)):
+            one_host(s)
+        barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        for s in range(Wm, Wm + K):
+            one_host(s)
+        g.sync()
+        t_e2e = time.perf_counter() - t0
+        barrier()
+        if dist is not None:
+            t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            t_e2e = float(t.item())
+        wbytes = Wn.nbytes
+        e2e = {"value": world * nw * K / t_e2e, "unit": UNIT,
+               "h2d_bytes_per_step": int(2 * wbytes + wn.nbytes + xp[0].numpy().nbytes),
+               "d2h_bytes_per_step": int(wbytes + wn.nbytes + En.nbytes)}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel -------------------------------------------------------
+    fl = flops_model(cfg, nw)
+    per_stage = {k: {"ms_per_step": v[0] / K, "launches": v[1]} for k, v in stages.items() if v[1]}
+    for k, f in fl.items():
+        if k in per_stage and per_stage[k]["ms_per_step"] > 0:
+            tf = f / (per_stage[k]["ms_per_step"] * 1e-3) / 1e12
+            per_stage[k]["tflops"] = tf
+            per_stage[k]["frac_of_dmma_peak"] = tf / peak_dmma
+    dom = max(per_stage, key=lambda k: per_stage[k]["ms_per_step"])
+    nl = {"exchange": 1 if cfg.walker_kind == 0 else 2, "taylor": cfg.taylor_order, "one_body": 2}.get(dom, 1)
+    roof = {"kernel": dom, "bound": "tensor", "unit": "TFLOP/s", "peak": peak_dmma,
+            "peak_source": "FP64 DMMA issue rate measured on this GPU by afqmc_measure_fp64_peak "
+                           "(register-only mma.sync.m8n8k4.f64 loop, 200 ms); MEASURED_PEAKS.json has "
+                           "no FP64 entry",
+            "achieved": per_stage[dom].get("tflops"), "frac": per_stage[dom].get("frac_of_dmma_peak"),
+            "flops_per_launch": fl.get(dom, 0.0) / nl,
+            "ms_per_launch": per_stage[dom]["ms_per_step"] / nl,
+            "share_of_step": per_stage[dom]["ms_per_step"] / (tmax / K),
+            "traffic": NCU_TRAFFIC.get((cfg.name, dom))}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+        "ms_per_step": tmax / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg.name, "M": cfg.M, "n_alpha": cfg.n_alpha, "n_beta": cfg.n_beta,
+                   "n_chol": cfg.n_chol, "n_walkers_per_gpu": nw, "dt": cfg.dt,
+                   "taylor_order": cfg.taylor_order, "ortho_every": cfg.ortho_every,
+                   "local_energy": "every step", "parallelism": f"replicas x{world}",
+                   "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "roofline": roof, "stages": per_stage,
+        "fp64_peaks_measured": {"dmma_tflops": peak_dmma, "dfma_tflops": peak_dfma},
+        "check": {"E_mean_real": float(np.mean(E_last[:, 0].real)), "weights_min": float(wt_last.min()),
+                  "weights_max": float(wt_last.max())},
+    }
+
+    if want_cpu:
+        g.close()
+        Lh = Ld.cpu().numpy()
+        del Ld
+        torch.cuda.empty_cache()
+        nw_s = sample_walkers(cfg)
+        v, sec, thr = oracle_sample(cfg, h1, Lh, trial, nw_s, 1, 0)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
+                                "sample": f"{nw_s} of {nw} walkers x 1 step (step + local energy), {sec:.1f} s"}
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

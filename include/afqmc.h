@@ -114,6 +114,30 @@ int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out);
 /* Number of kernel launches issued by this handle since create (for bench.py). */
 int64_t afqmc_launch_count(const afqmc_handle* h);
 
+/* Per-stage device timing (for bench.py's roofline figures; off by default).  With profiling on,
+ * every stage of afqmc_step / afqmc_local_energy is bracketed by two CUDA events recorded on the
+ * handle's stream (no synchronisation is added).  afqmc_get_stage_times synchronises the stream,
+ * adds the elapsed time of every bracket recorded since the last call to running totals and
+ * writes totals (milliseconds) and bracket counts; reset != 0 clears the totals afterwards.
+ * Stage indices: */
+#define AFQMC_STAGE_OVERLAP_THETA 0  /* a1/a2 overlap, inverse, Theta (step)                  */
+#define AFQMC_STAGE_FORCE_BIAS 1     /* a3 GEMM                                               */
+#define AFQMC_STAGE_FIELD_SHIFT 2    /* a4                                                    */
+#define AFQMC_STAGE_VHS 3            /* a5 GEMM over the Cholesky index                       */
+#define AFQMC_STAGE_ONE_BODY 4       /* a6 + a8                                               */
+#define AFQMC_STAGE_TAYLOR 5         /* a7, all orders                                        */
+#define AFQMC_STAGE_OVERLAP_NEW 6    /* a9 overlap of the propagated walkers                  */
+#define AFQMC_STAGE_WEIGHT 7         /* a9 weight update                                      */
+#define AFQMC_STAGE_REORTHO 8        /* a10                                                   */
+#define AFQMC_STAGE_E_THETA 9        /* a11: overlap, Theta, one-body energy                  */
+#define AFQMC_STAGE_EXCHANGE 10      /* a11: T = Lrot Theta, tr(TT), tr(T)                    */
+#define AFQMC_STAGE_E_REDUCE 11      /* a11: Coulomb sum and final energies                   */
+#define AFQMC_STAGE_E1_BUILD 12      /* expm(-dt/2 h_mod), only when dt changes               */
+#define AFQMC_STAGE_COUNT 13
+int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on);
+/*   ms_out HOST double [AFQMC_STAGE_COUNT]; count_out HOST int64 [AFQMC_STAGE_COUNT] or NULL. */
+int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset);
+
 /* Stream synchronise and surface any deferred CUDA error. */
 int32_t afqmc_sync(afqmc_handle* h);
 

@@ -17,7 +17,11 @@ LIB_PATH = os.path.join(_HERE, "libafqmc.so")
 
 EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overlaps",
            "afqmc_get_constants", "afqmc_debug_read", "afqmc_launch_count", "afqmc_sync",
-           "afqmc_last_error", "afqmc_destroy", "afqmc_measure_fp64_peak"]
+           "afqmc_last_error", "afqmc_destroy", "afqmc_measure_fp64_peak", "afqmc_set_profiling",
+           "afqmc_get_stage_times"]
+
+STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
+          "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build"]
 
 
 class AfqmcParams(C.Structure):
@@ -54,6 +58,10 @@ def _load():
     lib.afqmc_last_error.restype = C.c_char_p
     lib.afqmc_destroy.argtypes = [vp]
     lib.afqmc_destroy.restype = None
+    lib.afqmc_set_profiling.argtypes = [vp, i32]
+    lib.afqmc_set_profiling.restype = i32
+    lib.afqmc_get_stage_times.argtypes = [vp, vp, vp, i32]
+    lib.afqmc_get_stage_times.restype = i32
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
     return lib
@@ -143,6 +151,16 @@ class AFQMC:
         if r < 0:
             self._check(int(r))
         return out
+
+    def set_profiling(self, on):
+        self._check(lib.afqmc_set_profiling(self._h, 1 if on else 0))
+
+    def stage_times(self, reset=False):
+        """{stage: (total ms, brackets)} since the last reset (synchronises the stream)."""
+        ms = np.zeros(len(STAGES))
+        n = np.zeros(len(STAGES), dtype=np.int64)
+        self._check(lib.afqmc_get_stage_times(self._h, ms.ctypes.data, n.ctypes.data, 1 if reset else 0))
+        return {k: (float(ms[i]), int(n[i])) for i, k in enumerate(STAGES)}
 
     def launch_count(self):
         return int(lib.afqmc_launch_count(self._h))

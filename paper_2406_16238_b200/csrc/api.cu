@@ -37,6 +37,13 @@ struct afqmc_handle {
   int last_nw = 0;
   int64_t launches = 0;
   std::string err;
+  // per-stage event timing (afqmc_set_profiling)
+  bool prof = false;
+  std::vector<cudaEvent_t> ev_free;
+  struct Bracket { int stage; cudaEvent_t a, b; };
+  std::vector<Bracket> ev_pending;
+  double stage_ms[AFQMC_STAGE_COUNT] = {0};
+  int64_t stage_n[AFQMC_STAGE_COUNT] = {0};
 };
 
 static std::string g_create_err;
@@ -85,6 +92,29 @@ void to_device(afqmc_handle* h, double* dst, const void* src, size_t n) {
   cudaMemcpyAsync(dst, src, n * sizeof(double), cudaMemcpyDefault, h->st);
 }
 
+// Brackets the launches of one stage with two events when profiling is on.
+struct StageTimer {
+  afqmc_handle* h;
+  int stage;
+  cudaEvent_t a = nullptr, b = nullptr;
+  static cudaEvent_t get(afqmc_handle* h) {
+    cudaEvent_t e = nullptr;
+    if (!h->ev_free.empty()) { e = h->ev_free.back(); h->ev_free.pop_back(); }
+    else if (cudaEventCreate(&e) != cudaSuccess) { cudaGetLastError(); e = nullptr; }
+    return e;
+  }
+  StageTimer(afqmc_handle* h_, int stage_) : h(h_), stage(stage_) {
+    if (!h->prof) return;
+    a = get(h); b = get(h);
+    if (a && b) cudaEventRecord(a, h->st);
+  }
+  ~StageTimer() {
+    if (!h->prof || !a || !b) return;
+    cudaEventRecord(b, h->st);
+    h->ev_pending.push_back({stage, a, b});
+  }
+};
+
 GemmArgs gemm_args() {
   GemmArgs a;
   memset(&a, 0, sizeof(a));
@@ -97,6 +127,7 @@ GemmArgs gemm_args() {
 // E1 = expm(-dt/2 h_mod) by scaling and squaring of a degree-16 Taylor polynomial (Horner),
 // every product on the DMMA GEMM.  (The oracle uses an eigendecomposition instead: reading S6.)
 void build_E1(afqmc_handle* h, double dt) {
+  StageTimer tm(h, AFQMC_STAGE_E1_BUILD);
   const int M = h->M;
   const long MM = (long)M * M;
   double nrm = 0.5 * fabs(dt) * h->hmod_norm1;
@@ -135,14 +166,19 @@ OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, in
 }
 
 int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
-  h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
+  {
+    StageTimer tm(h, AFQMC_STAGE_E_THETA);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
+  }
   for (int b = 0; b < h->nblk; ++b) {
+    StageTimer tm(h, AFQMC_STAGE_EXCHANGE);
     ExArgs e;
     e.Lrot = h->Lrot; e.ThT = h->ThT; e.expart = h->expart[b]; e.X = h->Xe;
     e.M = h->M; e.Nt = h->Nt; e.n_chol = h->n_chol; e.nw = nw;
     e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
     h->launches += run_exchange(e, h->st);
   }
+  StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
   EnergyArgs r;
   r.expart = h->expart[0]; r.ngroups = h->exgroups[0];
   r.X = h->Xe; r.e1 = h->e1; r.E_out = E_out;
@@ -162,6 +198,8 @@ void afqmc_destroy(afqmc_handle* h) {
   cudaStreamSynchronize(h->st);
   for (void* p : h->allocs)
     if (p) cudaFree(p);
+  for (auto& br : h->ev_pending) { cudaEventDestroy(br.a); cudaEventDestroy(br.b); }
+  for (cudaEvent_t e : h->ev_free) cudaEventDestroy(e);
   if (h->own_stream) cudaStreamDestroy(h->st);
   delete h;
 }
@@ -369,9 +407,13 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   if (!(h->dt_cached == dt)) build_E1(h, dt);
 
   // a1/a2: overlap, Theta
-  h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+  {
+    StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+  }
   // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
   {
+    StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
     GemmArgs g = gemm_args();
     g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
     g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
@@ -380,6 +422,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   }
   // a4: shifted fields, scalars, V_HS coefficients
   {
+    StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
     ShiftArgs s;
     s.Xp = h->Xp; s.sXp = (long)2 * h->maxw * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
     s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
@@ -388,6 +431,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   }
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
   {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
     GemmArgs g = gemm_args();
     g.A = h->Cf; g.lda = nc; g.B = h->L; g.ldb = MM; g.C = h->A; g.ldc = MM;
     g.M = 2 * nw; g.N = (int)MM; g.K = nc;
@@ -396,6 +440,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   // a6: T0 = Acc = E1 phi
   const long wstride = (long)M * 2 * Nt;
   {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
     GemmArgs g = gemm_args();
     g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
     g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
@@ -404,6 +449,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   }
   // a7: T_n = A T_{n-1} / n, Acc += T_n
   {
+    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
     double *Tp = h->T0, *Tn = h->T1;
     for (int n = 1; n <= h->K; ++n) {
       GemmArgs g = gemm_args();
@@ -416,14 +462,19 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   }
   // a8: phi = E1 Acc, written into the caller's walkers
   {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
     GemmArgs g = gemm_args();
     g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
     g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
     h->launches += run_gemm(GEMM_KN, g, h->st);
   }
   // a9: new overlap and weights
-  h->launches += run_overlap_theta(ot_args(h, W, h->det_new, 0, 0), nw, h->st);
   {
+    StageTimer tm(h, AFQMC_STAGE_OVERLAP_NEW);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_new, 0, 0), nw, h->st);
+  }
+  {
+    StageTimer tm(h, AFQMC_STAGE_WEIGHT);
     WeightArgs a;
     a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = h->cfb; a.cmf = h->cmf;
     a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
@@ -434,6 +485,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   h->step_count += 1;
   h->last_nw = nw;
   if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) {
+    StageTimer tm(h, AFQMC_STAGE_REORTHO);
     QRArgs q;
     q.W = W; q.detR = h->detR; q.M = M; q.Nt = Nt; q.nblk = h->nblk;
     for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
@@ -505,6 +557,37 @@ int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
   if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_debug_read");
   int rc = check_cuda(h, "afqmc_debug_read");
   return rc == AFQMC_OK ? n : rc;
+}
+
+int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on) {
+  if (!h) return AFQMC_ERR_INVALID;
+  h->prof = on != 0;
+  return AFQMC_OK;
+}
+
+int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!ms_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  cudaError_t e = cudaStreamSynchronize(h->st);
+  if (e != cudaSuccess) return fail(h, AFQMC_ERR_CUDA, std::string("get_stage_times: ") + cudaGetErrorString(e));
+  for (auto& br : h->ev_pending) {
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, br.a, br.b) == cudaSuccess) {
+      h->stage_ms[br.stage] += ms;
+      h->stage_n[br.stage] += 1;
+    } else {
+      cudaGetLastError();
+    }
+    h->ev_free.push_back(br.a);
+    h->ev_free.push_back(br.b);
+  }
+  h->ev_pending.clear();
+  for (int i = 0; i < AFQMC_STAGE_COUNT; ++i) {
+    ms_out[i] = h->stage_ms[i];
+    if (count_out) count_out[i] = h->stage_n[i];
+    if (reset) { h->stage_ms[i] = 0.0; h->stage_n[i] = 0; }
+  }
+  return AFQMC_OK;
 }
 
 int64_t afqmc_launch_count(const afqmc_handle* h) { return h ? h->launches : -1; }

@@ -1,0 +1,78 @@
+"""CPU-side checks of the boundary: the library builds, loads, exports every symbol that
+include/afqmc.h declares, the ctypes struct matches the C struct, and argument validation
+that needs no device works.  No compute calls here."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "afqmc.h")
+
+
+def _declared():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(afqmc_[a-z0-9_]+)\s*\(", src)))
+
+
+def test_library_exports_every_declared_symbol():
+    import __graft_entry__ as ge
+    ge.build()
+    from paper_2406_16238_b200 import afqmc
+    names = _declared()
+    assert len(names) >= 10
+    for n in names:
+        assert hasattr(afqmc.lib, n), n
+    assert sorted(afqmc.EXPORTS) == names
+
+
+def test_params_struct_layout_matches_c(tmp_path):
+    from paper_2406_16238_b200 import afqmc
+    src = tmp_path / "sz.c"
+    src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "afqmc.h"\n'
+                   'int main(){printf("%zu %zu %zu %zu\\n", sizeof(afqmc_params), '
+                   'offsetof(afqmc_params, e_shift), offsetof(afqmc_params, stream), '
+                   'offsetof(afqmc_params, e_shift_auto));return 0;}\n')
+    exe = tmp_path / "sz"
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
+    P = afqmc.AfqmcParams
+    assert [int(v) for v in out] == [C.sizeof(P), P.e_shift.offset, P.stream.offset, P.e_shift_auto.offset]
+
+
+def test_header_is_plain_c():
+    r = subprocess.run(["gcc", "-std=c99", "-pedantic", "-Werror", "-fsyntax-only", "-x", "c", HEADER],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+
+
+def test_null_and_bad_arguments_are_rejected_without_a_device():
+    from paper_2406_16238_b200 import afqmc
+    lib = afqmc.lib
+    h = C.c_void_p()
+    p = afqmc.AfqmcParams()
+    assert lib.afqmc_create(None, None, None, C.byref(p), C.byref(h)) == -1
+    a = np.zeros(4)
+    p.struct_size = 3
+    assert lib.afqmc_create(a.ctypes.data, a.ctypes.data, a.ctypes.data, C.byref(p), C.byref(h)) == -1
+    assert b"struct_size" in lib.afqmc_last_error(None)
+    assert lib.afqmc_step(None, None, None, None, 0.005, 1) == -1
+    assert lib.afqmc_local_energy(None, None, None, 1) == -1
+    assert lib.afqmc_sync(None) == -1
+    assert lib.afqmc_launch_count(None) == -1
+    lib.afqmc_destroy(None)
+
+
+def test_no_cpu_fallback_in_the_product_path():
+    """The package never imports or executes anything under oracle/."""
+    pk = os.path.join(ROOT, "paper_2406_16238_b200")
+    pat = re.compile(r"^\s*(from|import)\s+oracle\b|oracle[./]afqmc_oracle", re.M)
+    for d, _, fs in os.walk(pk):
+        for f in fs:
+            if f.endswith((".py", ".cu", ".cuh", ".h")):
+                assert not pat.search(open(os.path.join(d, f)).read()), f

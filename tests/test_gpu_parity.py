@@ -1,0 +1,269 @@
+"""GPU parity: the CUDA path (through the C ABI, via the ctypes binding) against the CPU oracle,
+element by element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+1e-10 relative per step (walkers re-seeded from the oracle each step), 1e-8 relative on
+weights, overlaps and local energies after the stated number of free-running steps.
+Setup quantities and single contractions are held to 1e-12."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from tests.gpu_util import Pair, energy_scale, planar_to_complex, rel_fro, rel_max
+
+pytestmark = pytest.mark.gpu
+
+TOL_STAGE = 1e-12
+TOL_STEP = 1e-10
+TOL_RUN = 1e-8
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def gpu_step(pr, walkers, weights, x, dt):
+    """One afqmc_step on device buffers; returns host copies (walkers, weights, overlaps)."""
+    torch = _torch()
+    W = torch.from_numpy(np.ascontiguousarray(walkers)).cuda()
+    wt = torch.from_numpy(np.ascontiguousarray(weights)).cuda()
+    xd = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    ov = torch.empty(W.shape[0], dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    pr.gpu.step(W, wt, xd, dt)
+    pr.gpu.get_overlaps(ov)
+    pr.gpu.sync()
+    return W.cpu().numpy(), wt.cpu().numpy(), ov.cpu().numpy()
+
+
+def gpu_energy(pr, walkers):
+    torch = _torch()
+    W = torch.from_numpy(np.ascontiguousarray(walkers)).cuda()
+    E = torch.empty((W.shape[0], 3), dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    pr.gpu.local_energy(W, E)
+    pr.gpu.sync()
+    return E.cpu().numpy()
+
+
+# --------------------------------------------------------------------------- setup (row a0)
+@pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 8, {}),
+                                          ("c1", 4, dict(M=37, n_alpha=7, n_beta=7, n_chol=53))])
+def test_setup_quantities(name, nw, over):
+    _torch()
+    pr = Pair(name, nw=nw, **over)
+    o, g, cfg = pr.oracle, pr.gpu, pr.cfg
+    assert rel_max(g.debug_read(4), o.m, scale=np.abs(o.m).max()) < TOL_STAGE
+    hm = g.debug_read(3).reshape(cfg.M, cfg.M)
+    assert rel_fro(hm[None], o.h_mod[None]) < TOL_STAGE
+    lr = g.debug_read(5).reshape(cfg.n_chol, cfg.Nt, cfg.M)
+    lr_o = np.concatenate(o.Lrot, axis=1)
+    assert rel_fro(lr[None], lr_o[None]) < TOL_STAGE
+    c = g.constants()
+    assert abs(c["E_const"] - o.E_const) <= TOL_STAGE * abs(o.E_const)
+    assert abs(c["e_trial"] - o.e_shift) <= 1e-11 * abs(o.e_shift)
+    # E1 = expm(-dt/2 h_mod): library = scaling-and-squaring Taylor, oracle = eigendecomposition
+    gpu_step(pr, pr.walkers0, np.ones(pr.nw), pr.fields(0), cfg.dt)
+    E1 = g.debug_read(2).reshape(cfg.M, cfg.M)
+    assert rel_fro(E1[None], o.one_body_propagator(cfg.dt)[None]) < TOL_STAGE
+    pr.close()
+
+
+# --------------------------------------------------------------------------- stages a1-a9
+@pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 24, {}),
+                                          ("c1", 5, dict(M=37, n_alpha=7, n_beta=7, n_chol=53)),
+                                          ("c2", 3, dict(M=41, n_alpha=9, n_beta=1, n_chol=70))])
+def test_one_step_stage_by_stage(name, nw, over):
+    _torch()
+    pr = Pair(name, nw=nw, ortho_every=0, **over)
+    o, g, cfg = pr.oracle, pr.gpu, pr.cfg
+    x = pr.fields(0)
+    w0 = np.linspace(0.5, 1.5, nw)
+    new_o, info = o.propagate(pr.walkers0, x, cfg.dt)
+    Wg, wg, ovg = gpu_step(pr, pr.walkers0, w0, x, cfg.dt)
+    X = planar_to_complex(g.debug_read(0), (nw, cfg.n_chol))
+    assert rel_fro(X, info["X"]) < TOL_STAGE
+    A = planar_to_complex(g.debug_read(1), (nw, cfg.M, cfg.M))
+    assert rel_fro(A, info["A"]) < 1e-11
+    assert rel_fro(Wg, new_o) < TOL_STEP
+    o.n_steps_done = 0
+    _, w_o, ov_o = o.step(pr.walkers0, w0, x, cfg.dt)
+    assert rel_max(ovg, ov_o) < TOL_STEP
+    assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_STEP
+    pr.close()
+
+
+# --------------------------------------------------------------------------- local energy a11
+@pytest.mark.parametrize("name,nw,over", [
+    ("c1", 16, {}), ("c2", 24, {}),
+    ("c1", 3, dict(M=37, n_alpha=7, n_beta=7, n_chol=53)),
+    ("c2", 3, dict(M=41, n_alpha=9, n_beta=1, n_chol=70)),
+    ("c1", 2, dict(M=70, n_alpha=24, n_beta=24, n_chol=40)),
+    ("c1", 2, dict(M=70, n_alpha=33, n_beta=33, n_chol=41)),
+    ("c1", 2, dict(M=90, n_alpha=42, n_beta=42, n_chol=39)),
+    ("c1", 2, dict(M=90, n_alpha=50, n_beta=50, n_chol=37)),
+    ("c1", 2, dict(M=80, n_alpha=64, n_beta=64, n_chol=21)),
+    ("c2", 2, dict(M=80, n_alpha=57, n_beta=43, n_chol=21)),
+])
+def test_local_energy(name, nw, over):
+    """Every exchange tile shape (occupied block 1..64 columns), odd M, ragged gamma groups."""
+    _torch()
+    pr = Pair(name, nw=nw, **over)
+    E_o = pr.oracle.local_energy(pr.walkers0)
+    E_g = gpu_energy(pr, pr.walkers0)
+    sc = energy_scale(pr.oracle, pr.walkers0, E_o)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10
+    pr.close()
+
+
+# --------------------------------------------------------------------------- N steps
+def _run(pr, steps, reseed):
+    """Returns the worst per-step errors (walkers, weights, overlaps) and final states."""
+    o, cfg, nw = pr.oracle, pr.cfg, pr.nw
+    Wo, wo = pr.walkers0.copy(), np.ones(nw)
+    Wg, wg = pr.walkers0.copy(), np.ones(nw)
+    worst = dict(walkers=0.0, weights=0.0, ovlp=0.0)
+    for s in range(steps):
+        x = pr.fields(s)
+        if reseed:
+            Wg, wg = Wo.copy(), wo.copy()
+        Wg, wg, ovg = gpu_step(pr, Wg, wg, x, cfg.dt)
+        Wo, wo, ovo = o.step(Wo, wo, x, cfg.dt)
+        worst["walkers"] = max(worst["walkers"], rel_fro(Wg, Wo))
+        worst["weights"] = max(worst["weights"], rel_max(wg, wo, scale=np.maximum(np.abs(wo), 1e-3)))
+        worst["ovlp"] = max(worst["ovlp"], rel_max(ovg, ovo))
+    return worst, (Wg, wg, ovg), (Wo, wo, ovo)
+
+
+@pytest.mark.parametrize("name,nw", [("c1", 16), ("c2", 64)])
+def test_per_step_parity_reseeded(name, nw):
+    _torch()
+    pr = Pair(name, nw=nw)
+    worst, _, _ = _run(pr, pr.cfg.steps, reseed=True)
+    assert worst["walkers"] < TOL_STEP, worst
+    assert worst["weights"] < TOL_STEP, worst
+    assert worst["ovlp"] < TOL_STEP, worst
+    pr.close()
+
+
+@pytest.mark.parametrize("name,nw", [("c1", 16), ("c2", 640), ("c3", 16)])
+def test_free_running_parity(name, nw):
+    """The stated number of steps without re-seeding (c2: QR every 5 steps), then the local
+    energy: weights, overlaps, energies to 1e-8."""
+    _torch()
+    pr = Pair(name, nw=nw)
+    worst, (Wg, wg, ovg), (Wo, wo, ovo) = _run(pr, pr.cfg.steps, reseed=False)
+    assert worst["weights"] < TOL_RUN, worst
+    assert worst["ovlp"] < TOL_RUN, worst
+    assert worst["walkers"] < TOL_RUN, worst
+    assert np.all(wo > 0), "synthetic recipe should keep every walker alive"
+    E_o = pr.oracle.local_energy(Wo)
+    E_g = gpu_energy(pr, Wg)
+    sc = energy_scale(pr.oracle, Wo, E_o)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_RUN
+    pr.close()
+
+
+# --------------------------------------------------------------------------- boundary behaviour
+def test_host_pointers_equal_device_pointers():
+    torch = _torch()
+    pr = Pair("c1", nw=16, oracle=False)
+    x = pr.fields(0)
+    Wd, wd, ovd = gpu_step(pr, pr.walkers0, np.ones(16), x, pr.cfg.dt)
+    Wh, wh = pr.walkers0.copy(), np.ones(16)
+    pr.gpu.step(Wh, wh, x, pr.cfg.dt)
+    ovh = np.empty(16, dtype=np.complex128)
+    pr.gpu.get_overlaps(ovh)
+    assert np.array_equal(Wh, Wd) and np.array_equal(wh, wd) and np.array_equal(ovh, ovd)
+    Eh = np.empty((16, 3), dtype=np.complex128)
+    pr.gpu.local_energy(Wh, Eh)
+    assert np.array_equal(Eh, gpu_energy(pr, Wd))
+    pr.close()
+
+
+def test_fewer_walkers_than_max_and_single_walker():
+    _torch()
+    pr = Pair("c1", nw=16)
+    x = pr.fields(0)
+    Wa, wa, ova = gpu_step(pr, pr.walkers0, np.ones(16), x, pr.cfg.dt)
+    for n in (1, 5):
+        Wn, wn, ovn = gpu_step(pr, pr.walkers0[:n], np.ones(n), x[:n], pr.cfg.dt)
+        assert rel_fro(Wn, Wa[:n]) < 1e-13 and rel_max(wn, wa[:n]) < 1e-13
+        assert rel_max(gpu_energy(pr, Wn)[:, 0], gpu_energy(pr, Wa)[:n, 0]) < 1e-13
+    pr.close()
+
+
+def test_walker_equals_trial():
+    """Overlap 1, E = trial energy, force bias zero: X = m."""
+    _torch()
+    pr = Pair("c1", nw=2)
+    cfg = pr.cfg
+    W = np.repeat(pr.trial[None].astype(np.complex128), 2, axis=0)
+    E = gpu_energy(pr, W)
+    c = pr.gpu.constants()
+    assert np.max(np.abs(E[:, 0] - c["e_trial"])) < 1e-12 * abs(c["e_trial"])
+    gpu_step(pr, W, np.ones(2), np.zeros((2, cfg.n_chol)), cfg.dt)
+    X = planar_to_complex(pr.gpu.debug_read(0), (2, cfg.n_chol))
+    assert np.max(np.abs(X - pr.oracle.m[None])) < 1e-12 * np.abs(pr.oracle.m).max()
+    pr.close()
+
+
+def test_dead_walkers_get_zero_weight():
+    """Reading S10: zero overlap or cos(theta) <= 0 gives weight exactly 0, no error."""
+    _torch()
+    pr = Pair("c1", nw=4)
+    cfg = pr.cfg
+    W = pr.walkers0.copy()
+    # walker 1: first column replaced by an unoccupied eigenvector of h1 -> overlap exactly ~0
+    lam, v = np.linalg.eigh(pr.h1)
+    W[1] = pr.trial.astype(np.complex128)
+    W[1][:, 0] = v[:, cfg.M - 1]
+    W[2] = np.nan
+    Wg, wg, ovg = gpu_step(pr, W, np.ones(4), pr.fields(0), cfg.dt)
+    _, wo, _ = pr.oracle.step(W, np.ones(4), pr.fields(0), cfg.dt)
+    assert wg[2] == 0.0 and wo[2] == 0.0
+    assert wg[0] > 0 and wg[3] > 0
+    assert rel_max(wg[[0, 3]], wo[[0, 3]]) < TOL_STEP
+    assert np.isfinite(wg[1]) and wg[1] >= 0.0
+    pr.close()
+
+
+def test_error_codes():
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc, inputs
+    cfg = inputs.get_config("c1")
+    h1 = inputs.make_h1(cfg)
+    tr = inputs.make_trial(cfg, h1)
+    Lh = inputs.make_L_host(cfg)
+    Ld = torch.from_numpy(Lh).cuda()
+    kw = dict(M=cfg.M, n_alpha=5, n_beta=5, n_chol=cfg.n_chol, max_walkers=4, walker_kind=0)
+
+    def code(**over):
+        args = dict(kw)
+        L = over.pop("L", Ld)
+        t = over.pop("trial", tr)
+        args.update(over)
+        with pytest.raises(afqmc.AfqmcError) as e:
+            afqmc.AFQMC(h1, L, t, **args)
+        return e.value.code
+
+    assert code(n_beta=4) == -2
+    assert code(taylor_order=17) == -6
+    assert code(L=Lh) == -1
+    assert code(trial=tr * 1.001) == -5
+    assert code(n_alpha=cfg.M + 1, n_beta=cfg.M + 1) == -2
+    g = afqmc.AFQMC(h1, Ld, tr, **kw)
+    W = torch.zeros((5, cfg.M, 5), dtype=torch.complex128, device="cuda")
+    with pytest.raises(afqmc.AfqmcError) as e:
+        g.step(W, torch.ones(5, dtype=torch.float64, device="cuda"),
+               torch.zeros((5, cfg.n_chol), dtype=torch.float64, device="cuda"), 0.005)
+    assert e.value.code == -2
+    with pytest.raises(afqmc.AfqmcError) as e:
+        g.step(W[:2], torch.ones(2, dtype=torch.float64, device="cuda"),
+               torch.zeros((2, cfg.n_chol), dtype=torch.float64, device="cuda"), -1.0)
+    assert e.value.code == -1
+    g.close()
