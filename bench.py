@@ -34,7 +34,10 @@ METRIC = "walker-steps/s (propagate + local energy)"
 UNIT = "walker-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (file named beside each number).
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {
+    ("c5", "exchange"): 2.606e9,   # profiles/r1_full_c5.md (exchange_kernel<6,1,1>, 2.592 GB rd + 0.014 GB wr)
+    ("c5", "vhs"): 57.15e9,        # profiles/r1_full_c5.md (55.69 GB rd + 1.46 GB wr; L is 55.30 GB)
+}
 
 
 def flops_model(cfg, nw):
@@ -172,6 +175,8 @@ def main():
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--profiler-range", action="store_true",
+                    help="cudaProfilerStart/Stop around the timed steps (ncu --profile-from-start off)")
     args = ap.parse_args()
 
     import torch
@@ -232,11 +237,15 @@ def main():
         torch.cuda.synchronize()
         clk = ClockSampler(local)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        if args.profiler_range:
+            torch.cuda.profiler.start()
         e0.record(stream)
         for s in range(Wm, Wm + K):
             one(s)
         e1.record(stream)
         torch.cuda.synchronize()
+        if args.profiler_range:
+            torch.cuda.profiler.stop()
         barrier()
         clocks = clk.stop()
         ms = e0.elapsed_time(e1)
