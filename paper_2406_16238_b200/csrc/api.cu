@@ -2,6 +2,7 @@
 // sequence of kernels that makes one walker step / one local-energy evaluation.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <string>
@@ -33,6 +34,7 @@ struct afqmc_handle {
   // staging for host-pointer calls
   double *stW = nullptr, *stWt = nullptr, *stX = nullptr, *stE = nullptr;
   int fb_split = 1;
+  bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   long step_count = 0;
   int last_nw = 0;
   int64_t launches = 0;
@@ -176,7 +178,13 @@ int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw)
     e.Lrot = h->Lrot; e.ThT = h->ThT; e.expart = h->expart[b]; e.X = h->Xe;
     e.M = h->M; e.Nt = h->Nt; e.n_chol = h->n_chol; e.nw = nw;
     e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
-    h->launches += run_exchange(e, h->st);
+    if (h->ws) {
+      const int r = run_exchange_ws(e, h->st);
+      if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
+      h->launches += r;
+    } else {
+      h->launches += run_exchange(e, h->st);
+    }
   }
   StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
   EnergyArgs r;
@@ -232,6 +240,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->off[1] = p->n_alpha; h->ns[1] = h->rhf ? 0 : p->n_beta;
   h->Nt = h->rhf ? p->n_alpha : p->n_alpha + p->n_beta;
   h->L = L_chol;
+  // TMA needs 16-byte global strides: even M.  AFQMC_LEGACY_KERNELS=1 forces the cp.async
+  // kernels (used by the tests to cover both paths on the same inputs).
+  h->ws = (p->M % 2 == 0) && getenv("AFQMC_LEGACY_KERNELS") == nullptr;
   if (p->stream) {
     h->st = (cudaStream_t)p->stream;
   } else {
@@ -360,7 +371,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->T0 = dalloc(h, wsz); h->T1 = dalloc(h, wsz); h->Acc = dalloc(h, wsz);
   h->ovlp = dalloc(h, 2 * mw); h->detR = dalloc(h, 2 * mw);
   for (int b = 0; b < h->nblk; ++b) {
-    const int G = exchange_group_size(h->ns[b]);
+    const int G = h->ws ? exchange_ws_group_size(h->ns[b]) : exchange_group_size(h->ns[b]);
     h->exgroups[b] = (nc + G - 1) / G;
     h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mw * 2);
   }
@@ -376,7 +387,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     std::vector<double> wt((size_t)M * Nt * 2, 0.0);
     for (size_t i = 0; i < th.size(); ++i) wt[2 * i] = th[i];
     cudaMemcpyAsync(h->stW, wt.data(), wt.size() * 8, cudaMemcpyHostToDevice, h->st);
-    local_energy_device(h, h->stW, h->stE, 1);
+    if (local_energy_device(h, h->stW, h->stE, 1) != AFQMC_OK) return bail(AFQMC_ERR_CUDA, h->err);
     double e[6];
     cudaMemcpyAsync(e, h->stE, 48, cudaMemcpyDeviceToHost, h->st);
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
@@ -512,7 +523,10 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
   double* E = (double*)E_out;
   if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
   if (hostE) E = h->stE;
-  local_energy_device(h, W, E, nw);
+  {
+    const int rc = local_energy_device(h, W, E, nw);
+    if (rc != AFQMC_OK) return rc;
+  }
   if (hostE) {
     cudaMemcpyAsync(E_out, E, (size_t)nw * 48, cudaMemcpyDeviceToHost, h->st);
     if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_local_energy");

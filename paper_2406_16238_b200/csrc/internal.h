@@ -82,6 +82,11 @@ struct ExArgs {
 };
 int exchange_group_size(int ns);            // gamma per CTA tile for this block size
 int run_exchange(const ExArgs& a, cudaStream_t st);
+// exchange_ws.cu: warp-specialised TMA version (needs even M and 16-byte aligned operands)
+bool exchange_ws_usable(int M, const void* Lrot, const void* ThT);
+int exchange_ws_group_size(int ns);
+double exchange_ws_efficiency(int ns);
+int run_exchange_ws(const ExArgs& a, cudaStream_t st);
 
 struct EnergyArgs {
   const double* expart; int ngroups;
