@@ -47,7 +47,9 @@ def flops_model(cfg, nw):
     Nt = sum(blocks)
     return {
         "exchange": nw * sum(4.0 * ng * ns * ns * M + 8.0 * ng * ns * ns for ns in blocks),
-        "vhs": nw * 4.0 * ng * M * M,
+        # symmetric half of A only (L_g = L_g^T; SURVEY 8a row a5 "packed-symmetric minimum")
+        "vhs": nw * 2.0 * ng * M * (M + 1),
+        "vhs_dense_equivalent": nw * 4.0 * ng * M * M,
         "taylor": nw * 8.0 * K * M * M * Nt,
         "force_bias": nw * 4.0 * ng * Nt * M,
         "one_body": 2 * nw * 4.0 * M * M * Nt,

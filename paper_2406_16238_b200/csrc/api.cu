@@ -35,6 +35,9 @@ struct afqmc_handle {
   double *stW = nullptr, *stWt = nullptr, *stX = nullptr, *stE = nullptr;
   int fb_split = 1;
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
+  bool ws_vhs = false;
+  int* vhs_tiles = nullptr;
+  int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
   int64_t launches = 0;
@@ -382,6 +385,16 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
       !h->Xe || !h->e1 || !h->stW || !h->stWt || !h->stX || !h->stE)
     return bail(AFQMC_ERR_ALLOC, "device allocation failed (workspaces)");
 
+  h->ws_vhs = h->ws && vhs_ws_usable(M, nc, h->L, h->Cf, h->A);
+  if (h->ws_vhs) {
+    std::vector<int> tl;
+    h->vhs_ntile = vhs_ws_tile_list(M, &tl);
+    h->vhs_tiles = (int*)dalloc(h, (tl.size() + 1) / 2 + 1);
+    if (!h->vhs_tiles) return bail(AFQMC_ERR_ALLOC, "device allocation failed (tile list)");
+    if (cudaMemcpy(h->vhs_tiles, tl.data(), tl.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "tile list upload failed");
+  }
+
   // ---- E_shift = trial energy ---------------------------------------------------------------
   {
     std::vector<double> wt((size_t)M * Nt * 2, 0.0);
@@ -441,7 +454,12 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
     h->launches += run_field_shift(s, nw, h->st);
   }
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
-  {
+  if (h->ws_vhs) {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
+    const int r = run_vhs_ws(h->Cf, h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw, h->st);
+    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
+    h->launches += r;
+  } else {
     StageTimer tm(h, AFQMC_STAGE_VHS);
     GemmArgs g = gemm_args();
     g.A = h->Cf; g.lda = nc; g.B = h->L; g.ldb = MM; g.C = h->A; g.ldc = MM;

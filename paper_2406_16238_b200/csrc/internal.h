@@ -4,6 +4,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <vector>
 
 #include "../../include/afqmc.h"
 #include "gemm.cuh"
@@ -98,6 +99,12 @@ struct EnergyArgs {
 };
 int run_energy_reduce(const EnergyArgs& a, cudaStream_t st);
 int run_energy_reduce2(const EnergyArgs& a, const double* expart2, int ngroups2, cudaStream_t st);
+
+// vhs_ws.cu: symmetric-half V_HS build on the warp-specialised TMA pipeline
+bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void* C);
+int vhs_ws_tile_list(int M, std::vector<int>* out);
+int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
+               int n_chol, int rows, cudaStream_t st);
 
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);

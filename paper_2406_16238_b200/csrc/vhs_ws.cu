@@ -1,0 +1,236 @@
+// vhs_ws.cu - V_HS build (Eq. 9; "VHS step" PAPER.md:318):
+//     A[(w, plane)][p][q] = sum_g Cf[(w, plane)][g] * L[g][p][q]
+// warp-specialised TMA version that uses the symmetry L_g = L_g^T (8-fold real symmetry,
+// PAPER.md:189; the paper's pack_chol, stores the same half): only tiles that
+// touch the upper triangle (q >= p) are computed, straight out of the caller's DENSE L, and
+// every element is stored twice, at [p][q] and mirrored at [q][p].  Half the flops and half
+// the L bytes of the dense contraction, same result (each element of A is written once, from
+// the upper-triangle entry of L).
+//
+// Tile: 128 rows (w, plane) x (4 p x 32 q).  Producer: per 16-gamma stage one box of Cf
+// (k-major, 128 x 16) and eight boxes {16 q, 1 p, 16 gamma} of L, all SWIZZLE_128B.  Consumers:
+// 8 warps of 64 x 32 (8 x 4 DMMA blocks); a warp owns one q-octet and the 4 p rows, so the
+// mirrored store is 32 contiguous bytes per (row, q).
+#include <vector>
+
+#include "internal.h"
+#include "tma.cuh"
+
+namespace afq {
+
+namespace {
+
+constexpr int kProd = 128;
+constexpr int BMv = 128, PT = 4, QT = 32, BKv = 16;
+constexpr int NCWv = 8, NCTv = NCWv * 32, THREADSv = NCTv + kProd;
+constexpr int A_BYTES = BMv * 128, B_BOX = BKv * 128, B_BYTES = PT * (QT / 16) * B_BOX;
+constexpr int STAGE_BYTESv = A_BYTES + B_BYTES;    // 32 KB
+constexpr int STAGESv = 6;
+constexpr size_t SMEMv = (size_t)STAGESv * STAGE_BYTESv + 1024 + 256;
+
+struct VhsArgs {
+  double* C;            // [rows][M][M]
+  const int* tiles;     // [ntile_n] packed (pb << 16 | qb)
+  int M, n_chol, rows;  // rows = 2 nw
+  int ntile_n, mtiles;
+};
+
+__global__ void __launch_bounds__(THREADSv, 1)
+vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB, const VhsArgs a) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)STAGESv * STAGE_BYTESv);
+  uint64_t* empty = full + STAGESv;
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int KT = (a.n_chol + BKv - 1) / BKv;
+  const int ntiles = a.ntile_n * a.mtiles;
+
+  if (tid == 0) {
+    for (int s = 0; s < STAGESv; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCWv); }
+    fence_barrier_init();
+  }
+  __syncthreads();
+
+  if (warp >= NCWv) {
+    reg_dealloc<24>();
+    if (warp == NCWv && lane == 0) {
+      prefetch_tensormap(&tmA);
+      prefetch_tensormap(&tmB);
+      uint32_t it = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int tn = a.tiles[tile / a.mtiles], mt = tile % a.mtiles;
+        const int p0 = (tn >> 16) * PT, q0 = (tn & 0xffff) * QT;
+        for (int kt = 0; kt < KT; ++kt, ++it) {
+          const int s = it % STAGESv;
+          mbar_wait(&empty[s], ((it / STAGESv) & 1) ^ 1);
+          mbar_expect_tx(&full[s], STAGE_BYTESv);
+          unsigned char* sa = smem + (size_t)s * STAGE_BYTESv;
+          tma_load_2d(sa, &tmA, &full[s], kt * BKv, mt * BMv);
+          unsigned char* sb = sa + A_BYTES;
+#pragma unroll
+          for (int pl = 0; pl < PT; ++pl)
+#pragma unroll
+            for (int qb = 0; qb < QT / 16; ++qb)
+              tma_load_3d(sb + (pl * (QT / 16) + qb) * B_BOX, &tmB, &full[s], q0 + 16 * qb, p0 + pl, kt * BKv);
+        }
+      }
+    }
+    return;
+  }
+
+  reg_alloc<240>();
+  constexpr int MI = 8, NI = 4;
+  const int g = lane >> 2, t = lane & 3;
+  const int wm = warp & 1, wn = warp >> 1;       // wn: q-octet 0..3 of the 32-wide tile
+  const int p = rperm(g);
+  // A (k-major, 16-byte loads): chunk (4 kp + t) of row 8 b + p
+  const uint32_t la0 = (uint32_t)(p * 128 + ((t ^ p) << 4));
+  const uint32_t la1 = (uint32_t)(p * 128 + (((t ^ p) ^ 4) << 4));
+  // B (n-major, 8-byte loads): box (j, qb) row k = 8 kp + 2 t + par, element q = 8 h + g
+  const int qb = wn >> 1, hh = wn & 1;
+  const int chunk = 4 * hh + (g >> 1);
+  uint32_t lb[2][2];                              // [kp][par]
+#pragma unroll
+  for (int kp = 0; kp < 2; ++kp)
+#pragma unroll
+    for (int par = 0; par < 2; ++par) {
+      const int k = 8 * kp + 2 * t + par;
+      lb[kp][par] = (uint32_t)(qb * B_BOX + k * 128 + ((chunk ^ (k & 7)) << 4) + (g & 1) * 8);
+    }
+  const uint32_t smem_u = smem_u32(smem);
+  const uint32_t aoff = (uint32_t)(wm * MI) * 1024u;
+  const size_t MM = (size_t)a.M * a.M;
+
+  uint32_t it = 0;
+  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+    const int tn = a.tiles[tile / a.mtiles], mt = tile % a.mtiles;
+    const int p0 = (tn >> 16) * PT, q0 = (tn & 0xffff) * QT;
+
+    double acc[MI][NI][2];
+#pragma unroll
+    for (int i = 0; i < MI; ++i)
+#pragma unroll
+      for (int j = 0; j < NI; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
+
+    for (int kt = 0; kt < KT; ++kt, ++it) {
+      const int s = it % STAGESv;
+      mbar_wait(&full[s], (it / STAGESv) & 1);
+      const uint32_t sa = smem_u + (uint32_t)s * STAGE_BYTESv + aoff;
+      const uint32_t sb = smem_u + (uint32_t)s * STAGE_BYTESv + A_BYTES;
+#pragma unroll
+      for (int kp = 0; kp < 2; ++kp) {
+        double2 af[MI];
+#pragma unroll
+        for (int i = 0; i < MI; ++i) af[i] = lds128(sa + i * 1024 + (kp ? la1 : la0));
+        double b0[NI], b1[NI];
+#pragma unroll
+        for (int j = 0; j < NI; ++j) {
+          b0[j] = lds64(sb + j * (QT / 16) * B_BOX + lb[kp][0]);
+          b1[j] = lds64(sb + j * (QT / 16) * B_BOX + lb[kp][1]);
+        }
+#pragma unroll
+        for (int j = 0; j < NI; ++j)
+#pragma unroll
+          for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].x, b0[j]);
+#pragma unroll
+        for (int j = 0; j < NI; ++j)
+#pragma unroll
+          for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, b1[j]);
+      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&empty[s]);
+    }
+
+    // ---- epilogue: direct store at [p][q] (q >= p) and mirrored store at [q][p] (q > p)
+    const int ql = q0 + 8 * wn;                    // first q of this warp's octet
+    if (ql + 7 < p0) continue;                     // entirely below the diagonal: nothing to keep
+    const int q = ql + 2 * t;                      // this lane's q, q + 1
+    const bool fast = (ql >= p0 + PT) && (p0 + PT <= a.M) && (ql + 8 <= a.M);
+#pragma unroll
+    for (int i = 0; i < MI; ++i) {
+      const int r = mt * BMv + 8 * (wm * MI + i) + p;
+      if (r >= a.rows) continue;
+      double* Cr = a.C + (size_t)r * MM;
+      if (fast) {
+#pragma unroll
+        for (int j = 0; j < NI; ++j)
+          *reinterpret_cast<double2*>(Cr + (size_t)(p0 + j) * a.M + q) = make_double2(acc[i][j][0], acc[i][j][1]);
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+          double* d = Cr + (size_t)(q + e) * a.M + p0;
+          *reinterpret_cast<double2*>(d) = make_double2(acc[i][0][e], acc[i][1][e]);
+          *reinterpret_cast<double2*>(d + 2) = make_double2(acc[i][2][e], acc[i][3][e]);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < NI; ++j) {
+          const int pp = p0 + j;
+          if (pp >= a.M) continue;
+#pragma unroll
+          for (int e = 0; e < 2; ++e) {
+            const int qq = q + e;
+            if (qq >= a.M || qq < pp) continue;
+            Cr[(size_t)pp * a.M + qq] = acc[i][j][e];
+            if (qq > pp) Cr[(size_t)qq * a.M + pp] = acc[i][j][e];
+          }
+        }
+      }
+    }
+  }
+}
+
+}  // namespace
+
+// host: list of (p-block, q-block) tiles that intersect the upper triangle, row-major
+int vhs_ws_tile_list(int M, std::vector<int>* out) {
+  out->clear();
+  const int npb = (M + PT - 1) / PT, nqb = (M + QT - 1) / QT;
+  for (int pb = 0; pb < npb; ++pb)
+    for (int qb = 0; qb < nqb; ++qb)
+      if (qb * QT + QT - 1 >= pb * PT) out->push_back((pb << 16) | qb);
+  return (int)out->size();
+}
+
+bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void* C) {
+  return (M % 2 == 0) && (n_chol % 2 == 0) && M < 65536 * PT &&
+         ((((uintptr_t)L | (uintptr_t)Cf | (uintptr_t)C) & 15) == 0);
+}
+
+// algorithmic flops actually needed with the symmetric half: 2 * rows * n_chol * M (M + 1) / 2 * 2
+int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
+               int n_chol, int rows, cudaStream_t st) {
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(vhs_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
+    attr = true;
+  }
+  static int nsm = 0;
+  if (!nsm) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    if (nsm <= 0) nsm = 148;
+  }
+  TensorMap tmA, tmB;
+  {
+    const uint64_t dims[2] = {(uint64_t)n_chol, (uint64_t)rows};
+    const uint64_t str[1] = {(uint64_t)n_chol * 8};
+    const uint32_t box[2] = {BKv, BMv};
+    if (make_tensor_map_f64(&tmA, Cf, 2, dims, str, box) != 0) return -1;
+  }
+  {
+    const uint64_t dims[3] = {(uint64_t)M, (uint64_t)M, (uint64_t)n_chol};
+    const uint64_t str[2] = {(uint64_t)M * 8, (uint64_t)M * M * 8};
+    const uint32_t box[3] = {16, 1, BKv};
+    if (make_tensor_map_f64(&tmB, L, 3, dims, str, box) != 0) return -1;
+  }
+  VhsArgs a;
+  a.C = C; a.tiles = tiles_dev; a.M = M; a.n_chol = n_chol; a.rows = rows;
+  a.ntile_n = ntile_n; a.mtiles = (rows + BMv - 1) / BMv;
+  const long nt = (long)a.ntile_n * a.mtiles;
+  const int grid = nt < nsm ? (int)nt : nsm;
+  vhs_ws_kernel<<<grid, THREADSv, SMEMv, st>>>(tmA, tmB, a);
+  return 1;
+}
+
+}  // namespace afq
