@@ -363,7 +363,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     if (split > kmax) split = kmax;
     if (split > 16) split = 16;
     if (split < 1) split = 1;
-    h->fb_split = split;
+    h->fb_split = h->ws ? gemm_ws_nk_split(2 * mw, nc, Nt * M, 16) : split;
   }
   const size_t wsz = (size_t)mw * M * 2 * Nt;
   h->det_old = dalloc(h, (size_t)mw * 2 * 2); h->det_new = dalloc(h, (size_t)mw * 2 * 2);
@@ -442,7 +442,11 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
     g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
     g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
     g.splitK = h->fb_split; g.sCsplit = (long)2 * h->maxw * nc;
-    h->launches += run_gemm(GEMM_NK, g, h->st);
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_nk(h->ThT, (long)Nt * M, h->Lrot, (long)Nt * M, h->Xp, nc, g.sCsplit, 2 * nw, nc, Nt * M,
+                         h->fb_split, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_NK, g, h->st);
   }
   // a4: shifted fields, scalars, V_HS coefficients
   {
@@ -474,7 +478,11 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
     g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
     g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
     g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    h->launches += run_gemm(GEMM_KN, g, h->st);
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 2, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
   }
   // a7: T_n = A T_{n-1} / n, Acc += T_n
   {
@@ -485,7 +493,11 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
       g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
       g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
       g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
-      h->launches += run_gemm(GEMM_CPLX_KN, g, h->st);
+      int r = -1;
+      if (h->ws)
+        r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
+                           M, nw, 1.0 / n, 1, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
       std::swap(Tp, Tn);
     }
   }
@@ -495,7 +507,11 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
     GemmArgs g = gemm_args();
     g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
     g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    h->launches += run_gemm(GEMM_KN, g, h->st);
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 0, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
   }
   // a9: new overlap and weights
   {

@@ -106,6 +106,14 @@ int vhs_ws_tile_list(int M, std::vector<int>* out);
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
                int n_chol, int rows, cudaStream_t st);
 
+// gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
+int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
+                   double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,
+                   int mode, cudaStream_t st);
+int gemm_ws_nk_split(int M, int N, int K, int max_split);
+int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double* C, long ldc, long sCsplit,
+                   int M, int N, int K, int split, cudaStream_t st);
+
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);
 int run_sum_mL(const double* L, const double* m, double* out, int M, int n_chol, cudaStream_t st);
