@@ -142,6 +142,27 @@ def make_L(cfg, seed, want_host, want_dev):
     return Ld, (Lh if want_host else None)
 
 
+def replica_seed(rank):
+    """Every replica draws its own walkers and fields; the Hamiltonian (seed 0) is the same."""
+    return int(rank)
+
+
+def max_over_ranks(ms, dist, device):
+    """Slowest rank's time: all-reduce MAX over the process group (NCCL on the GPU box, gloo in
+    the CPU test); the identity without a group."""
+    if dist is None:
+        return float(ms)
+    import torch
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def job_value(world, nw_per_rank, steps, t_ms):
+    """Whole-job walker-steps/s of `world` replicas of nw_per_rank walkers (weak scaling)."""
+    return world * nw_per_rank * steps / (t_ms * 1e-3)
+
+
 def run_reference(args, cfg, rank):
     """--impl reference: the CPU oracle, as it stands, on a bounded sample of the workload."""
     if rank != 0:
@@ -205,7 +226,7 @@ def main():
             dist.barrier()
 
     K, Wm, nw = args.steps, args.warmup, cfg.nw
-    seed = rank           # every replica draws its own walkers / fields; same Hamiltonian shape
+    seed = replica_seed(rank)
     h1 = inputs.make_h1(cfg, 0)
     trial = inputs.make_trial(cfg, h1, 0)
     want_cpu = (rank == 0 and world == 1 and not args.no_cpu_baseline)
@@ -257,12 +278,8 @@ def main():
         E_last = E.cpu().numpy()
         wt_last = wt.cpu().numpy()
 
-    tmax = ms
-    if dist is not None:
-        t = torch.tensor([ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        tmax = float(t.item())
-    value = world * nw * K / (tmax * 1e-3)
+    tmax = max_over_ranks(ms, dist, "cuda")
+    value = job_value(world, nw, K, tmax)
 
     # ---- end to end through the C ABI with pinned host buffers ---------------------------------
     e2e = None
@@ -287,12 +304,9 @@ def main():
         g.sync()
         t_e2e = time.perf_counter() - t0
         barrier()
-        if dist is not None:
-            t = torch.tensor([t_e2e], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            t_e2e = float(t.item())
+        t_e2e = max_over_ranks(t_e2e, dist, "cuda")
         wbytes = Wn.nbytes
-        e2e = {"value": world * nw * K / t_e2e, "unit": UNIT,
+        e2e = {"value": job_value(world, nw, K, t_e2e * 1e3), "unit": UNIT,
                "h2d_bytes_per_step": int(2 * wbytes + wn.nbytes + xp[0].numpy().nbytes),
                "d2h_bytes_per_step": int(wbytes + wn.nbytes + En.nbytes)}
 

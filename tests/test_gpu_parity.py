@@ -168,6 +168,70 @@ def test_free_running_parity(name, nw):
     pr.close()
 
 
+# --------------------------------------------------------------------------- full sizes
+@pytest.mark.parametrize("name,idx,device_L", [("c3", (0, 129, 255), False),
+                                               ("c4", (0, 77, 127), True),
+                                               ("c5", (0, 37, 63), True)])
+def test_full_size_sampled_walkers(name, idx, device_L):
+    """BASELINE.json's full sizes in the launch configuration bench.py times (the whole batch of
+    Nw walkers per call, same handle parameters), checked on SAMPLED walkers: walkers are
+    independent given (h1, L, trial), so the oracle run on walkers `idx` alone gives exactly what
+    it would give for them inside the full batch.  Per step (sampled walkers of a copy of the
+    batch re-seeded from the oracle): 1e-10; free-running over the stated number of steps, then
+    the local energy: 1e-8."""
+    torch = _torch()
+    pr = Pair(name, device_L=device_L)
+    o, cfg, nw = pr.oracle, pr.cfg, pr.nw
+    assert cfg.ortho_every == 0          # two GPU steps per oracle step below: keep QR out of it
+    idx = np.asarray(idx)
+    ti = torch.from_numpy(idx).cuda()
+    Wg = torch.from_numpy(pr.walkers0).cuda()
+    wg = torch.ones(nw, dtype=torch.float64, device="cuda")
+    ov = torch.empty(nw, dtype=torch.complex128, device="cuda")
+    Wo, wo = pr.walkers0[idx].copy(), np.ones(len(idx))
+    step_err = dict(walkers=0.0, weights=0.0, ovlp=0.0)
+    run_err = dict(walkers=0.0, weights=0.0, ovlp=0.0)
+
+    def upd(d, W, w, v, Wref, wref, vref):
+        d["walkers"] = max(d["walkers"], rel_fro(W, Wref))
+        d["weights"] = max(d["weights"], rel_max(w, wref, scale=np.maximum(np.abs(wref), 1e-3)))
+        d["ovlp"] = max(d["ovlp"], rel_max(v, vref))
+
+    for s in range(cfg.steps):
+        x = pr.fields(s)
+        xd = torch.from_numpy(x).cuda()
+        Wr, wr = Wg.clone(), wg.clone()
+        Wr[ti] = torch.from_numpy(Wo).cuda()
+        wr[ti] = torch.from_numpy(wo).cuda()
+        pr.gpu.step(Wr, wr, xd, cfg.dt)
+        pr.gpu.get_overlaps(ov)
+        pr.gpu.sync()
+        re_s = (Wr[ti].cpu().numpy(), wr[ti].cpu().numpy(), ov[ti].cpu().numpy())
+        pr.gpu.step(Wg, wg, xd, cfg.dt)
+        pr.gpu.get_overlaps(ov)
+        pr.gpu.sync()
+        Wo, wo, ovo = o.step(Wo, wo, x[idx], cfg.dt)
+        upd(step_err, *re_s, Wo, wo, ovo)
+        upd(run_err, Wg[ti].cpu().numpy(), wg[ti].cpu().numpy(), ov[ti].cpu().numpy(), Wo, wo, ovo)
+        del Wr, wr
+    assert max(step_err.values()) < TOL_STEP, step_err
+    assert max(run_err.values()) < TOL_RUN, run_err
+    assert np.all(wo > 0)
+    assert bool(torch.all(torch.isfinite(wg))) and bool(torch.all(wg >= 0))
+    E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    pr.gpu.local_energy(Wg, E)
+    pr.gpu.sync()
+    E_g = E[ti].cpu().numpy()
+    E_o = o.local_energy(Wo)
+    sc = energy_scale(o, Wo, E_o)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_RUN
+    # every walker of the batch, not only the sampled ones, has a finite energy near the trial's
+    Ea = E.cpu().numpy()
+    assert np.all(np.isfinite(Ea.view(np.float64)))
+    pr.close()
+
+
 # --------------------------------------------------------------------------- boundary behaviour
 def test_host_pointers_equal_device_pointers():
     torch = _torch()
