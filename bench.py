@@ -35,8 +35,8 @@ UNIT = "walker-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (file named beside each number).
 NCU_TRAFFIC = {
-    ("c5", "exchange"): 2.606e9,   # profiles/r1_full_c5.md (exchange_kernel<6,1,1>, 2.592 GB rd + 0.014 GB wr)
-    ("c5", "vhs"): 57.15e9,        # profiles/r1_full_c5.md (55.69 GB rd + 1.46 GB wr; L is 55.30 GB)
+    ("c5", "exchange"): 3.140e9,   # profiles/r1v2_full_c5.md (exchange_ws_kernel<4,3,4,7>, 3.127 GB rd + 0.013 GB wr)
+    ("c5", "vhs"): 31.72e9,        # profiles/r1v2_full_c5.md (vhs_ws_kernel, 30.26 GB rd + 1.46 GB wr; upper tiles of L)
 }
 
 
