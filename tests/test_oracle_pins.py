@@ -338,3 +338,105 @@ def test_P13_weights_real_nonnegative_and_phaseless_cut():
     bad = walkers[:1].copy(); bad[:] = 0
     _, wb, _ = o.step(bad, np.ones(1), r.standard_normal((1, 6)), 0.05)
     assert wb[0] == 0.0
+
+
+# --------------------------------------------------------------------------- P14 comb
+from oracle.block_oracle import comb, estimators, run_block  # noqa: E402
+
+
+def _random_weights(r, nw, dead=0):
+    w = r.uniform(0.05, 3.0, nw) ** 2
+    if dead:
+        w[r.choice(nw, dead, replace=False)] = 0.0
+    return w
+
+
+@pytest.mark.parametrize("nw,dead", [(7, 0), (64, 5), (640, 40)])
+def test_P14_comb_counts_closed_form(nw, dead):
+    """Copies of walker i = number of integers k with c_{i-1} <= (k + xi) s < c_i, which has the
+    closed form ceil(c_i/s - xi) - ceil(c_{i-1}/s - xi): an independent count (no search)."""
+    r = np.random.default_rng(nw)
+    w = _random_weights(r, nw, dead)
+    c = np.concatenate([[0.0], np.cumsum(w)])
+    s = c[-1] / nw
+    for xi in (0.0, 0.123456789, 0.5, 0.999):
+        m, wn = comb(w, xi)
+        counts = np.bincount(m, minlength=nw)
+        closed = np.ceil(c[1:] / s - xi) - np.ceil(c[:-1] / s - xi)
+        closed[-1] += nw - closed.sum()          # the end point c_Nw/s = Nw is exact only up to rounding
+        assert np.array_equal(counts, closed.astype(int))
+        assert np.all(np.diff(m) >= 0)                              # a comb never reorders
+        assert np.all(counts[w == 0.0] == 0)                        # dead walkers are never copied
+        ideal = nw * w / c[-1]                                      # copies within one of the ideal
+        assert np.all(counts >= np.floor(ideal - 1e-9)) and np.all(counts <= np.ceil(ideal + 1e-9))
+        assert np.all(wn == wn[0]) and abs(wn.sum() - w.sum()) < 1e-13 * w.sum()   # total weight kept
+
+
+def test_P14_comb_is_unbiased():
+    """Averaged over xi (uniform grid), the number of copies of walker i is Nw w_i / W, i.e.
+    sum_k w'_k f(phi'_k) has the expectation sum_i w_i f(phi_i) (Eq. 10)."""
+    r = np.random.default_rng(5)
+    nw, J = 24, 2000
+    w = _random_weights(r, nw, 3)
+    mean = np.zeros(nw)
+    for j in range(J):
+        m, _ = comb(w, (j + 0.5) / J)
+        mean += np.bincount(m, minlength=nw)
+    mean /= J
+    assert np.abs(mean - nw * w / w.sum()).max() < 2.0 / J * nw
+
+
+def test_P14_comb_special_cases():
+    nw = 16
+    for xi, v in ((0.0, 0.75), (0.3, 0.7), (0.99, 0.7)):             # equal weights: nothing moves
+        m, wn = comb(np.full(nw, v), xi)                             # (xi = 0 puts the teeth ON the
+        assert np.array_equal(m, np.arange(nw)) and np.allclose(wn, v, rtol=1e-15)   # boundaries: exact sums)
+    w = np.zeros(nw); w[11] = 2.5                                    # one survivor takes every slot
+    m, wn = comb(w, 0.4)
+    assert np.all(m == 11) and np.allclose(wn, 2.5 / nw)
+    for bad in (np.zeros(nw), np.full(nw, np.nan), np.full(nw, np.inf)):   # nothing to resample
+        m, wn = comb(bad, 0.2)
+        assert np.array_equal(m, np.arange(nw)) and np.array_equal(wn, bad, equal_nan=True)
+    with pytest.raises(ValueError):
+        comb(np.ones(4), 1.0)
+
+
+# --------------------------------------------------------------------------- P15 estimator, block
+def test_P15_estimator_and_block_loop():
+    h, L, trial, walkers = small_problem(8, 3, 3, 6, 0, 21, lscale=0.15, noise=0.05, nw=6)
+    o = AFQMCOracle(h, L, trial, 3, 3, 0, ortho_every=2)
+    # (a) walkers = trial with arbitrary weights: ENumer/EDenom is the closed-form HF energy (P2),
+    # EDenom the total weight, and the one- and two-body parts add up
+    P = trial @ trial.T
+    e1 = 2 * np.trace(h @ P)
+    e2 = sum(2 * np.trace(Lg @ P) ** 2 - np.trace(Lg @ P @ Lg @ P) for Lg in L)
+    wts = np.array([0.3, 1.7, 0.0, 2.2])
+    Wt = np.repeat(trial[None].astype(np.complex128), 4, axis=0)
+    est = estimators(wts, o.local_energy(Wt))
+    assert abs(est[1] - 4.2) < 1e-14
+    assert abs(est[0] / est[1] - (e1 + e2)) < 1e-12 * abs(e1 + e2)
+    assert abs(est[2] / est[1] - e1) < 1e-12 * abs(e1) and abs(est[3] / est[1] - e2) < 1e-12 * abs(e2)
+    assert np.allclose(estimators(3.0 * wts, o.local_energy(Wt)), 3.0 * est, rtol=1e-14)
+    # (b) the block loop is the plain composition step -> comb -> ... -> local energy
+    r = np.random.default_rng(3)
+    x = r.standard_normal((4, 6, 6))
+    xi = [0.37, 0.81]
+    W, w, ov, E, est, maps = run_block(o, walkers, np.ones(6), x, xi, 0.01, 2)
+    o2 = AFQMCOracle(h, L, trial, 3, 3, 0, ortho_every=2)
+    W2, w2 = walkers, np.ones(6)
+    for s in range(4):
+        W2, w2, ov2 = o2.step(W2, w2, x[s], 0.01)
+        if s in (1, 3):
+            m, w2 = comb(w2, xi[s // 2])
+            W2, ov2 = W2[m], ov2[m]
+    assert np.array_equal(W, W2) and np.array_equal(w, w2) and np.array_equal(ov, ov2)
+    assert len(maps) == 2 and np.array_equal(E, o2.local_energy(W2))
+    assert np.allclose(ov, o.overlap(W), rtol=1e-10)                 # carried overlaps follow the walkers
+    # (c) population control does not change the total weight, and the estimate it leaves is a
+    # weighted mean of the local energies it was given
+    assert abs(w.sum() - est[1]) < 1e-13 * est[1]
+    assert E[:, 0].real.min() - 1e-12 <= est[0] / est[1] <= E[:, 0].real.max() + 1e-12
+    # (d) pop_every = 0: no comb at all
+    o3 = AFQMCOracle(h, L, trial, 3, 3, 0, ortho_every=2)
+    _, w3, _, _, _, maps3 = run_block(o3, walkers, np.ones(6), x, [], 0.01, 0)
+    assert maps3 == [] and not np.allclose(w3, w3[0])
