@@ -95,7 +95,49 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
  *           energy[:, 0..2] of the paper's Code Snippet 9. */
 int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, int32_t nw);
 
-/* Overlaps <Psi_T|phi_w> of the walkers as left by the last afqmc_step.
+/* Population control by the comb ("population control"; done locally on one
+ * GPU; the algorithm is DESIGN.md reading S21 - the paper names none).  With
+ * c_i = w_0 + ... + w_i (sequential float64 sum), W = c_{nw-1}, s = W / nw and the teeth
+ * t_k = (k + xi) s, the new walker k is a copy of the old walker i_k = min(#{j : c_j <= t_k},
+ * first j with c_j == W), and every new weight is s.  The overlaps kept in the handle are
+ * permuted with the walkers.  If W is not finite or not > 0 nothing changes (identity map).
+ *   walkers EITHER complex128 [nw][M][Nt], in/out.   weights EITHER double [nw], in/out.
+ *   xi      EITHER one double in [0, 1), drawn by the caller (the library draws no random numbers).
+ *   map_out EITHER int32 [nw] or NULL: receives i_k (non-decreasing). */
+int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi,
+                                 int32_t nw, int32_t* map_out);
+
+/* Estimator sums of the paper's Code Snippet 9:
+ * est_out[0..3] = (ENumer, EDenom, E1Body, E2Body) = sum_w weights[w] (Re E[w][0], 1, Re E[w][1],
+ * Re E[w][2]); the mixed energy estimate of Eq. (11) with Eq. (10)'s weights is ENumer/EDenom.
+ *   weights EITHER double [nw];  E EITHER complex128 [nw][3] (from afqmc_local_energy);
+ *   est_out EITHER double [4]. */
+int32_t afqmc_estimators(afqmc_handle* h, const double* weights, const void* E, double* est_out,
+                         int32_t nw);
+
+/* One block ("100 blocks, each containing 25 steps"): n_steps times
+ * afqmc_step (re-orthonormalising on the handle's ortho_every schedule), the comb after every
+ * pop_every-th step of the block (pop_every = 0: never) with xi[0], xi[1], ... in order, then
+ * afqmc_local_energy of the final walkers and afqmc_estimators.  One stream, no host
+ * synchronisation between the steps when every buffer is a device buffer.
+ *   walkers, weights  EITHER, in/out as in afqmc_step.
+ *   aux_fields EITHER double [n_steps][nw][n_chol].
+ *   xi         EITHER double [n_steps / pop_every] (may be NULL when pop_every = 0).
+ *   E_out      EITHER complex128 [nw][3] or NULL.    est_out EITHER double [4] or NULL. */
+int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields,
+                        const double* xi, double dt, int32_t nw, int32_t n_steps, int32_t pop_every,
+                        void* E_out, double* est_out);
+
+/* afqmc_run_block on device buffers replays a CUDA graph of the whole block from the third call
+ * with the same arguments on (first call: eager, second: stream capture); the graph is keyed by
+ * every pointer, nw, n_steps, pop_every, dt and the phase of the ortho_every schedule, so a
+ * caller that reuses its buffers block after block pays one cudaGraphLaunch per block.
+ * on = 1/0 switches this on (default) / off, on < 0 leaves it unchanged.  Returns the number of
+ * graph launches issued so far on this handle (or a negative code). */
+int64_t afqmc_set_block_graph(afqmc_handle* h, int32_t on);
+
+/* Overlaps <Psi_T|phi_w> of the walkers as left by the last afqmc_step (permuted by any
+ * afqmc_population_control since).
  *   ovlp_out EITHER complex128 [nw of that step]. */
 int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out);
 
@@ -133,7 +175,9 @@ int64_t afqmc_launch_count(const afqmc_handle* h);
 #define AFQMC_STAGE_EXCHANGE 10      /* a11: T = Lrot Theta, tr(TT), tr(T)                    */
 #define AFQMC_STAGE_E_REDUCE 11      /* a11: Coulomb sum and final energies                   */
 #define AFQMC_STAGE_E1_BUILD 12      /* expm(-dt/2 h_mod), only when dt changes               */
-#define AFQMC_STAGE_COUNT 13
+#define AFQMC_STAGE_POP_CONTROL 13   /* comb + walker permutation                            */
+#define AFQMC_STAGE_ESTIMATORS 14    /* weighted sums of Code Snippet 9                       */
+#define AFQMC_STAGE_COUNT 15
 int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on);
 /*   ms_out HOST double [AFQMC_STAGE_COUNT]; count_out HOST int64 [AFQMC_STAGE_COUNT] or NULL. */
 int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset);

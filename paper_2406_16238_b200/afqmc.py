@@ -18,10 +18,11 @@ LIB_PATH = os.path.join(_HERE, "libafqmc.so")
 EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overlaps",
            "afqmc_get_constants", "afqmc_debug_read", "afqmc_launch_count", "afqmc_sync",
            "afqmc_last_error", "afqmc_destroy", "afqmc_measure_fp64_peak", "afqmc_set_profiling",
-           "afqmc_get_stage_times"]
+           "afqmc_get_stage_times", "afqmc_population_control", "afqmc_estimators", "afqmc_run_block",
+           "afqmc_set_block_graph"]
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
-          "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build"]
+          "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators"]
 
 
 class AfqmcParams(C.Structure):
@@ -62,6 +63,14 @@ def _load():
     lib.afqmc_set_profiling.restype = i32
     lib.afqmc_get_stage_times.argtypes = [vp, vp, vp, i32]
     lib.afqmc_get_stage_times.restype = i32
+    lib.afqmc_population_control.argtypes = [vp, vp, vp, vp, i32, vp]
+    lib.afqmc_population_control.restype = i32
+    lib.afqmc_estimators.argtypes = [vp, vp, vp, vp, i32]
+    lib.afqmc_estimators.restype = i32
+    lib.afqmc_run_block.argtypes = [vp, vp, vp, vp, vp, dbl, i32, i32, i32, vp, vp]
+    lib.afqmc_run_block.restype = i32
+    lib.afqmc_set_block_graph.argtypes = [vp, i32]
+    lib.afqmc_set_block_graph.restype = i64
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
     return lib
@@ -133,6 +142,30 @@ class AFQMC:
     def local_energy(self, walkers, E_out, nw=None):
         nw = int(walkers.shape[0]) if nw is None else nw
         self._check(lib.afqmc_local_energy(self._h, _ptr(walkers), _ptr(E_out), nw))
+
+    def population_control(self, walkers, weights, xi, map_out=None, nw=None):
+        """xi: array/tensor holding one double in [0, 1) (host or device)."""
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_population_control(self._h, _ptr(walkers), _ptr(weights), _ptr(xi), nw,
+                                                 _ptr(map_out)))
+
+    def estimators(self, weights, E, est_out, nw=None):
+        nw = int(weights.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_estimators(self._h, _ptr(weights), _ptr(E), _ptr(est_out), nw))
+
+    def run_block(self, walkers, weights, aux_fields, xi, dt, pop_every, E_out=None, est_out=None, nw=None):
+        """aux_fields [n_steps][nw][n_chol]; xi [n_steps // pop_every] doubles (None if pop_every = 0)."""
+        nw = int(walkers.shape[0]) if nw is None else nw
+        n_steps = int(aux_fields.shape[0])
+        self._check(lib.afqmc_run_block(self._h, _ptr(walkers), _ptr(weights), _ptr(aux_fields), _ptr(xi),
+                                        float(dt), nw, n_steps, int(pop_every), _ptr(E_out), _ptr(est_out)))
+
+    def set_block_graph(self, on=-1):
+        """Switch CUDA-graph replay of run_block on/off (-1: query only); returns graph launches so far."""
+        n = lib.afqmc_set_block_graph(self._h, int(on))
+        if n < 0:
+            self._check(int(n))
+        return int(n)
 
     def get_overlaps(self, out):
         self._check(lib.afqmc_get_overlaps(self._h, _ptr(out)))

@@ -33,6 +33,21 @@ struct afqmc_handle {
   int exgroups[2] = {0, 0};
   // staging for host-pointer calls
   double *stW = nullptr, *stWt = nullptr, *stX = nullptr, *stE = nullptr;
+  // population control / estimators
+  double *cum = nullptr, *xi_dev = nullptr, *est_dev = nullptr, *ovlp_tmp = nullptr;
+  int* pmap = nullptr;
+  // CUDA graphs of whole blocks (afqmc_run_block on device buffers), keyed by the call's arguments
+  struct BlockGraph {
+    const void *W, *wt, *x, *xi, *E, *est;
+    int nw, n_steps, pop_every, ortho_phase;
+    double dt;
+    int seen;                 // eager runs so far with this key (the 2nd call captures)
+    cudaGraphExec_t exec;
+    int64_t launches;
+  };
+  std::vector<BlockGraph> graphs;
+  bool graph_on = true;
+  int64_t graph_replays = 0;
   int fb_split = 1;
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   bool ws_vhs = false;
@@ -198,6 +213,215 @@ int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw)
   return AFQMC_OK;
 }
 
+// One walker step on device buffers (rows a1-a10), stream ordered, no synchronisation.
+int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double dt, int nw) {
+  const int M = h->M, Nt = h->Nt, nc = h->n_chol;
+  const long MM = (long)M * M;
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
+
+  // a1/a2: overlap, Theta
+  {
+    StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+  }
+  // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
+  {
+    StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
+    GemmArgs g = gemm_args();
+    g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
+    g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
+    g.splitK = h->fb_split; g.sCsplit = (long)2 * h->maxw * nc;
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_nk(h->ThT, (long)Nt * M, h->Lrot, (long)Nt * M, h->Xp, nc, g.sCsplit, 2 * nw, nc, Nt * M,
+                         h->fb_split, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_NK, g, h->st);
+  }
+  // a4: shifted fields, scalars, V_HS coefficients
+  {
+    StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
+    ShiftArgs s;
+    s.Xp = h->Xp; s.sXp = (long)2 * h->maxw * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
+    s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
+    s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
+    h->launches += run_field_shift(s, nw, h->st);
+  }
+  // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
+  if (h->ws_vhs) {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
+    const int r = run_vhs_ws(h->Cf, h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw, h->st);
+    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
+    h->launches += r;
+  } else {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
+    GemmArgs g = gemm_args();
+    g.A = h->Cf; g.lda = nc; g.B = h->L; g.ldb = MM; g.C = h->A; g.ldc = MM;
+    g.M = 2 * nw; g.N = (int)MM; g.K = nc;
+    h->launches += run_gemm(GEMM_KN, g, h->st);
+  }
+  // a6: T0 = Acc = E1 phi
+  const long wstride = (long)M * 2 * Nt;
+  {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
+    g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 2, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+  }
+  // a7: T_n = A T_{n-1} / n, Acc += T_n
+  {
+    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
+    double *Tp = h->T0, *Tn = h->T1;
+    for (int n = 1; n <= h->K; ++n) {
+      GemmArgs g = gemm_args();
+      g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
+      g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
+      g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
+      int r = -1;
+      if (h->ws)
+        r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
+                           M, nw, 1.0 / n, 1, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
+      std::swap(Tp, Tn);
+    }
+  }
+  // a8: phi = E1 Acc, written into the caller's walkers
+  {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 0, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+  }
+  // a9: new overlap and weights
+  {
+    StageTimer tm(h, AFQMC_STAGE_OVERLAP_NEW);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_new, 0, 0), nw, h->st);
+  }
+  {
+    StageTimer tm(h, AFQMC_STAGE_WEIGHT);
+    WeightArgs a;
+    a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = h->cfb; a.cmf = h->cmf;
+    a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
+    a.expo = -dt * (h->E_const - h->e_shift);
+    h->launches += run_weight_update(a, nw, h->st);
+  }
+  // a10: re-orthonormalisation
+  h->step_count += 1;
+  h->last_nw = nw;
+  if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) {
+    StageTimer tm(h, AFQMC_STAGE_REORTHO);
+    QRArgs q;
+    q.W = W; q.detR = h->detR; q.M = M; q.Nt = Nt; q.nblk = h->nblk;
+    for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
+    h->launches += run_fill(h->detR, 1.0, (long)nw * h->nblk, h->st);
+    h->launches += run_cholqr_pass(q, nw, h->st);
+    h->launches += run_cholqr_pass(q, nw, h->st);
+    h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
+  }
+  return AFQMC_OK;
+}
+
+// Comb on device buffers: map -> h->pmap, weights in place, walkers and stored overlaps permuted.
+void population_control_device(afqmc_handle* h, double* W, double* wt, const double* xi_dev, int nw) {
+  StageTimer tm(h, AFQMC_STAGE_POP_CONTROL);
+  const long row_bytes = (long)h->M * h->Nt * 16;
+  h->launches += run_comb(wt, xi_dev, h->cum, h->pmap, nw, h->st);
+  h->launches += run_permute_rows(W, h->T0, h->pmap, row_bytes, nw, h->st);
+  if (h->last_nw == nw) h->launches += run_permute_rows(h->ovlp, h->ovlp_tmp, h->pmap, 16, nw, h->st);
+}
+
+void estimators_device(afqmc_handle* h, const double* wt, const double* E, double* out4, int nw) {
+  StageTimer tm(h, AFQMC_STAGE_ESTIMATORS);
+  h->launches += run_estimators(wt, E, out4, nw, h->st);
+}
+
+// The block loop on device buffers: stream ordered, no host synchronisation (capturable).
+int block_body_device(afqmc_handle* h, double* W, double* wt, const double* aux, const double* xi, double dt, int nw,
+                      int n_steps, int pop_every, double* E, double* est) {
+  int j = 0;
+  for (int s = 0; s < n_steps; ++s) {
+    const int rc = step_device(h, W, wt, aux + (size_t)s * nw * h->n_chol, dt, nw);
+    if (rc != AFQMC_OK) return rc;
+    if (pop_every > 0 && (s + 1) % pop_every == 0) population_control_device(h, W, wt, xi + j++, nw);
+  }
+  if (E) {
+    const int rc = local_energy_device(h, W, E, nw);
+    if (rc != AFQMC_OK) return rc;
+    if (est) estimators_device(h, wt, E, est, nw);
+  }
+  return AFQMC_OK;
+}
+
+// afqmc_run_block on device buffers: the first call with a given argument set runs eagerly
+// (it also pays every one-off cudaFuncSetAttribute), the second is captured into a CUDA graph,
+// later ones replay it.  The graph bakes in the pointers, sizes, dt and the phase of the
+// re-orthonormalisation schedule, which together form the key.
+int block_graphed(afqmc_handle* h, double* W, double* wt, const double* aux, const double* xi, double dt, int nw,
+                  int n_steps, int pop_every, double* E, double* est) {
+  if (!h->graph_on || h->prof)
+    return block_body_device(h, W, wt, aux, xi, dt, nw, n_steps, pop_every, E, est);
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
+  const int phase = h->p.ortho_every > 0 ? (int)(h->step_count % h->p.ortho_every) : 0;
+  afqmc_handle::BlockGraph* g = nullptr;
+  for (auto& c : h->graphs)
+    if (c.W == W && c.wt == wt && c.x == aux && c.xi == xi && c.E == E && c.est == est && c.nw == nw &&
+        c.n_steps == n_steps && c.pop_every == pop_every && c.ortho_phase == phase && c.dt == dt)
+      g = &c;
+  if (!g) {
+    if (h->graphs.size() >= 8) {
+      if (h->graphs.front().exec) cudaGraphExecDestroy(h->graphs.front().exec);
+      h->graphs.erase(h->graphs.begin());
+    }
+    h->graphs.push_back({W, wt, aux, xi, E, est, nw, n_steps, pop_every, phase, dt, 0, nullptr, 0});
+    g = &h->graphs.back();
+  }
+  if (g->exec) {
+    if (cudaGraphLaunch(g->exec, h->st) != cudaSuccess) return check_cuda(h, "cudaGraphLaunch");
+    h->step_count += n_steps;
+    h->last_nw = nw;
+    h->launches += g->launches;
+    h->graph_replays += 1;
+    return AFQMC_OK;
+  }
+  if (g->seen++ == 0) return block_body_device(h, W, wt, aux, xi, dt, nw, n_steps, pop_every, E, est);
+  // capture
+  const long sc0 = h->step_count;
+  const int64_t l0 = h->launches;
+  cudaGraph_t graph = nullptr;
+  if (cudaStreamBeginCapture(h->st, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+    cudaGetLastError();
+    h->graph_on = false;
+    return block_body_device(h, W, wt, aux, xi, dt, nw, n_steps, pop_every, E, est);
+  }
+  const int rc = block_body_device(h, W, wt, aux, xi, dt, nw, n_steps, pop_every, E, est);
+  const cudaError_t ce = cudaStreamEndCapture(h->st, &graph);
+  cudaGraphExec_t exec = nullptr;
+  if (rc != AFQMC_OK || ce != cudaSuccess || !graph || cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) {
+    cudaGetLastError();
+    if (graph) cudaGraphDestroy(graph);
+    h->graph_on = false;          // fall back to eager launches for good
+    h->step_count = sc0;
+    h->launches = l0;
+    return block_body_device(h, W, wt, aux, xi, dt, nw, n_steps, pop_every, E, est);
+  }
+  cudaGraphDestroy(graph);
+  g->exec = exec;
+  g->launches = h->launches - l0;
+  if (cudaGraphLaunch(exec, h->st) != cudaSuccess) return check_cuda(h, "cudaGraphLaunch");
+  h->graph_replays += 1;
+  return AFQMC_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -209,6 +433,8 @@ void afqmc_destroy(afqmc_handle* h) {
   cudaStreamSynchronize(h->st);
   for (void* p : h->allocs)
     if (p) cudaFree(p);
+  for (auto& g : h->graphs)
+    if (g.exec) cudaGraphExecDestroy(g.exec);
   for (auto& br : h->ev_pending) { cudaEventDestroy(br.a); cudaEventDestroy(br.b); }
   for (cudaEvent_t e : h->ev_free) cudaEventDestroy(e);
   if (h->own_stream) cudaStreamDestroy(h->st);
@@ -380,6 +606,10 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   }
   h->Xe = dalloc(h, (size_t)nc * mw * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
   h->stW = dalloc(h, wsz); h->stWt = dalloc(h, mw); h->stX = dalloc(h, (size_t)mw * nc); h->stE = dalloc(h, (size_t)mw * 6);
+  h->cum = dalloc(h, mw); h->xi_dev = dalloc(h, 4); h->est_dev = dalloc(h, 4); h->ovlp_tmp = dalloc(h, 2 * mw);
+  h->pmap = (int*)dalloc(h, (mw + 1) / 2 + 1);
+  if (!h->cum || !h->xi_dev || !h->est_dev || !h->ovlp_tmp || !h->pmap)
+    return bail(AFQMC_ERR_ALLOC, "device allocation failed (population control)");
   if (!h->det_old || !h->det_new || !h->ThT || !h->Xp || !h->X || !h->Cf || !h->cfb || !h->cmf || !h->A ||
       !h->T0 || !h->T1 || !h->Acc || !h->ovlp || !h->detR || !h->expart[0] || (h->nblk > 1 && !h->expart[1]) ||
       !h->Xe || !h->e1 || !h->stW || !h->stWt || !h->stX || !h->stE)
@@ -417,127 +647,17 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
-  const int M = h->M, Nt = h->Nt, nc = h->n_chol;
-  const long MM = (long)M * M;
-  const size_t wlen = (size_t)nw * M * 2 * Nt;
+  const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
   const bool hostW = !is_device_ptr(walkers), hostWt = !is_device_ptr(weights), hostX = !is_device_ptr(aux_fields);
   double* W = (double*)walkers;
   double* wt = weights;
   const double* x = aux_fields;
   if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
   if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
-  if (hostX) { to_device(h, h->stX, aux_fields, (size_t)nw * nc); x = h->stX; }
-
-  if (!(h->dt_cached == dt)) build_E1(h, dt);
-
-  // a1/a2: overlap, Theta
+  if (hostX) { to_device(h, h->stX, aux_fields, (size_t)nw * h->n_chol); x = h->stX; }
   {
-    StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
-    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
-  }
-  // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
-  {
-    StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
-    GemmArgs g = gemm_args();
-    g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
-    g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
-    g.splitK = h->fb_split; g.sCsplit = (long)2 * h->maxw * nc;
-    int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_nk(h->ThT, (long)Nt * M, h->Lrot, (long)Nt * M, h->Xp, nc, g.sCsplit, 2 * nw, nc, Nt * M,
-                         h->fb_split, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_NK, g, h->st);
-  }
-  // a4: shifted fields, scalars, V_HS coefficients
-  {
-    StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
-    ShiftArgs s;
-    s.Xp = h->Xp; s.sXp = (long)2 * h->maxw * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
-    s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
-    s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
-    h->launches += run_field_shift(s, nw, h->st);
-  }
-  // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
-  if (h->ws_vhs) {
-    StageTimer tm(h, AFQMC_STAGE_VHS);
-    const int r = run_vhs_ws(h->Cf, h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw, h->st);
-    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
-    h->launches += r;
-  } else {
-    StageTimer tm(h, AFQMC_STAGE_VHS);
-    GemmArgs g = gemm_args();
-    g.A = h->Cf; g.lda = nc; g.B = h->L; g.ldb = MM; g.C = h->A; g.ldc = MM;
-    g.M = 2 * nw; g.N = (int)MM; g.K = nc;
-    h->launches += run_gemm(GEMM_KN, g, h->st);
-  }
-  // a6: T0 = Acc = E1 phi
-  const long wstride = (long)M * 2 * Nt;
-  {
-    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
-    GemmArgs g = gemm_args();
-    g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
-    g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
-    g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 2, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
-  }
-  // a7: T_n = A T_{n-1} / n, Acc += T_n
-  {
-    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
-    double *Tp = h->T0, *Tn = h->T1;
-    for (int n = 1; n <= h->K; ++n) {
-      GemmArgs g = gemm_args();
-      g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
-      g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
-      g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
-      int r = -1;
-      if (h->ws)
-        r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
-                           M, nw, 1.0 / n, 1, h->st);
-      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
-      std::swap(Tp, Tn);
-    }
-  }
-  // a8: phi = E1 Acc, written into the caller's walkers
-  {
-    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
-    GemmArgs g = gemm_args();
-    g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
-    g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 0, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
-  }
-  // a9: new overlap and weights
-  {
-    StageTimer tm(h, AFQMC_STAGE_OVERLAP_NEW);
-    h->launches += run_overlap_theta(ot_args(h, W, h->det_new, 0, 0), nw, h->st);
-  }
-  {
-    StageTimer tm(h, AFQMC_STAGE_WEIGHT);
-    WeightArgs a;
-    a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = h->cfb; a.cmf = h->cmf;
-    a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
-    a.expo = -dt * (h->E_const - h->e_shift);
-    h->launches += run_weight_update(a, nw, h->st);
-  }
-  // a10: re-orthonormalisation
-  h->step_count += 1;
-  h->last_nw = nw;
-  if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) {
-    StageTimer tm(h, AFQMC_STAGE_REORTHO);
-    QRArgs q;
-    q.W = W; q.detR = h->detR; q.M = M; q.Nt = Nt; q.nblk = h->nblk;
-    for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
-    h->launches += run_fill(h->detR, 1.0, (long)nw * h->nblk, h->st);
-    h->launches += run_cholqr_pass(q, nw, h->st);
-    h->launches += run_cholqr_pass(q, nw, h->st);
-    h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
+    const int rc = step_device(h, W, wt, x, dt, nw);
+    if (rc != AFQMC_OK) return rc;
   }
   if (hostW) cudaMemcpyAsync(walkers, W, wlen * 8, cudaMemcpyDeviceToHost, h->st);
   if (hostWt) cudaMemcpyAsync(weights, wt, (size_t)nw * 8, cudaMemcpyDeviceToHost, h->st);
@@ -566,6 +686,106 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
     if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_local_energy");
   }
   return check_cuda(h, "afqmc_local_energy");
+}
+
+int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi, int32_t nw,
+                                 int32_t* map_out) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!walkers || !weights || !xi) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
+  const bool hostW = !is_device_ptr(walkers), hostWt = !is_device_ptr(weights), hostXi = !is_device_ptr(xi);
+  if (hostXi && !(xi[0] >= 0.0 && xi[0] < 1.0)) return fail(h, AFQMC_ERR_INVALID, "xi must be in [0, 1)");
+  double* W = (double*)walkers;
+  double* wt = weights;
+  const double* xd = xi;
+  if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
+  if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
+  if (hostXi) { to_device(h, h->xi_dev, xi, 1); xd = h->xi_dev; }
+  population_control_device(h, W, wt, xd, nw);
+  bool sync = false;
+  if (hostW) { cudaMemcpyAsync(walkers, W, wlen * 8, cudaMemcpyDeviceToHost, h->st); sync = true; }
+  if (hostWt) { cudaMemcpyAsync(weights, wt, (size_t)nw * 8, cudaMemcpyDeviceToHost, h->st); sync = true; }
+  if (map_out) {
+    cudaMemcpyAsync(map_out, h->pmap, (size_t)nw * 4, cudaMemcpyDefault, h->st);
+    if (!is_device_ptr(map_out)) sync = true;
+  }
+  if (sync && cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_population_control");
+  return check_cuda(h, "afqmc_population_control");
+}
+
+int32_t afqmc_estimators(afqmc_handle* h, const double* weights, const void* E, double* est_out, int32_t nw) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!weights || !E || !est_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  const bool hostWt = !is_device_ptr(weights), hostE = !is_device_ptr(E), hostO = !is_device_ptr(est_out);
+  const double* wt = weights;
+  const double* Ed = (const double*)E;
+  if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
+  if (hostE) { to_device(h, h->stE, E, (size_t)nw * 6); Ed = h->stE; }
+  double* out = hostO ? h->est_dev : est_out;
+  estimators_device(h, wt, Ed, out, nw);
+  if (hostO) {
+    cudaMemcpyAsync(est_out, out, 32, cudaMemcpyDeviceToHost, h->st);
+    if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_estimators");
+  }
+  return check_cuda(h, "afqmc_estimators");
+}
+
+int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, const double* xi,
+                        double dt, int32_t nw, int32_t n_steps, int32_t pop_every, void* E_out, double* est_out) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  if (n_steps <= 0 || pop_every < 0) return fail(h, AFQMC_ERR_INVALID, "bad n_steps / pop_every");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
+  const int n_pop = pop_every > 0 ? n_steps / pop_every : 0;
+  if (n_pop > 0 && !xi) return fail(h, AFQMC_ERR_INVALID, "xi is needed when pop_every > 0");
+  const int nc = h->n_chol;
+  const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
+  const bool hostW = !is_device_ptr(walkers), hostWt = !is_device_ptr(weights), hostX = !is_device_ptr(aux_fields);
+  const bool hostXi = n_pop > 0 && !is_device_ptr(xi);
+  const bool hostE = E_out && !is_device_ptr(E_out), hostO = est_out && !is_device_ptr(est_out);
+  if (hostXi)
+    for (int j = 0; j < n_pop; ++j)
+      if (!(xi[j] >= 0.0 && xi[j] < 1.0)) return fail(h, AFQMC_ERR_INVALID, "xi must be in [0, 1)");
+  double* W = (double*)walkers;
+  double* wt = weights;
+  if (!hostW && !hostWt && !hostX && !hostXi && !hostE && !hostO) {
+    double* E = E_out ? (double*)E_out : (est_out ? h->stE : nullptr);
+    const int rc = block_graphed(h, W, wt, aux_fields, xi, dt, nw, n_steps, pop_every, E, est_out);
+    return rc != AFQMC_OK ? rc : check_cuda(h, "afqmc_run_block");
+  }
+  if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
+  if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
+  int j = 0;
+  for (int s = 0; s < n_steps; ++s) {
+    const double* x = aux_fields + (size_t)s * nw * nc;
+    if (hostX) { to_device(h, h->stX, x, (size_t)nw * nc); x = h->stX; }
+    const int rc = step_device(h, W, wt, x, dt, nw);
+    if (rc != AFQMC_OK) return rc;
+    if (pop_every > 0 && (s + 1) % pop_every == 0) {
+      const double* xd = xi + j;
+      // a host xi is staged one value at a time: the copy is stream ordered before its comb
+      if (hostXi) { to_device(h, h->xi_dev + (j & 3), xi + j, 1); xd = h->xi_dev + (j & 3); }
+      population_control_device(h, W, wt, xd, nw);
+      ++j;
+    }
+  }
+  if (E_out || est_out) {
+    double* E = (hostE || !E_out) ? h->stE : (double*)E_out;
+    const int rc = local_energy_device(h, W, E, nw);
+    if (rc != AFQMC_OK) return rc;
+    if (est_out) estimators_device(h, wt, E, hostO ? h->est_dev : est_out, nw);
+    if (hostE) cudaMemcpyAsync(E_out, E, (size_t)nw * 48, cudaMemcpyDeviceToHost, h->st);
+    if (hostO) cudaMemcpyAsync(est_out, h->est_dev, 32, cudaMemcpyDeviceToHost, h->st);
+  }
+  if (hostW) cudaMemcpyAsync(walkers, W, wlen * 8, cudaMemcpyDeviceToHost, h->st);
+  if (hostWt) cudaMemcpyAsync(weights, wt, (size_t)nw * 8, cudaMemcpyDeviceToHost, h->st);
+  if (hostW || hostWt || hostE || hostO) {
+    if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_run_block");
+  }
+  return check_cuda(h, "afqmc_run_block");
 }
 
 int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out) {
@@ -605,6 +825,12 @@ int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
   if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_debug_read");
   int rc = check_cuda(h, "afqmc_debug_read");
   return rc == AFQMC_OK ? n : rc;
+}
+
+int64_t afqmc_set_block_graph(afqmc_handle* h, int32_t on) {
+  if (!h) return AFQMC_ERR_INVALID;
+  if (on >= 0) h->graph_on = on != 0;
+  return h->graph_replays;
 }
 
 int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on) {

@@ -114,6 +114,11 @@ int gemm_ws_nk_split(int M, int N, int K, int max_split);
 int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double* C, long ldc, long sCsplit,
                    int M, int N, int K, int split, cudaStream_t st);
 
+// block.cu: population control (comb), walker permutation, estimator sums
+int run_comb(double* weights, const double* xi, double* cum, int* map, int nw, cudaStream_t st);
+int run_permute_rows(void* rows, void* tmp, const int* map, long row_bytes, int nw, cudaStream_t st);
+int run_estimators(const double* weights, const double* E, double* out4, int nw, cudaStream_t st);
+
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);
 int run_sum_mL(const double* L, const double* m, double* out, int M, int n_chol, cudaStream_t st);

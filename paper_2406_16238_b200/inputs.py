@@ -15,7 +15,7 @@ from dataclasses import dataclass
 import numpy as np
 
 __all__ = ["Config", "CONFIGS", "get_config", "make_h1", "make_trial", "make_walkers",
-           "make_aux_fields", "chol_scale", "make_L_slab", "make_L_host", "make_L_device",
+           "make_aux_fields", "make_pop_uniforms", "chol_scale", "make_L_slab", "make_L_host", "make_L_device",
            "device_slab_provider", "make_problem_host"]
 
 
@@ -104,6 +104,12 @@ def make_aux_fields(cfg, seed, step, nw=None):
     """x[w, g] ~ N(0, 1) float64 for one step; host-drawn, fed identically to both paths."""
     nw = cfg.nw if nw is None else nw
     return _rng(seed, 1000, step).standard_normal((nw, cfg.n_chol))
+
+
+def make_pop_uniforms(seed, n, block=0):
+    """xi[j] ~ U[0, 1) float64, one per population-control call of a block; host-drawn, fed
+    identically to both paths (the library draws no random numbers)."""
+    return _rng(seed, 2000, block).random(n)
 
 
 def chol_scale(cfg, literal=False):

@@ -203,6 +203,7 @@ def test_full_size_sampled_walkers(name, idx, device_L):
         Wr, wr = Wg.clone(), wg.clone()
         Wr[ti] = torch.from_numpy(Wo).cuda()
         wr[ti] = torch.from_numpy(wo).cuda()
+        torch.cuda.synchronize()          # the library runs on its own stream, torch on another
         pr.gpu.step(Wr, wr, xd, cfg.dt)
         pr.gpu.get_overlaps(ov)
         pr.gpu.sync()
@@ -219,6 +220,7 @@ def test_full_size_sampled_walkers(name, idx, device_L):
     assert np.all(wo > 0)
     assert bool(torch.all(torch.isfinite(wg))) and bool(torch.all(wg >= 0))
     E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
     pr.gpu.local_energy(Wg, E)
     pr.gpu.sync()
     E_g = E[ti].cpu().numpy()
