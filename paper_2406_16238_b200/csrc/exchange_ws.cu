@@ -127,6 +127,7 @@ exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant_
     for (int kt = 0; kt < KT; ++kt, ++it) {
       const int s = it % S;
       mbar_wait(&full[s], (it / S) & 1);
+      consumer_release_prev(empty, it, S, lane);
       const uint32_t sa = tiles_u32 + (uint32_t)s * Cfg::STAGE_BYTES + aoff;
       const uint32_t sb = tiles_u32 + (uint32_t)s * Cfg::STAGE_BYTES + boff;
 #pragma unroll
@@ -144,8 +145,6 @@ exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant_
           for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, bf.y);
         }
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[s]);
     }
 
     // ------------------------------------------------------------------ epilogue

@@ -133,6 +133,7 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
     for (int kt = 0; kt < KT; ++kt, ++it) {
       const int s = it % S;
       mbar_wait(&full[s], (it / S) & 1);
+      consumer_release_prev(empty, it, S, lane);
       const uint32_t sa = smem_u + (uint32_t)s * Cfg::STAGE_BYTES + aoff;
       const uint32_t sb = smem_u + (uint32_t)s * Cfg::STAGE_BYTES + Cfg::A_BYTES;
 #pragma unroll
@@ -157,8 +158,6 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
             for (int i = 0; i < MI; ++i) dmma884(acc[pl][i][j][0], acc[pl][i][j][1], af[pl][i].y, b1);
         }
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[s]);
     }
 
     double* C = a.C + (size_t)b * a.sC;
@@ -308,6 +307,7 @@ gemm_ws_nk_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
     for (int k0 = kbeg; k0 < kend; k0 += 16, ++it) {
       const int s = it % S;
       mbar_wait(&full[s], (it / S) & 1);
+      consumer_release_prev(empty, it, S, lane);
       const uint32_t sa = smem_u + (uint32_t)s * NK_STAGE + aoff;
       const uint32_t sb = smem_u + (uint32_t)s * NK_STAGE + boff;
 #pragma unroll
@@ -325,8 +325,6 @@ gemm_ws_nk_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
           for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, bf.y);
         }
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[s]);
     }
 
     double* C = a.C + (size_t)ks * a.sCsplit;

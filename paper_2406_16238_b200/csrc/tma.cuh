@@ -62,6 +62,16 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
   while (!mbar_try_wait(bar, parity)) {}
 }
+// Consumer release of a ring stage, LAGGED BY ONE ITERATION.  Releasing stage `it` right after its
+// fragment loads lets ptxas place the mbarrier.arrive directly behind the last LDS, ahead of the
+// DMMAs that consume it; that LDS can then still be in flight when the producer's TMA refills the
+// stage (seen on B200 as one warp's last-loaded B fragment of one stage going stale, about once per
+// 1e6 stages).  Called right after the full-barrier wait of iteration `it`, it releases the stage of
+// iteration it - 1: every DMMA of that iteration sits before the wait loop, and a DMMA cannot
+// issue before the LDS feeding it has returned.  Costs one stage of prefetch depth.
+__device__ __forceinline__ void consumer_release_prev(uint64_t* empty, uint32_t it, int stages, int lane) {
+  if (it > 0 && lane == 0) mbar_arrive(&empty[(it - 1) % stages]);
+}
 // named barrier among `count` threads (count a multiple of 32), id 1..15
 __device__ __forceinline__ void named_bar_sync(int id, int count) {
   asm volatile("bar.sync %0, %1;\n" ::"r"(id), "r"(count) : "memory");

@@ -115,6 +115,7 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
     for (int kt = 0; kt < KT; ++kt, ++it) {
       const int s = it % STAGESv;
       mbar_wait(&full[s], (it / STAGESv) & 1);
+      consumer_release_prev(empty, it, STAGESv, lane);
       const uint32_t sa = smem_u + (uint32_t)s * STAGE_BYTESv + aoff;
       const uint32_t sb = smem_u + (uint32_t)s * STAGE_BYTESv + A_BYTES;
 #pragma unroll
@@ -137,8 +138,6 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
 #pragma unroll
           for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, b1[j]);
       }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&empty[s]);
     }
 
     // ---- epilogue: direct store at [p][q] (q >= p) and mirrored store at [q][p] (q > p)
