@@ -147,3 +147,44 @@ def test_run_block_matches_the_oracle_block_loop(name, nw, n_steps, pop_every, o
     assert np.array_equal(En, E.cpu().numpy()) and np.array_equal(estn, est.cpu().numpy())
     pr2.close()
     pr.close()
+
+
+@pytest.mark.parametrize("name,nw,ortho", [("c1", 16, 5), ("c2", 32, 3)])
+def test_run_block_graph_replay_is_bit_identical_to_eager_launches(name, nw, ortho):
+    """Third call on with the same buffers replays a CUDA graph of the whole block: same bits as
+    the eager launches, including the phase of the QR schedule that the graph bakes in."""
+    torch = _torch()
+    pr = Pair(name, nw=nw, ortho_every=ortho, oracle=False)
+    cfg = pr.cfg
+    n_steps, pop_every = 10, 5          # 10 % 3 != 0 for c2: the ortho phase changes from block to block
+    x = torch.from_numpy(np.stack([pr.fields(s) for s in range(n_steps)])).cuda()
+    xi = torch.from_numpy(inputs.make_pop_uniforms(0, 2)).cuda()
+    W0 = torch.from_numpy(pr.walkers0).cuda()
+    W, w = torch.empty_like(W0), torch.empty(nw, dtype=torch.float64, device="cuda")
+    E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    est = torch.empty(4, dtype=torch.float64, device="cuda")
+
+    def blocks(n):
+        out = []
+        for _ in range(n):
+            W.copy_(W0); w.fill_(1.0)
+            torch.cuda.synchronize()
+            pr.gpu.run_block(W, w, x, xi, cfg.dt, pop_every, E, est)
+            pr.gpu.sync()
+            out.append((W.cpu().numpy(), w.cpu().numpy(), E.cpu().numpy(), est.cpu().numpy()))
+        return out
+
+    pr.gpu.set_block_graph(0)
+    eager = blocks(6)
+    assert pr.gpu.set_block_graph(-1) == 0
+    pr2 = Pair(name, nw=nw, ortho_every=ortho, oracle=False)       # fresh handle: same QR phases
+    gpu_keep = pr.gpu
+    pr.gpu = pr2.gpu
+    graphed = blocks(6)
+    assert pr2.gpu.set_block_graph(-1) >= (1 if n_steps % ortho else 4)
+    for a, b in zip(eager, graphed):
+        for u, v in zip(a, b):
+            assert np.array_equal(u, v)
+    pr.gpu = gpu_keep
+    pr2.close()
+    pr.close()
