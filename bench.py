@@ -247,6 +247,9 @@ def main():
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--pack-chol", action="store_true",
+                    help="handle keeps the tile-packed upper triangles of L (PAPER.md:205); the dense tensor is "
+                         "freed after afqmc_create")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
     ap.add_argument("--profiler-range", action="store_true",
@@ -286,7 +289,11 @@ def main():
     g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta,
                     n_chol=cfg.n_chol, max_walkers=nw, walker_kind=cfg.walker_kind,
                     taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every,
-                    stream=stream.cuda_stream)
+                    stream=stream.cuda_stream, pack_chol=args.pack_chol)
+    if args.pack_chol:
+        Ld = None
+        torch.cuda.empty_cache()
+    hbm_resident_gb = (torch.cuda.mem_get_info()[1] - torch.cuda.mem_get_info()[0]) / 1e9
     peak_dmma, peak_dfma, _ = afqmc.measure_fp64_peak(200.0)
 
     walkers_h = inputs.make_walkers(cfg, trial, seed, nw)
@@ -399,6 +406,7 @@ def main():
                    "n_chol": cfg.n_chol, "n_walkers_per_gpu": nw, "dt": cfg.dt,
                    "taylor_order": cfg.taylor_order, "ortho_every": cfg.ortho_every,
                    "local_energy": "every step", "parallelism": f"replicas x{world}",
+                   "pack_chol": bool(args.pack_chol), "hbm_resident_gb": round(hbm_resident_gb, 1),
                    "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "stages": per_stage, "block": block,
@@ -409,6 +417,8 @@ def main():
 
     if want_cpu:
         g.close()
+        if Ld is None:
+            Ld, _ = make_L(cfg, 0, False, True)
         Lh = Ld.cpu().numpy()
         del Ld
         torch.cuda.empty_cache()

@@ -62,6 +62,10 @@ typedef struct {
   int32_t e_shift_auto; /* 1: E_shift = local energy of the trial; 0: use e_shift         */
   double e_shift;       /* energy shift in the weight, exp(-dt (E_const - E_shift))       */
   void* stream;         /* cudaStream_t to run on; NULL = the library creates its own     */
+  int32_t pack_chol;    /* 1: keep a tile-packed copy of the upper triangle of every L_g    */
+                        /* (the paper's pack_chol) and stop borrowing L_chol  */
+                        /* when afqmc_create returns; needs even M and n_chol               */
+  int32_t reserved;     /* 0                                                              */
 } afqmc_params;
 
 /* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;
@@ -70,7 +74,11 @@ typedef struct {
  * hrot = trial^T h1 and (if e_shift_auto) the trial's local energy, all on the device.
  *   h1     EITHER [M][M] symmetric, COPIED.
  *   L_chol DEVICE [n_chol][M][M], each L_g symmetric; BORROWED read-only until afqmc_destroy
- *          (it is the dominant resident array, 55 GB in the largest configuration).
+ *          (it is the dominant resident array, 55 GB in the largest configuration).  With
+ *          pack_chol = 1 it is borrowed only for the duration of afqmc_create: the handle keeps
+ *          Lrot and a tile-packed copy of the upper triangles ([tiles][n_chol][4][32] doubles,
+ *          0.53x the dense size at M = 1200) and every later call gives the same bits as with
+ *          the dense tensor, so the caller may free L_chol afterwards.
  *   trial  EITHER [M][Nt] real, COPIED.
  *   out    receives the handle; NULL on failure. */
 int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial,

@@ -30,7 +30,8 @@ class AfqmcParams(C.Structure):
                 ("n_beta", C.c_int32), ("n_chol", C.c_int32), ("max_walkers", C.c_int32),
                 ("walker_kind", C.c_int32), ("taylor_order", C.c_int32),
                 ("ortho_every", C.c_int32), ("e_shift_auto", C.c_int32),
-                ("e_shift", C.c_double), ("stream", C.c_void_p)]
+                ("e_shift", C.c_double), ("stream", C.c_void_p), ("pack_chol", C.c_int32),
+                ("reserved", C.c_int32)]
 
 
 def _load():
@@ -113,7 +114,7 @@ class AFQMC:
     """Handle wrapper with the same calls as the C ABI."""
 
     def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
-                 walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None):
+                 walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False):
         p = AfqmcParams()
         p.struct_size = C.sizeof(AfqmcParams)
         p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
@@ -122,7 +123,9 @@ class AFQMC:
         p.e_shift_auto = 1 if e_shift is None else 0
         p.e_shift = 0.0 if e_shift is None else float(e_shift)
         p.stream = stream
-        self._keep = (h1, L_chol, trial)     # L_chol is borrowed by the library
+        p.pack_chol = 1 if pack_chol else 0
+        # L_chol is borrowed by the library (only during create when pack_chol is set)
+        self._keep = (h1, None if pack_chol else L_chol, trial)
         self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers
         self.Nt = n_alpha if walker_kind == 0 else n_alpha + n_beta
         h = C.c_void_p()

@@ -52,6 +52,7 @@ struct afqmc_handle {
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   bool ws_vhs = false;
   int* vhs_tiles = nullptr;
+  double* Lpk = nullptr;   // tile-packed upper triangle of L (pack_chol)
   int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
@@ -249,7 +250,8 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
   if (h->ws_vhs) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
-    const int r = run_vhs_ws(h->Cf, h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw, h->st);
+    const int r = run_vhs_ws(h->Cf, h->Lpk ? h->Lpk : h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw,
+                             h->Lpk != nullptr, h->st);
     if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
     h->launches += r;
   } else {
@@ -447,7 +449,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (!h1 || !L_chol || !trial || !p || !out) return fail(nullptr, AFQMC_ERR_INVALID, "null argument");
   if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
   if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
-      p->ortho_every < 0 || p->taylor_order < 0 || (p->walker_kind != 0 && p->walker_kind != 1))
+      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
     return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
   if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
   if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
@@ -625,6 +627,13 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
       return bail(AFQMC_ERR_CUDA, "tile list upload failed");
   }
 
+  if (p->pack_chol) {
+    if (!h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "pack_chol needs even M and n_chol (TMA strides)");
+    h->Lpk = dalloc(h, vhs_ws_packed_doubles(h->vhs_ntile, nc));
+    if (!h->Lpk) return bail(AFQMC_ERR_ALLOC, "device allocation failed (packed Cholesky tensor)");
+    h->launches += run_pack_tiles(h->L, h->Lpk, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
+  }
+
   // ---- E_shift = trial energy ---------------------------------------------------------------
   {
     std::vector<double> wt((size_t)M * Nt * 2, 0.0);
@@ -638,6 +647,10 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->e_trial = e[0];
   }
   h->e_shift = p->e_shift_auto ? h->e_trial : p->e_shift;
+  if (h->Lpk) {                      // the dense tensor is not touched after this point
+    if (cudaStreamSynchronize(h->st) != cudaSuccess) return bail(AFQMC_ERR_CUDA, "pack_chol failed");
+    h->L = nullptr;
+  }
   *out = h;
   return AFQMC_OK;
 }

@@ -104,7 +104,11 @@ int run_energy_reduce2(const EnergyArgs& a, const double* expart2, int ngroups2,
 bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void* C);
 int vhs_ws_tile_list(int M, std::vector<int>* out);
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
-               int n_chol, int rows, cudaStream_t st);
+               int n_chol, int rows, bool packed, cudaStream_t st);
+// tile-packed upper triangle of L (the paper's pack_chol): [ntile_n][n_chol][4][32]
+size_t vhs_ws_packed_doubles(int ntile_n, int n_chol);
+int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
+                   cudaStream_t st);
 
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,

@@ -35,6 +35,7 @@ struct VhsArgs {
   int ntile_n, mtiles;
 };
 
+template <bool PACKED>
 __global__ void __launch_bounds__(THREADSv, 1)
 vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB, const VhsArgs a) {
   extern __shared__ unsigned char smem_raw[];
@@ -58,7 +59,8 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       prefetch_tensormap(&tmB);
       uint32_t it = 0;
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int tn = a.tiles[tile / a.mtiles], mt = tile % a.mtiles;
+        const int tl = tile / a.mtiles;                // position in the upper-triangle tile list
+        const int tn = a.tiles[tl], mt = tile % a.mtiles;
         const int p0 = (tn >> 16) * PT, q0 = (tn & 0xffff) * QT;
         for (int kt = 0; kt < KT; ++kt, ++it) {
           const int s = it % STAGESv;
@@ -71,7 +73,10 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
           for (int pl = 0; pl < PT; ++pl)
 #pragma unroll
             for (int qb = 0; qb < QT / 16; ++qb)
-              tma_load_3d(sb + (pl * (QT / 16) + qb) * B_BOX, &tmB, &full[s], q0 + 16 * qb, p0 + pl, kt * BKv);
+              if (PACKED)   // tile-packed copy [tile][gamma][pl][q]: box (pl, qb) of tile tl
+                tma_load_4d(sb + (pl * (QT / 16) + qb) * B_BOX, &tmB, &full[s], 0, pl * (QT / 16) + qb, kt * BKv, tl);
+              else
+                tma_load_3d(sb + (pl * (QT / 16) + qb) * B_BOX, &tmB, &full[s], q0 + 16 * qb, p0 + pl, kt * BKv);
         }
       }
     }
@@ -178,7 +183,28 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
   }
 }
 
+// Lpk[t][g][pl][q] = L[g][p0(t) + pl][q0(t) + q] (zero outside the matrix); grid (ntile_n, gamma chunks)
+__global__ void __launch_bounds__(PT * QT) pack_tiles_kernel(const double* L, double* Lpk, const int* tiles, int M,
+                                                             int n_chol) {
+  const int t = blockIdx.x;
+  const int tn = tiles[t];
+  const int p = (tn >> 16) * PT + threadIdx.x / QT, q = (tn & 0xffff) * QT + threadIdx.x % QT;
+  const bool in = p < M && q < M;
+  const size_t MM = (size_t)M * M;
+  for (int g = blockIdx.y; g < n_chol; g += gridDim.y)
+    Lpk[((size_t)t * n_chol + g) * (PT * QT) + threadIdx.x] = in ? L[(size_t)g * MM + (size_t)p * M + q] : 0.0;
+}
+
 }  // namespace
+
+size_t vhs_ws_packed_doubles(int ntile_n, int n_chol) { return (size_t)ntile_n * n_chol * PT * QT; }
+
+int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
+                   cudaStream_t st) {
+  const int gy = n_chol < 64 ? n_chol : 64;
+  pack_tiles_kernel<<<dim3(ntile_n, gy), PT * QT, 0, st>>>(L, Lpk, tiles_dev, M, n_chol);
+  return 1;
+}
 
 // host: list of (p-block, q-block) tiles that intersect the upper triangle, row-major
 int vhs_ws_tile_list(int M, std::vector<int>* out) {
@@ -197,10 +223,11 @@ bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void*
 
 // algorithmic flops actually needed with the symmetric half: 2 * rows * n_chol * M (M + 1) / 2 * 2
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
-               int n_chol, int rows, cudaStream_t st) {
+               int n_chol, int rows, bool packed, cudaStream_t st) {
   static bool attr = false;
   if (!attr) {
-    cudaFuncSetAttribute(vhs_ws_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
+    cudaFuncSetAttribute(vhs_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
+    cudaFuncSetAttribute(vhs_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
     attr = true;
   }
   static int nsm = 0;
@@ -217,7 +244,12 @@ int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_de
     const uint32_t box[2] = {BKv, BMv};
     if (make_tensor_map_f64(&tmA, Cf, 2, dims, str, box) != 0) return -1;
   }
-  {
+  if (packed) {   // L = the tile-packed copy [ntile_n][n_chol][PT * QT / 16][16]
+    const uint64_t dims[4] = {16, (uint64_t)(PT * QT / 16), (uint64_t)n_chol, (uint64_t)ntile_n};
+    const uint64_t str[3] = {128, (uint64_t)PT * QT * 8, (uint64_t)n_chol * PT * QT * 8};
+    const uint32_t box[4] = {16, 1, BKv, 1};
+    if (make_tensor_map_f64(&tmB, L, 4, dims, str, box) != 0) return -1;
+  } else {
     const uint64_t dims[3] = {(uint64_t)M, (uint64_t)M, (uint64_t)n_chol};
     const uint64_t str[2] = {(uint64_t)M * 8, (uint64_t)M * M * 8};
     const uint32_t box[3] = {16, 1, BKv};
@@ -228,7 +260,8 @@ int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_de
   a.ntile_n = ntile_n; a.mtiles = (rows + BMv - 1) / BMv;
   const long nt = (long)a.ntile_n * a.mtiles;
   const int grid = nt < nsm ? (int)nt : nsm;
-  vhs_ws_kernel<<<grid, THREADSv, SMEMv, st>>>(tmA, tmB, a);
+  if (packed) vhs_ws_kernel<true><<<grid, THREADSv, SMEMv, st>>>(tmA, tmB, a);
+  else vhs_ws_kernel<false><<<grid, THREADSv, SMEMv, st>>>(tmA, tmB, a);
   return 1;
 }
 

@@ -234,6 +234,44 @@ def test_full_size_sampled_walkers(name, idx, device_L):
     pr.close()
 
 
+# --------------------------------------------------------------------------- packed Cholesky tensor
+@pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 24, {}),
+                                          ("c1", 5, dict(M=70, n_alpha=9, n_beta=9, n_chol=54)),
+                                          ("c1", 3, dict(M=130, n_alpha=12, n_beta=12, n_chol=50))])
+def test_pack_chol_gives_the_same_bits_and_releases_L(name, nw, over):
+    """pack_chol: the handle keeps a tile-packed copy of the upper triangles and no
+    longer reads the caller's dense tensor after afqmc_create (it is overwritten with NaN here);
+    steps and energies are bit-identical to the dense-tensor handle and match the oracle."""
+    torch = _torch()
+    dense = Pair(name, nw=nw, **over)
+    packed = Pair(name, nw=nw, oracle=False, pack_chol=True, **over)
+    packed.L_dev.fill_(float("nan"))
+    torch.cuda.synchronize()
+    cfg = dense.cfg
+    Wd, wd = dense.walkers0.copy(), np.ones(nw)
+    Wp, wp = dense.walkers0.copy(), np.ones(nw)
+    Wo, wo = dense.walkers0.copy(), np.ones(nw)
+    for s in range(3):
+        x = dense.fields(s)
+        Wd, wd, ovd = gpu_step(dense, Wd, wd, x, cfg.dt)
+        Wp, wp, ovp = gpu_step(packed, Wp, wp, x, cfg.dt)
+        assert np.array_equal(dense.gpu.debug_read(1), packed.gpu.debug_read(1))      # A = V_HS
+        assert np.array_equal(Wd, Wp) and np.array_equal(wd, wp) and np.array_equal(ovd, ovp)
+        Wo, wo, ovo = dense.oracle.step(Wo, wo, x, cfg.dt)
+    assert rel_fro(Wp, Wo) < TOL_RUN and rel_max(wp, wo) < TOL_RUN and rel_max(ovp, ovo) < TOL_RUN
+    assert np.array_equal(gpu_energy(dense, Wd), gpu_energy(packed, Wp))
+    dense.close()
+    packed.close()
+
+
+def test_pack_chol_needs_even_dimensions():
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc
+    with pytest.raises(afqmc.AfqmcError) as e:
+        Pair("c1", nw=2, oracle=False, pack_chol=True, M=37, n_alpha=7, n_beta=7, n_chol=53)
+    assert e.value.code == -6
+
+
 # --------------------------------------------------------------------------- boundary behaviour
 def test_host_pointers_equal_device_pointers():
     torch = _torch()
