@@ -65,7 +65,11 @@ typedef struct {
   int32_t pack_chol;    /* 1: keep a tile-packed copy of the upper triangle of every L_g    */
                         /* (the paper's pack_chol) and stop borrowing L_chol  */
                         /* when afqmc_create returns; needs even M and n_chol               */
-  int32_t reserved;     /* 0                                                              */
+  int32_t group_size;   /* distributed Hamiltonian: members G of the group that  */
+                        /* shares one Cholesky tensor, 0 or 1 = none, at most 8; with G > 1 L_chol, */
+                        /* n_chol describe THIS member's gamma slice and max_walkers its own walkers */
+  int32_t group_rank;   /* this member's index in the group, 0 .. G-1                             */
+  int32_t reserved;     /* 0                                                                      */
 } afqmc_params;
 
 /* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;
@@ -185,7 +189,9 @@ int64_t afqmc_launch_count(const afqmc_handle* h);
 #define AFQMC_STAGE_E1_BUILD 12      /* expm(-dt/2 h_mod), only when dt changes               */
 #define AFQMC_STAGE_POP_CONTROL 13   /* comb + walker permutation                            */
 #define AFQMC_STAGE_ESTIMATORS 14    /* weighted sums of Code Snippet 9                       */
-#define AFQMC_STAGE_COUNT 15
+#define AFQMC_STAGE_SHARD_EXCHANGE 15 /* distributed Hamiltonian: pushes into peer slots (copies)  */
+#define AFQMC_STAGE_SHARD_REDUCE 16   /* distributed Hamiltonian: fixed-order sums of the slots    */
+#define AFQMC_STAGE_COUNT 17
 int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on);
 /*   ms_out HOST double [AFQMC_STAGE_COUNT]; count_out HOST int64 [AFQMC_STAGE_COUNT] or NULL. */
 int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset);
@@ -196,6 +202,73 @@ int32_t afqmc_sync(afqmc_handle* h);
 const char* afqmc_last_error(const afqmc_handle* h);
 
 void afqmc_destroy(afqmc_handle* h);
+
+/* ---- Distributed Hamiltonian ("Distributed Hamiltonian for limited memory", PAPER.md:308-318,
+ * Fig. 6) -------------------------------------------------------------------
+ * When the Cholesky tensor does not fit one GPU it is split over the gamma index among the G
+ * members of a group; every member owns its own nw walkers.  Everything that is a sum over gamma
+ *     h_mod - h1, E_const, A = V_HS (Eq. 9), c_fb, c_mf (Eqs. 12, 16), E_C + E_X (Eq. 11)
+ * is computed slice by slice by the member holding the slice FOR ALL G * nw WALKERS OF THE GROUP
+ * and added up by the walker's owner in fixed member order 0 .. G-1 (results do not depend on
+ * timing).  The paper passes walkers cyclically over MPI; here the members' buffers
+ * are mapped into each other's address space (NVLink peer memory, CUDA IPC between processes, or
+ * simply the same device) and
+ *   - Theta^T of a member's walkers is pushed into every member's gather buffer (slot = owner),
+ *   - the V_HS kernel's epilogue stores each walker's partial A straight into its OWNER's receive
+ *     slot [source member] (the scatter of the reduce-scatter is the GEMM epilogue itself),
+ *   - the partial scalars and energies follow the same way.
+ * The library never synchronises members: the caller puts a group barrier ORDERED ON EVERY
+ * MEMBER'S STREAM (e.g. a one-element NCCL all-reduce on that stream, or a stream synchronise
+ * plus a host barrier) where "== barrier ==" stands below.  One step of the whole group is
+ *     afqmc_shard_theta(for_energy = 0)  == barrier ==  afqmc_shard_vhs  == barrier ==
+ *     afqmc_shard_propagate
+ * and one local-energy evaluation
+ *     afqmc_shard_theta(for_energy = 1)  == barrier ==  afqmc_shard_energy  == barrier ==
+ *     afqmc_shard_energy_finish.
+ * Two more barriers are needed only where a phase overwrites what a peer may still read: none in
+ * the sequences above as long as every member issues the same sequence.
+ * Restrictions: even M and even local n_chol; nw == max_walkers on every member (the group batch
+ * is contiguous); device pointers only.  afqmc_step / afqmc_local_energy / afqmc_run_block /
+ * afqmc_population_control return AFQMC_ERR_UNSUPPORTED on such a handle.
+ *
+ * Setup.  afqmc_create on a member computes everything that is local to its slice (m_g, Lrot,
+ * its share of h_mod - h1, of E_const and of the trial's two-body energy).
+ * afqmc_shard_setup_partial writes these M*M + 2 doubles to `out` (EITHER); the caller adds them
+ * over the group (all-reduce, or member order 0..G-1) and gives every member the same sums
+ * through afqmc_shard_setup_finish (`sum` EITHER, [M*M + 2]).  Phases fail with AFQMC_ERR_INVALID
+ * before that. */
+int32_t afqmc_shard_setup_partial(afqmc_handle* h, double* out);
+int32_t afqmc_shard_setup_finish(afqmc_handle* h, const double* sum);
+
+/* The four exchange buffers of this member, as device addresses: out[0] Theta^T gather buffer
+ * [G][nw][2][Nt][M], out[1] V_HS receive slots [G][nw][2][M][M], out[2] scalar slots
+ * [G][2][nw] complex (c_fb, c_mf), out[3] energy slots [G][nw] complex.  HOST pointer. */
+int32_t afqmc_shard_get_buffers(afqmc_handle* h, uint64_t* out4);
+/* CUDA IPC handle (64 bytes, HOST) of buffer `which` (0..3) for members in other processes, and
+ * the matching open / close in the importing process (cudaIpcOpenMemHandle / Close). */
+int32_t afqmc_shard_ipc_export(afqmc_handle* h, int32_t which, void* handle64);
+int32_t afqmc_shard_ipc_open(const void* handle64, uint64_t* addr_out);
+int32_t afqmc_shard_ipc_close(uint64_t addr);
+/* addrs HOST [G][4]: the buffers of every member as seen from THIS process (row group_rank
+ * must be this handle's own).  The pointers are borrowed until afqmc_destroy. */
+int32_t afqmc_shard_set_peers(afqmc_handle* h, const uint64_t* addrs);
+
+/* a1-a2 on this member's own walkers (DEVICE complex128 [nw][M][Nt]); Theta^T goes to slot
+ * group_rank of every member's gather buffer.  for_energy != 0 also keeps the one-body energy. */
+int32_t afqmc_shard_theta(afqmc_handle* h, const void* walkers, int32_t nw, int32_t for_energy);
+/* a3-a5 with this member's Cholesky vectors for all G * nw walkers of the group.
+ *   aux_local DEVICE double [G * nw][n_chol]: the fields x of every group walker (member-major
+ *   order) restricted to this member's gamma slice.
+ * Partial c_fb, c_mf and V_HS go to the owners' slots. */
+int32_t afqmc_shard_vhs(afqmc_handle* h, const double* aux_local, double dt, int32_t nw);
+/* Owner side: A, c_fb, c_mf = sums of the G slots, then a6-a10 on the own walkers (as afqmc_step).
+ *   walkers DEVICE in/out, weights DEVICE in/out. */
+int32_t afqmc_shard_propagate(afqmc_handle* h, void* walkers, double* weights, double dt, int32_t nw);
+/* a11 with this member's Cholesky vectors for all group walkers (after afqmc_shard_theta with
+ * for_energy = 1 on every member): partial E_C + E_X to the owners' slots. */
+int32_t afqmc_shard_energy(afqmc_handle* h, int32_t nw);
+/* Owner side: E_out DEVICE complex128 [nw][3] = (E, E_1body, E_2body). */
+int32_t afqmc_shard_energy_finish(afqmc_handle* h, void* E_out, int32_t nw);
 
 /* Measurement helper (not part of the method): register-only issue loops on all SMs for
  * `ms` milliseconds each.  out[0] = FP64 mma.sync m8n8k4 (DMMA) TFLOP/s, out[1] = FP64 FMA

@@ -19,10 +19,14 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_get_constants", "afqmc_debug_read", "afqmc_launch_count", "afqmc_sync",
            "afqmc_last_error", "afqmc_destroy", "afqmc_measure_fp64_peak", "afqmc_set_profiling",
            "afqmc_get_stage_times", "afqmc_population_control", "afqmc_estimators", "afqmc_run_block",
-           "afqmc_set_block_graph"]
+           "afqmc_set_block_graph", "afqmc_shard_setup_partial", "afqmc_shard_setup_finish",
+           "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
+           "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
+           "afqmc_shard_energy", "afqmc_shard_energy_finish"]
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
-          "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators"]
+          "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
+          "shard_exchange", "shard_reduce"]
 
 
 class AfqmcParams(C.Structure):
@@ -31,7 +35,7 @@ class AfqmcParams(C.Structure):
                 ("walker_kind", C.c_int32), ("taylor_order", C.c_int32),
                 ("ortho_every", C.c_int32), ("e_shift_auto", C.c_int32),
                 ("e_shift", C.c_double), ("stream", C.c_void_p), ("pack_chol", C.c_int32),
-                ("reserved", C.c_int32)]
+                ("group_size", C.c_int32), ("group_rank", C.c_int32), ("reserved", C.c_int32)]
 
 
 def _load():
@@ -72,6 +76,15 @@ def _load():
     lib.afqmc_run_block.restype = i32
     lib.afqmc_set_block_graph.argtypes = [vp, i32]
     lib.afqmc_set_block_graph.restype = i64
+    u64 = C.c_uint64
+    for name, args in [("afqmc_shard_setup_partial", [vp, vp]), ("afqmc_shard_setup_finish", [vp, vp]),
+                       ("afqmc_shard_get_buffers", [vp, vp]), ("afqmc_shard_ipc_export", [vp, i32, vp]),
+                       ("afqmc_shard_ipc_open", [vp, vp]), ("afqmc_shard_ipc_close", [u64]),
+                       ("afqmc_shard_set_peers", [vp, vp]), ("afqmc_shard_theta", [vp, vp, i32, i32]),
+                       ("afqmc_shard_vhs", [vp, vp, dbl, i32]), ("afqmc_shard_propagate", [vp, vp, vp, dbl, i32]),
+                       ("afqmc_shard_energy", [vp, i32]), ("afqmc_shard_energy_finish", [vp, vp, i32])]:
+        getattr(lib, name).argtypes = args
+        getattr(lib, name).restype = i32
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
     return lib
@@ -114,7 +127,8 @@ class AFQMC:
     """Handle wrapper with the same calls as the C ABI."""
 
     def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
-                 walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False):
+                 walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False,
+                 group_size=0, group_rank=0):
         p = AfqmcParams()
         p.struct_size = C.sizeof(AfqmcParams)
         p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
@@ -124,6 +138,7 @@ class AFQMC:
         p.e_shift = 0.0 if e_shift is None else float(e_shift)
         p.stream = stream
         p.pack_chol = 1 if pack_chol else 0
+        p.group_size, p.group_rank = int(group_size), int(group_rank)
         # L_chol is borrowed by the library (only during create when pack_chol is set)
         self._keep = (h1, None if pack_chol else L_chol, trial)
         self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers
@@ -187,6 +202,47 @@ class AFQMC:
         if r < 0:
             self._check(int(r))
         return out
+
+    # ---- distributed Hamiltonian (group_size > 1): the afqmc_shard_* phases, same names ----
+    def shard_setup_partial(self):
+        out = np.empty(self.M * self.M + 2)
+        self._check(lib.afqmc_shard_setup_partial(self._h, out.ctypes.data))
+        return out
+
+    def shard_setup_finish(self, total):
+        self._check(lib.afqmc_shard_setup_finish(self._h, _ptr(total)))
+
+    def shard_get_buffers(self):
+        out = np.zeros(4, dtype=np.uint64)
+        self._check(lib.afqmc_shard_get_buffers(self._h, out.ctypes.data))
+        return out
+
+    def shard_ipc_export(self, which):
+        buf = np.zeros(64, dtype=np.uint8)
+        self._check(lib.afqmc_shard_ipc_export(self._h, int(which), buf.ctypes.data))
+        return buf
+
+    def shard_set_peers(self, addrs):
+        a = np.ascontiguousarray(addrs, dtype=np.uint64)
+        self._check(lib.afqmc_shard_set_peers(self._h, a.ctypes.data))
+
+    def shard_theta(self, walkers, for_energy=False, nw=None):
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_shard_theta(self._h, _ptr(walkers), nw, 1 if for_energy else 0))
+
+    def shard_vhs(self, aux_local, dt, nw):
+        self._check(lib.afqmc_shard_vhs(self._h, _ptr(aux_local), float(dt), int(nw)))
+
+    def shard_propagate(self, walkers, weights, dt, nw=None):
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_shard_propagate(self._h, _ptr(walkers), _ptr(weights), float(dt), nw))
+
+    def shard_energy(self, nw):
+        self._check(lib.afqmc_shard_energy(self._h, int(nw)))
+
+    def shard_energy_finish(self, E_out, nw=None):
+        nw = int(E_out.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_shard_energy_finish(self._h, _ptr(E_out), nw))
 
     def set_profiling(self, on):
         self._check(lib.afqmc_set_profiling(self._h, 1 if on else 0))

@@ -48,6 +48,13 @@ struct afqmc_handle {
   std::vector<BlockGraph> graphs;
   bool graph_on = true;
   int64_t graph_replays = 0;
+  // distributed Hamiltonian (afqmc_shard_*): group of G members, this one holds a gamma slice
+  int G = 1, rank = 0, mwg = 0;                 // mwg = G * maxw: walkers of the whole group
+  bool shard_ready = true, peers_set = false;
+  double *theta_buf = nullptr, *a_slots = nullptr, *scal_slots = nullptr, *e_slots = nullptr;
+  double *hmod_part = nullptr, *setup_buf = nullptr, *e1zero = nullptr, *Etmp = nullptr, *scal_sum = nullptr;
+  double Ec_part = 0.0, e2trial_part = 0.0, e1b_trial = 0.0;
+  double* peer[4][kMaxGroup] = {};              // [theta, a, scal, e][member]
   int fb_split = 1;
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   bool ws_vhs = false;
@@ -177,20 +184,18 @@ void build_E1(afqmc_handle* h, double dt) {
   h->dt_cached = dt;
 }
 
-OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, int want_e1) {
+OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, int want_e1,
+               double* ThT = nullptr) {
   OTArgs a;
-  a.W = W; a.trial = h->trial; a.hrot = h->hrot; a.det = det; a.ThT = h->ThT; a.e1 = h->e1;
+  a.W = W; a.trial = h->trial; a.hrot = h->hrot; a.det = det; a.ThT = ThT ? ThT : h->ThT; a.e1 = h->e1;
   a.M = h->M; a.Nt = h->Nt; a.nblk = h->nblk;
   for (int b = 0; b < 2; ++b) { a.off[b] = h->off[b]; a.ns[b] = h->ns[b]; }
   a.want_theta = want_theta; a.want_e1 = want_e1;
   return a;
 }
 
-int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
-  {
-    StageTimer tm(h, AFQMC_STAGE_E_THETA);
-    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
-  }
+// exchange + Coulomb + final sums for the nw walkers whose Theta^T sits in h->ThT; e1 [nw][nblk]
+int energy_from_theta(afqmc_handle* h, const double* e1, double* E_out, int nw) {
   for (int b = 0; b < h->nblk; ++b) {
     StageTimer tm(h, AFQMC_STAGE_EXCHANGE);
     ExArgs e;
@@ -208,30 +213,31 @@ int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw)
   StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
   EnergyArgs r;
   r.expart = h->expart[0]; r.ngroups = h->exgroups[0];
-  r.X = h->Xe; r.e1 = h->e1; r.E_out = E_out;
+  r.X = h->Xe; r.e1 = e1; r.E_out = E_out;
   r.n_chol = h->n_chol; r.nw = nw; r.nblk = h->nblk; r.spin_factor = h->sf;
   h->launches += run_energy_reduce2(r, h->nblk > 1 ? h->expart[1] : nullptr, h->exgroups[1], h->st);
   return AFQMC_OK;
 }
 
-// One walker step on device buffers (rows a1-a10), stream ordered, no synchronisation.
-int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double dt, int nw) {
-  const int M = h->M, Nt = h->Nt, nc = h->n_chol;
-  const long MM = (long)M * M;
-  if (!(h->dt_cached == dt)) build_E1(h, dt);
-
-  // a1/a2: overlap, Theta
+int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
   {
-    StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
-    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+    StageTimer tm(h, AFQMC_STAGE_E_THETA);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
   }
+  return energy_from_theta(h, h->e1, E_out, nw);
+}
+
+// One walker step on device buffers (rows a1-a10), stream ordered, no synchronisation.
+// a3 + a4 for the nw walkers whose Theta^T sits in h->ThT (with this handle's Cholesky vectors)
+void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw) {
+  const int M = h->M, Nt = h->Nt, nc = h->n_chol;
   // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
   {
     StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
     GemmArgs g = gemm_args();
     g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
     g.C = h->Xp; g.ldc = nc; g.M = 2 * nw; g.N = nc; g.K = Nt * M;
-    g.splitK = h->fb_split; g.sCsplit = (long)2 * h->maxw * nc;
+    g.splitK = h->fb_split; g.sCsplit = (long)2 * h->mwg * nc;
     int r = -1;
     if (h->ws)
       r = run_gemm_ws_nk(h->ThT, (long)Nt * M, h->Lrot, (long)Nt * M, h->Xp, nc, g.sCsplit, 2 * nw, nc, Nt * M,
@@ -242,11 +248,26 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   {
     StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
     ShiftArgs s;
-    s.Xp = h->Xp; s.sXp = (long)2 * h->maxw * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
+    s.Xp = h->Xp; s.sXp = (long)2 * h->mwg * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
     s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
     s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
     h->launches += run_field_shift(s, nw, h->st);
   }
+}
+
+int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
+
+int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double dt, int nw) {
+  const int M = h->M, nc = h->n_chol;
+  const long MM = (long)M * M;
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
+
+  // a1/a2: overlap, Theta
+  {
+    StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
+    h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
+  }
+  force_bias_shift_device(h, x, dt, nw);
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
   if (h->ws_vhs) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
@@ -261,6 +282,14 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
     g.M = 2 * nw; g.N = (int)MM; g.K = nc;
     h->launches += run_gemm(GEMM_KN, g, h->st);
   }
+  return propagate_device(h, W, wt, h->cfb, h->cmf, dt, nw);
+}
+
+// a6-a10 with A = V_HS in h->A and the overlap determinants of the incoming walkers in h->det_old
+int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw) {
+  const int M = h->M, Nt = h->Nt;
+  const long MM = (long)M * M;
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
   // a6: T0 = Acc = E1 phi
   const long wstride = (long)M * 2 * Nt;
   {
@@ -312,7 +341,7 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   {
     StageTimer tm(h, AFQMC_STAGE_WEIGHT);
     WeightArgs a;
-    a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = h->cfb; a.cmf = h->cmf;
+    a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = cfb; a.cmf = cmf;
     a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
     a.expo = -dt * (h->E_const - h->e_shift);
     h->launches += run_weight_update(a, nw, h->st);
@@ -458,11 +487,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->n_alpha > kMaxOcc || p->n_beta > kMaxOcc) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "occupied block > 64 columns");
   if ((long)p->n_chol * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
   if (!is_device_ptr(L_chol)) return fail(nullptr, AFQMC_ERR_INVALID, "L_chol must be a device pointer");
+  const int G = p->group_size > 0 ? p->group_size : 1;
+  if (G > kMaxGroup) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "group_size > 8");
+  if (p->group_rank < 0 || p->group_rank >= G) return fail(nullptr, AFQMC_ERR_INVALID, "group_rank out of range");
+  if (G > 1 && (p->M % 2 != 0 || p->n_chol % 2 != 0))
+    return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "a distributed Hamiltonian needs even M and an even local n_chol (TMA strides)");
 
   afqmc_handle* h = new (std::nothrow) afqmc_handle();
   if (!h) return fail(nullptr, AFQMC_ERR_ALLOC, "host allocation failed");
   h->p = *p;
   h->M = p->M; h->n_chol = p->n_chol; h->maxw = p->max_walkers;
+  h->G = G; h->rank = p->group_rank; h->mwg = G * p->max_walkers;
+  h->shard_ready = G == 1;
   h->K = p->taylor_order ? p->taylor_order : 6;
   h->rhf = p->walker_kind == 0;
   h->sf = h->rhf ? 2.0 : 1.0;
@@ -473,7 +509,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->L = L_chol;
   // TMA needs 16-byte global strides: even M.  AFQMC_LEGACY_KERNELS=1 forces the cp.async
   // kernels (used by the tests to cover both paths on the same inputs).
-  h->ws = (p->M % 2 == 0) && getenv("AFQMC_LEGACY_KERNELS") == nullptr;
+  h->ws = (p->M % 2 == 0) && (G > 1 || getenv("AFQMC_LEGACY_KERNELS") == nullptr);
   if (p->stream) {
     h->st = (cudaStream_t)p->stream;
   } else {
@@ -483,7 +519,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     }
     h->own_stream = true;
   }
-  const int M = h->M, Nt = h->Nt, nc = h->n_chol, mw = h->maxw;
+  const int M = h->M, Nt = h->Nt, nc = h->n_chol, mw = h->maxw, mwg = h->mwg;
   const long MM = (long)M * M;
   auto bail = [&](int code, const std::string& msg) {
     std::string m2 = msg;
@@ -542,7 +578,17 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     g.A = h->L; g.lda = M; g.B = h->L; g.ldb = M; g.C = part; g.ldc = M;
     g.M = M; g.N = M; g.K = nc * M; g.splitK = split; g.sCsplit = MM;
     h->launches += run_gemm(GEMM_KMKN, g, h->st);
-    h->launches += run_hmod(h->h1, part, split, mL, h->hmod, M, h->st);
+    if (G > 1) {
+      // this member's share of h_mod - h1 = sum over ITS gamma of (-1/2 L_g L_g + m_g L_g); the
+      // group sum is added to h1 in afqmc_shard_setup_finish
+      h->hmod_part = dalloc(h, MM);
+      if (!h->hmod_part) return bail(AFQMC_ERR_ALLOC, "device allocation failed (setup)");
+      h->launches += run_fill(h->Xs, 0.0, MM, h->st);
+      h->launches += run_hmod(h->Xs, part, split, mL, h->hmod_part, M, h->st);
+      h->launches += run_scale_copy(h->hmod, h->h1, 1.0, MM, h->st);    // placeholder until the finish
+    } else {
+      h->launches += run_hmod(h->h1, part, split, mL, h->hmod, M, h->st);
+    }
     cudaStreamSynchronize(h->st);
     dfree_one(h, part);
   }
@@ -572,6 +618,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     double s = 0.0;
     for (int g = 0; g < nc; ++g) s += mh[g] * mh[g];
     h->E_const = -0.5 * s;
+    h->Ec_part = h->E_const;
     double n1 = 0.0;
     for (int c = 0; c < M; ++c) {
       double cs = 0.0;
@@ -585,28 +632,45 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
 
   // ---- workspaces ----------------------------------------------------------------------
   {
-    const int tiles = ((2 * mw + 127) / 128) * ((nc + 127) / 128);
+    const int tiles = ((2 * mwg + 127) / 128) * ((nc + 127) / 128);
     int split = (296 + tiles - 1) / tiles;
     const int kmax = std::max(1, (Nt * M) / 512);
     if (split > kmax) split = kmax;
     if (split > 16) split = 16;
     if (split < 1) split = 1;
-    h->fb_split = h->ws ? gemm_ws_nk_split(2 * mw, nc, Nt * M, 16) : split;
+    h->fb_split = h->ws ? gemm_ws_nk_split(2 * mwg, nc, Nt * M, 16) : split;
   }
   const size_t wsz = (size_t)mw * M * 2 * Nt;
   h->det_old = dalloc(h, (size_t)mw * 2 * 2); h->det_new = dalloc(h, (size_t)mw * 2 * 2);
-  h->ThT = dalloc(h, wsz); h->Xp = dalloc(h, (size_t)h->fb_split * 2 * mw * nc);
-  h->X = dalloc(h, (size_t)2 * mw * nc); h->Cf = dalloc(h, (size_t)2 * mw * nc);
-  h->cfb = dalloc(h, 2 * mw); h->cmf = dalloc(h, 2 * mw);
+  // Theta^T of every walker the force bias / exchange kernels see: the whole group's in a
+  // distributed Hamiltonian (member r's walkers in slot r, written by member r)
+  h->ThT = dalloc(h, (size_t)G * wsz); h->Xp = dalloc(h, (size_t)h->fb_split * 2 * mwg * nc);
+  h->X = dalloc(h, (size_t)2 * mwg * nc); h->Cf = dalloc(h, (size_t)2 * mwg * nc);
+  h->cfb = dalloc(h, 2 * mwg); h->cmf = dalloc(h, 2 * mwg);
   h->A = dalloc(h, (size_t)mw * 2 * MM);
   h->T0 = dalloc(h, wsz); h->T1 = dalloc(h, wsz); h->Acc = dalloc(h, wsz);
   h->ovlp = dalloc(h, 2 * mw); h->detR = dalloc(h, 2 * mw);
   for (int b = 0; b < h->nblk; ++b) {
     const int G = h->ws ? exchange_ws_group_size(h->ns[b]) : exchange_group_size(h->ns[b]);
     h->exgroups[b] = (nc + G - 1) / G;
-    h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mw * 2);
+    h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mwg * 2);
   }
-  h->Xe = dalloc(h, (size_t)nc * mw * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
+  h->Xe = dalloc(h, (size_t)nc * mwg * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
+  if (G > 1) {
+    h->theta_buf = h->ThT;
+    h->a_slots = dalloc(h, (size_t)G * mw * 2 * MM);
+    h->scal_slots = dalloc(h, (size_t)G * mw * 4);
+    h->e_slots = dalloc(h, (size_t)G * mw * 2);
+    h->scal_sum = dalloc(h, (size_t)mw * 4);
+    h->e1zero = dalloc(h, (size_t)mwg * 2 * 2);
+    h->Etmp = dalloc(h, (size_t)mwg * 6);
+    h->setup_buf = dalloc(h, (size_t)MM + 2);
+    if (!h->a_slots || !h->scal_slots || !h->e_slots || !h->scal_sum || !h->e1zero || !h->Etmp || !h->setup_buf)
+      return bail(AFQMC_ERR_ALLOC, "device allocation failed (distributed-Hamiltonian slots)");
+    cudaMemsetAsync(h->e1zero, 0, (size_t)mwg * 2 * 2 * 8, h->st);
+    h->peer[0][h->rank] = h->theta_buf; h->peer[1][h->rank] = h->a_slots;
+    h->peer[2][h->rank] = h->scal_slots; h->peer[3][h->rank] = h->e_slots;
+  }
   h->stW = dalloc(h, wsz); h->stWt = dalloc(h, mw); h->stX = dalloc(h, (size_t)mw * nc); h->stE = dalloc(h, (size_t)mw * 6);
   h->cum = dalloc(h, mw); h->xi_dev = dalloc(h, 4); h->est_dev = dalloc(h, 4); h->ovlp_tmp = dalloc(h, 2 * mw);
   h->pmap = (int*)dalloc(h, (mw + 1) / 2 + 1);
@@ -645,7 +709,10 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
       return bail(AFQMC_ERR_CUDA, std::string("trial energy failed: ") + cudaGetErrorString(cudaPeekAtLastError()));
     h->e_trial = e[0];
+    h->e1b_trial = e[2];
+    h->e2trial_part = e[4];
   }
+  if (G > 1 && !h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "a distributed Hamiltonian needs the TMA V_HS kernel (16-byte aligned L)");
   h->e_shift = p->e_shift_auto ? h->e_trial : p->e_shift;
   if (h->Lpk) {                      // the dense tensor is not touched after this point
     if (cudaStreamSynchronize(h->st) != cudaSuccess) return bail(AFQMC_ERR_CUDA, "pack_chol failed");
@@ -657,6 +724,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
 
 int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {
   if (!h) return AFQMC_ERR_INVALID;
+  if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
@@ -682,6 +750,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
 
 int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, int32_t nw) {
   if (!h) return AFQMC_ERR_INVALID;
+  if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !E_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
@@ -704,6 +773,7 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
 int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi, int32_t nw,
                                  int32_t* map_out) {
   if (!h) return AFQMC_ERR_INVALID;
+  if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !xi) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
@@ -748,6 +818,7 @@ int32_t afqmc_estimators(afqmc_handle* h, const double* weights, const void* E, 
 int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, const double* xi,
                         double dt, int32_t nw, int32_t n_steps, int32_t pop_every, void* E_out, double* est_out) {
   if (!h) return AFQMC_ERR_INVALID;
+  if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   if (n_steps <= 0 || pop_every < 0) return fail(h, AFQMC_ERR_INVALID, "bad n_steps / pop_every");
@@ -878,6 +949,197 @@ int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_ou
 }
 
 int64_t afqmc_launch_count(const afqmc_handle* h) { return h ? h->launches : -1; }
+
+// ------------------------------------------------------------------ distributed Hamiltonian
+#define SHARD_CHECK(h, need_ready)                                                                     \
+  if (!h) return AFQMC_ERR_INVALID;                                                                    \
+  if (h->G <= 1) return fail(h, AFQMC_ERR_INVALID, "not a distributed-Hamiltonian handle (group_size <= 1)"); \
+  if (need_ready && !h->shard_ready) return fail(h, AFQMC_ERR_INVALID, "afqmc_shard_setup_finish has not been called"); \
+  if (need_ready && !h->peers_set) return fail(h, AFQMC_ERR_INVALID, "afqmc_shard_set_peers has not been called");
+
+int32_t afqmc_shard_setup_partial(afqmc_handle* h, double* out) {
+  SHARD_CHECK(h, false);
+  if (!out) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  const long MM = (long)h->M * h->M;
+  const double sc[2] = {h->Ec_part, h->e2trial_part};
+  cudaMemcpyAsync(h->setup_buf, h->hmod_part, MM * 8, cudaMemcpyDeviceToDevice, h->st);
+  cudaMemcpyAsync(h->setup_buf + MM, sc, 16, cudaMemcpyHostToDevice, h->st);
+  cudaMemcpyAsync(out, h->setup_buf, (MM + 2) * 8, cudaMemcpyDefault, h->st);
+  if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_shard_setup_partial");
+  return check_cuda(h, "afqmc_shard_setup_partial");
+}
+
+int32_t afqmc_shard_setup_finish(afqmc_handle* h, const double* sum) {
+  SHARD_CHECK(h, false);
+  if (!sum) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  const int M = h->M;
+  const long MM = (long)M * M;
+  std::vector<double> s((size_t)MM + 2), hh((size_t)MM);
+  if (cudaMemcpyAsync(s.data(), sum, (MM + 2) * 8, cudaMemcpyDefault, h->st) != cudaSuccess ||
+      cudaMemcpyAsync(hh.data(), h->h1, MM * 8, cudaMemcpyDeviceToHost, h->st) != cudaSuccess ||
+      cudaStreamSynchronize(h->st) != cudaSuccess)
+    return check_cuda(h, "afqmc_shard_setup_finish");
+  double n1 = 0.0;
+  for (long i = 0; i < MM; ++i) hh[i] += s[i];
+  for (int c = 0; c < M; ++c) {
+    double cs = 0.0;
+    for (int r = 0; r < M; ++r) cs += fabs(hh[(size_t)r * M + c]);
+    if (cs > n1) n1 = cs;
+  }
+  cudaMemcpyAsync(h->hmod, hh.data(), MM * 8, cudaMemcpyHostToDevice, h->st);
+  if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_shard_setup_finish");
+  h->hmod_norm1 = n1;
+  h->E_const = s[MM];
+  h->e_trial = h->e1b_trial + s[MM + 1];
+  h->e_shift = h->p.e_shift_auto ? h->e_trial : h->p.e_shift;
+  h->dt_cached = NAN;
+  h->shard_ready = true;
+  return check_cuda(h, "afqmc_shard_setup_finish");
+}
+
+int32_t afqmc_shard_get_buffers(afqmc_handle* h, uint64_t* out4) {
+  SHARD_CHECK(h, false);
+  if (!out4) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  for (int k = 0; k < 4; ++k) out4[k] = (uint64_t)(uintptr_t)h->peer[k][h->rank];
+  return AFQMC_OK;
+}
+
+int32_t afqmc_shard_ipc_export(afqmc_handle* h, int32_t which, void* handle64) {
+  SHARD_CHECK(h, false);
+  if (!handle64 || which < 0 || which > 3) return fail(h, AFQMC_ERR_INVALID, "bad argument");
+  static_assert(sizeof(cudaIpcMemHandle_t) == 64, "IPC handle size");
+  cudaIpcMemHandle_t mh;
+  if (cudaIpcGetMemHandle(&mh, h->peer[which][h->rank]) != cudaSuccess) return check_cuda(h, "cudaIpcGetMemHandle");
+  memcpy(handle64, &mh, 64);
+  return AFQMC_OK;
+}
+
+int32_t afqmc_shard_ipc_open(const void* handle64, uint64_t* addr_out) {
+  if (!handle64 || !addr_out) return AFQMC_ERR_INVALID;
+  cudaIpcMemHandle_t mh;
+  memcpy(&mh, handle64, 64);
+  void* p = nullptr;
+  const cudaError_t e = cudaIpcOpenMemHandle(&p, mh, cudaIpcMemLazyEnablePeerAccess);
+  if (e != cudaSuccess) {
+    g_create_err = std::string("cudaIpcOpenMemHandle: ") + cudaGetErrorString(e);
+    cudaGetLastError();
+    return AFQMC_ERR_CUDA;
+  }
+  *addr_out = (uint64_t)(uintptr_t)p;
+  return AFQMC_OK;
+}
+
+int32_t afqmc_shard_ipc_close(uint64_t addr) {
+  if (!addr) return AFQMC_ERR_INVALID;
+  if (cudaIpcCloseMemHandle((void*)(uintptr_t)addr) != cudaSuccess) {
+    cudaGetLastError();
+    return AFQMC_ERR_CUDA;
+  }
+  return AFQMC_OK;
+}
+
+int32_t afqmc_shard_set_peers(afqmc_handle* h, const uint64_t* addrs) {
+  SHARD_CHECK(h, false);
+  if (!addrs) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  for (int k = 0; k < 4; ++k)
+    if (addrs[(size_t)h->rank * 4 + k] != (uint64_t)(uintptr_t)h->peer[k][h->rank])
+      return fail(h, AFQMC_ERR_INVALID, "row group_rank of addrs must hold this handle's own buffers");
+  for (int r = 0; r < h->G; ++r)
+    for (int k = 0; k < 4; ++k) {
+      if (!addrs[(size_t)r * 4 + k] || (addrs[(size_t)r * 4 + k] & 15)) return fail(h, AFQMC_ERR_INVALID, "null or misaligned peer buffer");
+      h->peer[k][r] = (double*)(uintptr_t)addrs[(size_t)r * 4 + k];
+    }
+  h->peers_set = true;
+  return AFQMC_OK;
+}
+
+int32_t afqmc_shard_theta(afqmc_handle* h, const void* walkers, int32_t nw, int32_t for_energy) {
+  SHARD_CHECK(h, true);
+  if (!walkers || !is_device_ptr(walkers)) return fail(h, AFQMC_ERR_INVALID, "walkers must be a device pointer");
+  if (nw != h->maxw) return fail(h, AFQMC_ERR_DIMS, "a distributed Hamiltonian needs nw == max_walkers");
+  const size_t wsz = (size_t)h->maxw * h->M * 2 * h->Nt;
+  double* own = h->theta_buf + (size_t)h->rank * wsz;
+  {
+    StageTimer tm(h, for_energy ? AFQMC_STAGE_E_THETA : AFQMC_STAGE_OVERLAP_THETA);
+    h->launches += run_overlap_theta(ot_args(h, (const double*)walkers, h->det_old, 1, for_energy ? 1 : 0, own), nw, h->st);
+  }
+  StageTimer tm(h, AFQMC_STAGE_SHARD_EXCHANGE);
+  for (int r = 0; r < h->G; ++r)
+    if (r != h->rank)
+      cudaMemcpyAsync(h->peer[0][r] + (size_t)h->rank * wsz, own, wsz * 8, cudaMemcpyDefault, h->st);
+  return check_cuda(h, "afqmc_shard_theta");
+}
+
+int32_t afqmc_shard_vhs(afqmc_handle* h, const double* aux_local, double dt, int32_t nw) {
+  SHARD_CHECK(h, true);
+  if (!aux_local || !is_device_ptr(aux_local)) return fail(h, AFQMC_ERR_INVALID, "aux_local must be a device pointer");
+  if (nw != h->maxw) return fail(h, AFQMC_ERR_DIMS, "a distributed Hamiltonian needs nw == max_walkers");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
+  const int G = h->G, mw = h->maxw, nwg = G * nw;
+  const long MM = (long)h->M * h->M;
+  force_bias_shift_device(h, aux_local, dt, nwg);
+  {
+    StageTimer tm(h, AFQMC_STAGE_SHARD_EXCHANGE);
+    for (int o = 0; o < G; ++o) {
+      double* dst = h->peer[2][o] + (size_t)h->rank * mw * 4;
+      cudaMemcpyAsync(dst, h->cfb + (size_t)o * nw * 2, (size_t)nw * 16, cudaMemcpyDefault, h->st);
+      cudaMemcpyAsync(dst + (size_t)mw * 2, h->cmf + (size_t)o * nw * 2, (size_t)nw * 16, cudaMemcpyDefault, h->st);
+    }
+  }
+  StageTimer tm(h, AFQMC_STAGE_VHS);
+  double* Cb[kMaxGroup];
+  for (int o = 0; o < G; ++o) Cb[o] = h->peer[1][o] + (size_t)h->rank * mw * 2 * MM;
+  const int r = run_vhs_ws_scatter(h->Cf, h->Lpk ? h->Lpk : h->L, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile, h->M,
+                                   h->n_chol, h->Lpk != nullptr, h->st);
+  if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
+  h->launches += r;
+  return check_cuda(h, "afqmc_shard_vhs");
+}
+
+int32_t afqmc_shard_propagate(afqmc_handle* h, void* walkers, double* weights, double dt, int32_t nw) {
+  SHARD_CHECK(h, true);
+  if (!walkers || !weights || !is_device_ptr(walkers) || !is_device_ptr(weights))
+    return fail(h, AFQMC_ERR_INVALID, "walkers and weights must be device pointers");
+  if (nw != h->maxw) return fail(h, AFQMC_ERR_DIMS, "a distributed Hamiltonian needs nw == max_walkers");
+  if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
+  const int G = h->G, mw = h->maxw;
+  const long MM = (long)h->M * h->M;
+  {
+    StageTimer tm(h, AFQMC_STAGE_SHARD_REDUCE);
+    const double *sa[kMaxGroup], *ss[kMaxGroup];
+    for (int r = 0; r < G; ++r) {
+      sa[r] = h->a_slots + (size_t)r * mw * 2 * MM;
+      ss[r] = h->scal_slots + (size_t)r * mw * 4;
+    }
+    h->launches += run_sum_slots(h->A, sa, G, (long)nw * 2 * MM, h->st);
+    h->launches += run_sum_slots(h->scal_sum, ss, G, (long)mw * 4, h->st);
+  }
+  const int rc = propagate_device(h, (double*)walkers, weights, h->scal_sum, h->scal_sum + (size_t)mw * 2, dt, nw);
+  return rc != AFQMC_OK ? rc : check_cuda(h, "afqmc_shard_propagate");
+}
+
+int32_t afqmc_shard_energy(afqmc_handle* h, int32_t nw) {
+  SHARD_CHECK(h, true);
+  if (nw != h->maxw) return fail(h, AFQMC_ERR_DIMS, "a distributed Hamiltonian needs nw == max_walkers");
+  const int G = h->G, mw = h->maxw;
+  const int rc = energy_from_theta(h, h->e1zero, h->Etmp, G * nw);
+  if (rc != AFQMC_OK) return rc;
+  StageTimer tm(h, AFQMC_STAGE_SHARD_EXCHANGE);
+  for (int o = 0; o < G; ++o)
+    h->launches += run_push_e2(h->peer[3][o] + (size_t)h->rank * mw * 2, h->Etmp + (size_t)o * nw * 6, nw, h->st);
+  return check_cuda(h, "afqmc_shard_energy");
+}
+
+int32_t afqmc_shard_energy_finish(afqmc_handle* h, void* E_out, int32_t nw) {
+  SHARD_CHECK(h, true);
+  if (!E_out || !is_device_ptr(E_out)) return fail(h, AFQMC_ERR_INVALID, "E_out must be a device pointer");
+  if (nw != h->maxw) return fail(h, AFQMC_ERR_DIMS, "a distributed Hamiltonian needs nw == max_walkers");
+  StageTimer tm(h, AFQMC_STAGE_SHARD_REDUCE);
+  const double* se[kMaxGroup];
+  for (int r = 0; r < h->G; ++r) se[r] = h->e_slots + (size_t)r * h->maxw * 2;
+  h->launches += run_energy_finish((double*)E_out, h->e1, se, h->G, h->nblk, h->sf, nw, h->st);
+  return check_cuda(h, "afqmc_shard_energy_finish");
+}
 
 int32_t afqmc_sync(afqmc_handle* h) {
   if (!h) return AFQMC_ERR_INVALID;

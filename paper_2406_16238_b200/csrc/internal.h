@@ -13,6 +13,7 @@ namespace afq {
 
 constexpr int kMaxOcc = 64;     // largest occupied block (columns per spin) supported
 constexpr int kMaxTaylor = 16;
+constexpr int kMaxGroup = 8;    // members of a distributed-Hamiltonian group
 
 enum GemmKind { GEMM_KN = 0, GEMM_NK = 1, GEMM_KMKN = 2, GEMM_CPLX_KN = 3 };
 
@@ -105,6 +106,11 @@ bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void*
 int vhs_ws_tile_list(int M, std::vector<int>* out);
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
                int n_chol, int rows, bool packed, cudaStream_t st);
+// the same contraction with the output rows scattered by blocks of rows_per_member rows: row r goes
+// to Cb[r / rows_per_member] + (r % rows_per_member) * M * M (distributed Hamiltonian: the partial
+// V_HS of a walker is stored straight into its owner's receive slot, possibly peer memory)
+int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int nmember, int rows_per_member,
+                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st);
 // tile-packed upper triangle of L (the paper's pack_chol): [ntile_n][n_chol][4][32]
 size_t vhs_ws_packed_doubles(int ntile_n, int n_chol);
 int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
@@ -122,6 +128,12 @@ int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double*
 int run_comb(double* weights, const double* xi, double* cum, int* map, int nw, cudaStream_t st);
 int run_permute_rows(void* rows, void* tmp, const int* map, long row_bytes, int nw, cudaStream_t st);
 int run_estimators(const double* weights, const double* E, double* out4, int nw, cudaStream_t st);
+
+// shard.cu: fixed-order reductions of the per-member receive slots (distributed Hamiltonian)
+int run_sum_slots(double* dst, const double* const* slots, int G, long n, cudaStream_t st);
+int run_push_e2(double* dst, const double* E, int n, cudaStream_t st);
+int run_energy_finish(double* E_out, const double* e1, const double* const* slots, int G, int nblk, double sf,
+                      int nw, cudaStream_t st);
 
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);

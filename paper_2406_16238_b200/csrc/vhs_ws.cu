@@ -29,7 +29,8 @@ constexpr int STAGESv = 6;
 constexpr size_t SMEMv = (size_t)STAGESv * STAGE_BYTESv + 1024 + 256;
 
 struct VhsArgs {
-  double* C;            // [rows][M][M]
+  double* Cb[kMaxGroup];  // output base per block of rpm rows: row r -> Cb[r / rpm] + (r % rpm) M M
+  int rpm;
   const int* tiles;     // [ntile_n] packed (pb << 16 | qb)
   int M, n_chol, rows;  // rows = 2 nw
   int ntile_n, mtiles;
@@ -154,7 +155,7 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
     for (int i = 0; i < MI; ++i) {
       const int r = mt * BMv + 8 * (wm * MI + i) + p;
       if (r >= a.rows) continue;
-      double* Cr = a.C + (size_t)r * MM;
+      double* Cr = a.Cb[r / a.rpm] + (size_t)(r % a.rpm) * MM;
       if (fast) {
 #pragma unroll
         for (int j = 0; j < NI; ++j)
@@ -224,6 +225,14 @@ bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void*
 // algorithmic flops actually needed with the symmetric half: 2 * rows * n_chol * M (M + 1) / 2 * 2
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
                int n_chol, int rows, bool packed, cudaStream_t st) {
+  double* Cb[1] = {C};
+  return run_vhs_ws_scatter(Cf, L, Cb, 1, rows, tiles_dev, ntile_n, M, n_chol, packed, st);
+}
+
+int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int nmember, int rows_per_member,
+                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st) {
+  if (nmember < 1 || nmember > kMaxGroup || rows_per_member < 1) return -1;
+  const int rows = nmember * rows_per_member;
   static bool attr = false;
   if (!attr) {
     cudaFuncSetAttribute(vhs_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
@@ -256,7 +265,9 @@ int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_de
     if (make_tensor_map_f64(&tmB, L, 3, dims, str, box) != 0) return -1;
   }
   VhsArgs a;
-  a.C = C; a.tiles = tiles_dev; a.M = M; a.n_chol = n_chol; a.rows = rows;
+  for (int r = 0; r < kMaxGroup; ++r) a.Cb[r] = r < nmember ? Cb[r] : nullptr;
+  a.rpm = rows_per_member;
+  a.tiles = tiles_dev; a.M = M; a.n_chol = n_chol; a.rows = rows;
   a.ntile_n = ntile_n; a.mtiles = (rows + BMv - 1) / BMv;
   const long nt = (long)a.ntile_n * a.mtiles;
   const int grid = nt < nsm ? (int)nt : nsm;
