@@ -35,8 +35,8 @@ UNIT = "walker-steps/s"
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
 # `ncu --set full` captures summarised under profiles/ (file named beside each number).
 NCU_TRAFFIC = {
-    ("c5", "exchange"): 3.140e9,   # profiles/r1v2_full_c5.md (exchange_ws_kernel<4,3,4,7>, 3.127 GB rd + 0.013 GB wr)
-    ("c5", "vhs"): 31.72e9,        # profiles/r1v2_full_c5.md (vhs_ws_kernel, 30.26 GB rd + 1.46 GB wr; upper tiles of L)
+    ("c5", "exchange"): 3.234e9,   # profiles/r1v4_full_c5.md (exchange_ws_kernel<4,3,4,7>, 3.220 GB rd + 0.014 GB wr)
+    ("c5", "vhs"): 30.48e9,        # profiles/r1v4_full_c5.md (vhs_ws_kernel<0>, 29.02 GB rd + 1.46 GB wr; upper tiles of L)
 }
 
 
@@ -191,6 +191,51 @@ def time_blocks(g, cfg, stream, walkers_h, seed, nw, reps, n_steps=25, pop_every
             "graph_equals_eager": bool(np.array_equal(est_eager, est_graph))}
 
 
+def time_sharded(cfg, h1, Ld, trial, G, K, Wm, seed):
+    """Secondary figure (--group G): the distributed-Hamiltonian route with all G
+    members on THIS one GPU, each holding a gamma slice of the same tensor (views, no copy) and
+    Nw / G walkers, so the group does the same work as the plain step.  A phase is issued member
+    after member on the members' own streams (their persistent kernels share the SMs; no kernel
+    waits on another), barriers are stream synchronisations; the figure is the cost of the slot
+    traffic and the owner-side sums, not of NVLink."""
+    import torch
+    from paper_2406_16238_b200 import inputs, sharded
+    nw = cfg.nw // G
+    slices = sharded.gamma_slices(cfg.n_chol, G)
+    grp = sharded.LocalGroup(h1, [Ld[a:b] for a, b in slices], trial, M=cfg.M, n_alpha=cfg.n_alpha,
+                             n_beta=cfg.n_beta, max_walkers=nw, walker_kind=cfg.walker_kind,
+                             taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every)
+    walkers = inputs.make_walkers(cfg, trial, seed, G * nw)
+    W = [torch.from_numpy(np.ascontiguousarray(walkers[r * nw:(r + 1) * nw])).cuda() for r in range(G)]
+    wt = [torch.ones(nw, dtype=torch.float64, device="cuda") for _ in range(G)]
+    E = [torch.empty((nw, 3), dtype=torch.complex128, device="cuda") for _ in range(G)]
+    xs = []
+    for s in range(Wm + K):
+        x = inputs.make_aux_fields(cfg, seed, s, G * nw)
+        xs.append([torch.from_numpy(np.ascontiguousarray(x[r * nw:(r + 1) * nw])).cuda() for r in range(G)])
+
+    def one(s):
+        grp.step(W, wt, xs[s], cfg.dt)
+        grp.local_energy(W, E)
+
+    for s in range(Wm):
+        one(s)
+    l0 = sum(m.launch_count() for m in grp.members)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    for s in range(Wm, Wm + K):
+        one(s)
+    torch.cuda.synchronize()
+    t = time.perf_counter() - t0
+    launches = sum(m.launch_count() for m in grp.members) - l0
+    Em = float(np.mean(np.concatenate([e.cpu().numpy()[:, 0].real for e in E])))
+    grp.close()
+    return {"members_on_this_gpu": G, "walkers_per_member": nw, "gamma_per_member": [b - a for a, b in slices],
+            "ms_per_group_step": t / K * 1e3, "walker_steps_per_s": G * nw * K / t, "timing": "host clock around "
+            "K x (group step + group local energy), stream synchronisations as group barriers",
+            "launches": int(launches), "E_mean_real": Em}
+
+
 def replica_seed(rank):
     """Every replica draws its own walkers and fields; the Hamiltonian (seed 0) is the same."""
     return int(rank)
@@ -252,6 +297,8 @@ def main():
                          "freed after afqmc_create")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
+    ap.add_argument("--group", type=int, default=0,
+                    help="also time the distributed-Hamiltonian route with this many members on the one GPU")
     ap.add_argument("--profiler-range", action="store_true",
                     help="cudaProfilerStart/Stop around the timed steps (ncu --profile-from-start off)")
     args = ap.parse_args()
@@ -414,6 +461,11 @@ def main():
         "check": {"E_mean_real": float(np.mean(E_last[:, 0].real)), "weights_min": float(wt_last.min()),
                   "weights_max": float(wt_last.max())},
     }
+
+    if args.group > 1 and world == 1:
+        if Ld is None:
+            Ld, _ = make_L(cfg, 0, False, True)
+        line["distributed_hamiltonian"] = time_sharded(cfg, h1, Ld, trial, args.group, K, Wm, seed)
 
     if want_cpu:
         g.close()
