@@ -295,6 +295,9 @@ def main():
     ap.add_argument("--pack-chol", action="store_true",
                     help="handle keeps the tile-packed upper triangles of L (PAPER.md:205); the dense tensor is "
                          "freed after afqmc_create")
+    ap.add_argument("--mixed-precision", action="store_true",
+                    help="V_HS build in emulated single precision on tcgen05 (afqmc_params.mixed_precision); "
+                         "not the headline configuration (north_star: complex128 throughout)")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
     ap.add_argument("--group", type=int, default=0,
@@ -336,8 +339,9 @@ def main():
     g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta,
                     n_chol=cfg.n_chol, max_walkers=nw, walker_kind=cfg.walker_kind,
                     taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every,
-                    stream=stream.cuda_stream, pack_chol=args.pack_chol)
-    if args.pack_chol:
+                    stream=stream.cuda_stream, pack_chol=args.pack_chol,
+                    mixed_precision=args.mixed_precision)
+    if args.pack_chol or args.mixed_precision:
         Ld = None
         torch.cuda.empty_cache()
     hbm_resident_gb = (torch.cuda.mem_get_info()[1] - torch.cuda.mem_get_info()[0]) / 1e9
@@ -433,6 +437,17 @@ def main():
             tf = f / (per_stage[k]["ms_per_step"] * 1e-3) / 1e12
             per_stage[k]["tflops"] = tf
             per_stage[k]["frac_of_dmma_peak"] = tf / peak_dmma
+    if args.mixed_precision and "vhs" in per_stage:
+        # bf16 x 3 on tcgen05: HBM bound (the split upper-triangle tiles are streamed once per step)
+        ntile = sum(1 for pb in range((cfg.M + 3) // 4) for qb in range((cfg.M + 31) // 32) if qb * 32 + 31 >= pb * 4)
+        gp = (cfg.n_chol + 63) // 64 * 64
+        by = ntile * 3 * 128 * gp * 2 + nw * 2 * cfg.M * cfg.M * 8
+        v = per_stage["vhs"]
+        v.pop("frac_of_dmma_peak", None)
+        v["tflops"] = 6 * fl["vhs"] / (v["ms_per_step"] * 1e-3) / 1e12      # bf16 flops issued: 6 plane pairs
+        v["algorithmic_bytes"] = by
+        v["gbytes_per_s"] = by / (v["ms_per_step"] * 1e-3) / 1e9
+        v["note"] = "emulated single precision (bf16 x 3, FP32 accumulate in TMEM); bound: hbm"
     dom = max(per_stage, key=lambda k: per_stage[k]["ms_per_step"])
     nl = {"exchange": 1 if cfg.walker_kind == 0 else 2, "taylor": cfg.taylor_order, "one_body": 2}.get(dom, 1)
     roof = {"kernel": dom, "bound": "tensor", "unit": "TFLOP/s", "peak": peak_dmma,
@@ -453,7 +468,7 @@ def main():
                    "n_chol": cfg.n_chol, "n_walkers_per_gpu": nw, "dt": cfg.dt,
                    "taylor_order": cfg.taylor_order, "ortho_every": cfg.ortho_every,
                    "local_energy": "every step", "parallelism": f"replicas x{world}",
-                   "pack_chol": bool(args.pack_chol), "hbm_resident_gb": round(hbm_resident_gb, 1),
+                   "pack_chol": bool(args.pack_chol), "mixed_precision": bool(args.mixed_precision), "hbm_resident_gb": round(hbm_resident_gb, 1),
                    "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "stages": per_stage, "block": block,

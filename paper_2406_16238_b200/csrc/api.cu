@@ -60,6 +60,7 @@ struct afqmc_handle {
   bool ws_vhs = false;
   int* vhs_tiles = nullptr;
   double* Lpk = nullptr;   // tile-packed upper triangle of L (pack_chol)
+  void *Lb = nullptr, *Ab = nullptr;   // mixed precision: bf16 x 3 split tiles of L, split coefficients
   int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
@@ -269,7 +270,13 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   }
   force_bias_shift_device(h, x, dt, nw);
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
-  if (h->ws_vhs) {
+  if (h->Lb) {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
+    double* Cb[1] = {h->A};
+    const int r = run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, 1, 2 * nw, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
+    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs (mixed precision): tensor map encode failed");
+    h->launches += r;
+  } else if (h->ws_vhs) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
     const int r = run_vhs_ws(h->Cf, h->Lpk ? h->Lpk : h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw,
                              h->Lpk != nullptr, h->st);
@@ -478,7 +485,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (!h1 || !L_chol || !trial || !p || !out) return fail(nullptr, AFQMC_ERR_INVALID, "null argument");
   if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
   if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
-      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
+      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
     return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
   if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
   if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
@@ -698,6 +705,15 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->launches += run_pack_tiles(h->L, h->Lpk, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
   }
 
+  if (p->mixed_precision) {
+    if (!h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "mixed_precision needs even M and n_chol");
+    if (p->pack_chol) return bail(AFQMC_ERR_INVALID, "mixed_precision keeps its own split tiles: pack_chol must be 0");
+    h->Lb = dalloc(h, (vhs_tc_L_elems(h->vhs_ntile, nc) * 2 + 7) / 8);
+    h->Ab = dalloc(h, (vhs_tc_cf_elems(2 * mwg, nc) * 2 + 7) / 8);
+    if (!h->Lb || !h->Ab) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Cholesky tensor)");
+    h->launches += run_vhs_tc_split_L(h->L, h->Lb, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
+  }
+
   // ---- E_shift = trial energy ---------------------------------------------------------------
   {
     std::vector<double> wt((size_t)M * Nt * 2, 0.0);
@@ -714,8 +730,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   }
   if (G > 1 && !h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "a distributed Hamiltonian needs the TMA V_HS kernel (16-byte aligned L)");
   h->e_shift = p->e_shift_auto ? h->e_trial : p->e_shift;
-  if (h->Lpk) {                      // the dense tensor is not touched after this point
-    if (cudaStreamSynchronize(h->st) != cudaSuccess) return bail(AFQMC_ERR_CUDA, "pack_chol failed");
+  if (h->Lpk || h->Lb) {             // the dense tensor is not touched after this point
+    if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "packing / splitting the Cholesky tensor failed");
     h->L = nullptr;
   }
   *out = h;
@@ -1089,8 +1106,9 @@ int32_t afqmc_shard_vhs(afqmc_handle* h, const double* aux_local, double dt, int
   StageTimer tm(h, AFQMC_STAGE_VHS);
   double* Cb[kMaxGroup];
   for (int o = 0; o < G; ++o) Cb[o] = h->peer[1][o] + (size_t)h->rank * mw * 2 * MM;
-  const int r = run_vhs_ws_scatter(h->Cf, h->Lpk ? h->Lpk : h->L, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile, h->M,
-                                   h->n_chol, h->Lpk != nullptr, h->st);
+  const int r = h->Lb ? run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile, h->M, h->n_chol, h->st)
+                      : run_vhs_ws_scatter(h->Cf, h->Lpk ? h->Lpk : h->L, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile,
+                                           h->M, h->n_chol, h->Lpk != nullptr, h->st);
   if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");
   h->launches += r;
   return check_cuda(h, "afqmc_shard_vhs");

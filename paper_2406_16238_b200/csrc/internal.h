@@ -116,6 +116,15 @@ size_t vhs_ws_packed_doubles(int ntile_n, int n_chol);
 int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
                    cudaStream_t st);
 
+// vhs_tc.cu: V_HS build in emulated single precision (bf16 x 3 on tcgen05, FP32 accumulation in TMEM)
+int vhs_tc_gamma_padded(int n_chol);
+size_t vhs_tc_L_elems(int ntile_n, int n_chol);      // bf16 elements of the split tile tensor
+size_t vhs_tc_cf_elems(int rows, int n_chol);        // bf16 elements of the split coefficient scratch
+int run_vhs_tc_split_L(const double* L, void* Lb, const int* tiles_dev, int ntile_n, int M, int n_chol,
+                       cudaStream_t st);
+int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, int nmember, int rows_per_member,
+               const int* tiles_dev, int ntile_n, int M, int n_chol, cudaStream_t st);
+
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
                    double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,

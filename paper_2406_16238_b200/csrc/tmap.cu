@@ -29,8 +29,8 @@ EncodeTiledFn encode_fn() {
 }
 }  // namespace
 
-int make_tensor_map_f64(TensorMap* out, const void* base, int rank, const uint64_t* dims,
-                        const uint64_t* strides_bytes, const uint32_t* box) {
+static int make_tensor_map(TensorMap* out, CUtensorMapDataType dt, const void* base, int rank,
+                           const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box) {
   static_assert(sizeof(TensorMap) == sizeof(CUtensorMap), "CUtensorMap is 128 bytes");
   EncodeTiledFn fn = encode_fn();
   if (!fn) return -1;
@@ -39,11 +39,21 @@ int make_tensor_map_f64(TensorMap* out, const void* base, int rank, const uint64
   cuuint32_t bx[5], es[5];
   for (int i = 0; i < rank; ++i) { gd[i] = dims[i]; bx[i] = box[i]; es[i] = 1; }
   for (int i = 0; i < rank - 1; ++i) gs[i] = strides_bytes[i];
-  CUresult r = fn(reinterpret_cast<CUtensorMap*>(out), CU_TENSOR_MAP_DATA_TYPE_FLOAT64, (cuuint32_t)rank,
+  CUresult r = fn(reinterpret_cast<CUtensorMap*>(out), dt, (cuuint32_t)rank,
                   const_cast<void*>(base), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
                   CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return (int)r;
+}
+
+int make_tensor_map_f64(TensorMap* out, const void* base, int rank, const uint64_t* dims,
+                        const uint64_t* strides_bytes, const uint32_t* box) {
+  return make_tensor_map(out, CU_TENSOR_MAP_DATA_TYPE_FLOAT64, base, rank, dims, strides_bytes, box);
+}
+
+int make_tensor_map_bf16(TensorMap* out, const void* base, int rank, const uint64_t* dims,
+                         const uint64_t* strides_bytes, const uint32_t* box) {
+  return make_tensor_map(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, base, rank, dims, strides_bytes, box);
 }
 
 }  // namespace afq

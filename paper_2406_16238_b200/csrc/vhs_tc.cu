@@ -1,0 +1,361 @@
+// vhs_tc.cu - V_HS build in emulated single precision on the 5th-generation tensor cores
+// (mixed precision: "single precision is used for propagations and double precision is used for
+// local energy estimation"; Eq. 9):
+//     A[(w, plane)][p][q] = sum_g Cf[(w, plane)][g] * L[g][p][q]
+//
+// FP64 has no tcgen05 kind, FP32 neither (kind::tf32 keeps 10 mantissa bits).  Single precision is
+// therefore EMULATED: every double x is split once into three bfloat16 numbers x = h + m + l + O(2^-24 x)
+// (h = bf16(x), m = bf16(x - h), l = bf16(x - h - m)), and the product of two such numbers keeps the six
+// terms of order <= 2:  hh + hm + mh + hl + lh + mm.  A bf16 x bf16 product is exact in FP32 and
+// tcgen05.mma.kind::f16 accumulates in FP32 in tensor memory, so the result carries the 24 significant bits
+// of an FP32 GEMM with FP32 accumulation.
+//
+// Data: only tiles touching the upper triangle (same 4 p x 32 q tiles and tile list as vhs_ws.cu) are kept,
+// K-MAJOR (gamma contiguous) so that both operands are the canonical SWIZZLE_128B K-major UMMA layout:
+//     Lb[tile][3 planes][128 n = (pl, qj)][Gp]   bf16, Gp = n_chol rounded up to 64, zero padded   (setup)
+//     Ab[3 planes][Rp rows = (w, plane)][Gp]     bf16, Rp = rows rounded up to 128                 (per step)
+// 6 bytes per kept element of L: 21.5 GB at M = 1200, Nchol = 4800 (dense FP64: 55.3 GB).
+//
+// Kernel: one persistent CTA per SM, 6 warps.  Warp 0: TMA producer (one box {64 g, 128 rows, 3 planes}
+// per operand and stage, mbarrier ring).  Warp 1: allocates tensor memory and issues tcgen05.mma
+// (M = 128, N = 128, K = 16; 4 k-steps x 6 plane pairs per stage); tcgen05.commit frees the stage and
+// publishes the accumulator.  Warps 2-5: epilogue - tcgen05.ld of the 128 x 128 FP32 accumulator (one row
+// per thread), conversion to double, store at [p][q] and mirrored at [q][p]; two accumulators in tensor
+// memory let the epilogue of one tile overlap the mainloop of the next.
+#include <cuda_bf16.h>
+
+#include <vector>
+
+#include "internal.h"
+#include "tma.cuh"
+
+namespace afq {
+
+namespace {
+
+constexpr int TC_BK = 64;                       // gamma per stage: 128 bytes of bf16 = one swizzle row
+constexpr int TC_M = 128, TC_N = 128;
+constexpr int TC_PT = 4, TC_QT = 32;            // tile = 4 p x 32 q, as vhs_ws.cu
+constexpr int TC_PLANE = TC_M * 128;            // bytes of one plane of one operand in a stage (16 KB)
+constexpr int TC_OPER = 3 * TC_PLANE;           // 48 KB
+constexpr int TC_STAGE = 2 * TC_OPER;           // 96 KB
+constexpr int TC_STAGES = 2;
+constexpr int TC_ACC = 2;                       // accumulators in tensor memory (128 columns each)
+constexpr int TC_TMEM_COLS = 256;
+constexpr int TC_THREADS = 192;
+constexpr size_t TC_SMEM = (size_t)TC_STAGES * TC_STAGE + 1024 + 256;
+
+// ------------------------------------------------------------------ bf16 x 3 splitting
+__device__ __forceinline__ void split3(double x, __nv_bfloat16& h, __nv_bfloat16& m, __nv_bfloat16& l) {
+  h = __float2bfloat16_rn((float)x);
+  const double r1 = x - (double)__bfloat162float(h);
+  m = __float2bfloat16_rn((float)r1);
+  const double r2 = r1 - (double)__bfloat162float(m);
+  l = __float2bfloat16_rn((float)r2);
+}
+
+// Lb[t][plane][n][g] from the dense L[g][p][q]; grid (ntile, Gp / 64), 256 threads
+__global__ void __launch_bounds__(256) split_L_kernel(const double* __restrict__ L, __nv_bfloat16* __restrict__ Lb,
+                                                      const int* __restrict__ tiles, int M, int n_chol, int Gp) {
+  __shared__ double sm[32][TC_N + 1];
+  const int t = blockIdx.x, g00 = blockIdx.y * 64;
+  const int tn = tiles[t];
+  const int p0 = (tn >> 16) * TC_PT, q0 = (tn & 0xffff) * TC_QT;
+  const size_t MM = (size_t)M * M;
+  for (int pass = 0; pass < 2; ++pass) {
+    const int g0 = g00 + pass * 32;
+    for (int idx = threadIdx.x; idx < 32 * TC_N; idx += 256) {
+      const int gl = idx / TC_N, n = idx % TC_N;
+      const int p = p0 + n / TC_QT, q = q0 + n % TC_QT, g = g0 + gl;
+      sm[gl][n] = (g < n_chol && p < M && q < M) ? L[(size_t)g * MM + (size_t)p * M + q] : 0.0;
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < 32 * TC_N; idx += 256) {
+      const int n = idx / 32, gl = idx % 32;
+      __nv_bfloat16 h, m, l;
+      split3(sm[gl][n], h, m, l);
+      const size_t o = ((size_t)t * 3 * TC_N + n) * Gp + g0 + gl;
+      Lb[o] = h;
+      Lb[o + (size_t)TC_N * Gp] = m;
+      Lb[o + (size_t)2 * TC_N * Gp] = l;
+    }
+    __syncthreads();
+  }
+}
+
+// Ab[plane][r][g] from Cf[r][g]; rows >= rows and g >= n_chol are zero
+__global__ void __launch_bounds__(256) split_cf_kernel(const double* __restrict__ Cf, __nv_bfloat16* __restrict__ Ab,
+                                                       int rows, int n_chol, int Rp, int Gp) {
+  const int r = blockIdx.y;
+  const size_t plane = (size_t)Rp * Gp;
+  for (int g = blockIdx.x * blockDim.x + threadIdx.x; g < Gp; g += gridDim.x * blockDim.x) {
+    const double x = (r < rows && g < n_chol) ? Cf[(size_t)r * n_chol + g] : 0.0;
+    __nv_bfloat16 h, m, l;
+    split3(x, h, m, l);
+    const size_t o = (size_t)r * Gp + g;
+    Ab[o] = h;
+    Ab[o + plane] = m;
+    Ab[o + 2 * plane] = l;
+  }
+}
+
+// ------------------------------------------------------------------ tcgen05 building blocks
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
+
+// whole warp: allocate TC_TMEM_COLS columns, base address written to *slot (shared memory)
+__device__ __forceinline__ void tmem_alloc(uint32_t* slot) {
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(slot)),
+               "n"(TC_TMEM_COLS)
+               : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t base) {
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(base), "n"(TC_TMEM_COLS) : "memory");
+}
+
+// shared-memory matrix descriptor: K-major, SWIZZLE_128B, 8-row groups 1024 bytes apart
+__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
+  uint64_t d = (uint64_t)((saddr & 0x3FFFF) >> 4);
+  d |= (uint64_t)1 << 16;                 // leading byte offset (unused for swizzled K-major)
+  d |= (uint64_t)(1024 >> 4) << 32;       // stride byte offset
+  d |= (uint64_t)1 << 46;                 // descriptor version (Blackwell)
+  d |= (uint64_t)2 << 61;                 // SWIZZLE_128B
+  return d;
+}
+// instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = 128
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) |
+                            ((uint32_t)(TC_M >> 4) << 24);
+
+__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
+      "l"(adesc), "l"(bdesc), "r"(kIdesc), "r"(accumulate)
+      : "memory");
+}
+// arrive on an mbarrier when every tcgen05.mma issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint64_t* bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(smem_u32(bar))
+               : "memory");
+}
+// this thread's lane of tensor memory, 32 consecutive FP32 columns
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
+        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
+        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr)
+      : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
+}
+
+struct TcArgs {
+  double* Cb[kMaxGroup];   // output base per block of rpm rows (as vhs_ws.cu)
+  int rpm;
+  const int* tiles;        // [ntile_n] packed (pb << 16 | qb)
+  int M, rows, KT;         // KT = Gp / 64
+  int ntile_n, mtiles;
+};
+
+__global__ void __launch_bounds__(TC_THREADS, 1)
+vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB, const TcArgs a) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)TC_STAGES * TC_STAGE);
+  uint64_t* empty = full + TC_STAGES;
+  uint64_t* tfull = empty + TC_STAGES;
+  uint64_t* tempty = tfull + TC_ACC;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + TC_ACC);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int ntiles = a.ntile_n * a.mtiles;
+
+  if (tid == 0) {
+    for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < TC_ACC; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      prefetch_tensormap(&tmA);
+      prefetch_tensormap(&tmB);
+      uint32_t it = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int tl = tile / a.mtiles, mt = tile % a.mtiles;
+        for (int kt = 0; kt < a.KT; ++kt, ++it) {
+          const int s = it % TC_STAGES;
+          mbar_wait(&empty[s], ((it / TC_STAGES) & 1) ^ 1);
+          mbar_expect_tx(&full[s], TC_STAGE);
+          unsigned char* sa = smem + (size_t)s * TC_STAGE;
+          tma_load_3d(sa, &tmA, &full[s], kt * TC_BK, mt * TC_M, 0);
+          tma_load_4d(sa + TC_OPER, &tmB, &full[s], kt * TC_BK, 0, 0, tl);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------------ MMA issuer (lane 0)
+    uint32_t it = 0, tc = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++tc) {
+      const int acc = tc % TC_ACC;
+      mbar_wait(&tempty[acc], ((tc / TC_ACC) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t d = tmem_base + (uint32_t)acc * TC_N;
+      for (int kt = 0; kt < a.KT; ++kt, ++it) {
+        const int s = it % TC_STAGES;
+        mbar_wait(&full[s], (it / TC_STAGES) & 1);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t sa = smem_u32(smem + (size_t)s * TC_STAGE), sb = sa + TC_OPER;
+          // plane pairs (A plane, B plane), small terms first: lh hl mm mh hm hh
+          const int pa[6] = {2, 0, 1, 1, 0, 0}, pb[6] = {0, 2, 1, 0, 1, 0};
+#pragma unroll
+          for (int k = 0; k < TC_BK / 16; ++k) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+              const uint64_t da = umma_desc(sa + pa[q] * TC_PLANE + k * 32);
+              const uint64_t db = umma_desc(sb + pb[q] * TC_PLANE + k * 32);
+              umma_bf16(d, da, db, (kt | k | q) != 0 ? 1u : 0u);
+            }
+          }
+          umma_commit(&empty[s]);                       // stage free when these MMAs have read it
+          if (kt == a.KT - 1) umma_commit(&tfull[acc]);  // accumulator complete
+        }
+        __syncwarp();
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ epilogue warps 2..5
+    const int quarter = warp & 3;                 // tensor-memory lanes 32 quarter .. 32 quarter + 31
+    const size_t MM = (size_t)a.M * a.M;
+    uint32_t tc = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++tc) {
+      const int acc = tc % TC_ACC;
+      const int tn = a.tiles[tile / a.mtiles], mt = tile % a.mtiles;
+      const int p0 = (tn >> 16) * TC_PT, q0 = (tn & 0xffff) * TC_QT;
+      mbar_wait(&tfull[acc], (tc / TC_ACC) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (uint32_t)acc * TC_N + ((uint32_t)(quarter * 32) << 16);
+      float v[TC_PT][32];
+#pragma unroll
+      for (int c = 0; c < TC_PT; ++c) tmem_ld32(taddr + c * 32, v[c]);
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(&tempty[acc]);    // the accumulator may be overwritten from here on
+      const int r = mt * TC_M + quarter * 32 + lane;
+      if (r >= a.rows) continue;
+      double* Cr = a.Cb[r / a.rpm] + (size_t)(r % a.rpm) * MM;
+      const bool fast = (q0 >= p0 + TC_PT) && (p0 + TC_PT <= a.M) && (q0 + TC_QT <= a.M);
+      if (fast) {
+        // strictly above the diagonal and inside the matrix: 4 rows of 32 q, and 32 mirrored rows of 4 p
+#pragma unroll
+        for (int c = 0; c < TC_PT; ++c) {
+          double2* d2 = reinterpret_cast<double2*>(Cr + (size_t)(p0 + c) * a.M + q0);
+#pragma unroll
+          for (int j = 0; j < 16; ++j) d2[j] = make_double2((double)v[c][2 * j], (double)v[c][2 * j + 1]);
+        }
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          double2* d2 = reinterpret_cast<double2*>(Cr + (size_t)(q0 + j) * a.M + p0);
+          d2[0] = make_double2((double)v[0][j], (double)v[1][j]);
+          d2[1] = make_double2((double)v[2][j], (double)v[3][j]);
+        }
+      } else {
+#pragma unroll
+        for (int c = 0; c < TC_PT; ++c) {
+          const int pp = p0 + c;
+          if (pp >= a.M) continue;
+#pragma unroll
+          for (int j = 0; j < 32; ++j) {
+            const int qq = q0 + j;
+            if (qq >= a.M || qq < pp) continue;
+            const double x = (double)v[c][j];
+            Cr[(size_t)pp * a.M + qq] = x;
+            if (qq > pp) Cr[(size_t)qq * a.M + pp] = x;
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc(tmem_base);
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------- host side
+int vhs_tc_gamma_padded(int n_chol) { return (n_chol + TC_BK - 1) / TC_BK * TC_BK; }
+int vhs_tc_rows_padded(int rows) { return (rows + TC_M - 1) / TC_M * TC_M; }
+size_t vhs_tc_L_elems(int ntile_n, int n_chol) { return (size_t)ntile_n * 3 * TC_N * vhs_tc_gamma_padded(n_chol); }
+size_t vhs_tc_cf_elems(int rows, int n_chol) { return (size_t)3 * vhs_tc_rows_padded(rows) * vhs_tc_gamma_padded(n_chol); }
+
+int run_vhs_tc_split_L(const double* L, void* Lb, const int* tiles_dev, int ntile_n, int M, int n_chol,
+                       cudaStream_t st) {
+  const int Gp = vhs_tc_gamma_padded(n_chol);
+  // grid.x up to 2^31 - 1 tiles; grid.y = Gp / 64 <= 65535 (n_chol < 4.2e6)
+  split_L_kernel<<<dim3(ntile_n, Gp / 64), 256, 0, st>>>(L, (__nv_bfloat16*)Lb, tiles_dev, M, n_chol, Gp);
+  return 1;
+}
+
+// A (scattered by owner as run_vhs_ws_scatter) from Cf [rows][n_chol] and the split tensor Lb; Ab is scratch
+int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, int nmember, int rows_per_member,
+               const int* tiles_dev, int ntile_n, int M, int n_chol, cudaStream_t st) {
+  if (nmember < 1 || nmember > kMaxGroup || rows_per_member < 1) return -1;
+  const int rows = nmember * rows_per_member;
+  const int Gp = vhs_tc_gamma_padded(n_chol), Rp = vhs_tc_rows_padded(rows);
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(vhs_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+    attr = true;
+  }
+  static int nsm = 0;
+  if (!nsm) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    if (nsm <= 0) nsm = 148;
+  }
+  split_cf_kernel<<<dim3((Gp + 255) / 256, Rp), 256, 0, st>>>(Cf, (__nv_bfloat16*)Ab, rows, n_chol, Rp, Gp);
+  TensorMap tmA, tmB;
+  {
+    const uint64_t dims[3] = {(uint64_t)Gp, (uint64_t)Rp, 3};
+    const uint64_t str[2] = {(uint64_t)Gp * 2, (uint64_t)Rp * Gp * 2};
+    const uint32_t box[3] = {TC_BK, TC_M, 3};
+    if (make_tensor_map_bf16(&tmA, Ab, 3, dims, str, box) != 0) return -1;
+  }
+  {
+    const uint64_t dims[4] = {(uint64_t)Gp, TC_N, 3, (uint64_t)ntile_n};
+    const uint64_t str[3] = {(uint64_t)Gp * 2, (uint64_t)TC_N * Gp * 2, (uint64_t)3 * TC_N * Gp * 2};
+    const uint32_t box[4] = {TC_BK, TC_N, 3, 1};
+    if (make_tensor_map_bf16(&tmB, Lb, 4, dims, str, box) != 0) return -1;
+  }
+  TcArgs a;
+  for (int r = 0; r < kMaxGroup; ++r) a.Cb[r] = r < nmember ? Cb[r] : nullptr;
+  a.rpm = rows_per_member;
+  a.tiles = tiles_dev; a.M = M; a.rows = rows; a.KT = Gp / TC_BK;
+  a.ntile_n = ntile_n; a.mtiles = Rp / TC_M;
+  const long nt = (long)a.ntile_n * a.mtiles;
+  const int grid = nt < nsm ? (int)nt : nsm;
+  vhs_tc_kernel<<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmB, a);
+  return 2;
+}
+
+}  // namespace afq

@@ -1,0 +1,181 @@
+"""GPU parity of the mixed-precision mode ("single precision is used for propagations and
+double precision is used for local energy estimation"): the V_HS build runs in
+emulated single precision on the tcgen05 tensor cores (bf16 x 3 operands, FP32 accumulation in tensor
+memory), everything else in double.  The oracle stays the FP64 definition; the tolerances below are
+single-precision ones derived in DESIGN.md (operand splitting keeps 24 bits; FP32 accumulation of
+n_chol <= 4800 terms: a few 1e-6 relative on A, times ||A|| ~ 0.4 on the walkers)."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from tests.gpu_util import Pair, energy_scale, planar_to_complex, rel_fro, rel_max
+
+pytestmark = pytest.mark.gpu
+
+TOL_A = 2e-5          # ||A_mixed - A||_F / ||A||_F per walker
+TOL_STEP = 1e-5       # walkers after one step
+TOL_OVLP = 5e-5       # overlaps (determinants of Nocc x Nocc blocks: errors add over the columns) and weights
+TOL_RUN = 2e-4        # after 10 free-running steps
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _mixed(pr, nw, **kw):
+    from paper_2406_16238_b200 import afqmc
+    cfg = pr.cfg
+    return afqmc.AFQMC(pr.h1, pr.L_dev, pr.trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=cfg.n_chol,
+                       max_walkers=nw, walker_kind=cfg.walker_kind, taylor_order=cfg.taylor_order,
+                       mixed_precision=True, **kw)
+
+
+def _step(g, walkers, weights, x, dt):
+    torch = _torch()
+    W = torch.from_numpy(np.ascontiguousarray(walkers)).cuda()
+    wt = torch.from_numpy(np.ascontiguousarray(weights)).cuda()
+    xd = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    ov = torch.empty(W.shape[0], dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    g.step(W, wt, xd, dt)
+    g.get_overlaps(ov)
+    g.sync()
+    return W.cpu().numpy(), wt.cpu().numpy(), ov.cpu().numpy()
+
+
+# tile shapes: M below one q tile (24), ragged q tiles (38, 108), several row tiles (nw = 70 -> 140 rows),
+# n_chol not a multiple of the 64-gamma stage (54, 300, 540)
+CASES = [("c1", 16, {}), ("c2", 24, {}), ("c1", 5, dict(M=38, n_alpha=7, n_beta=7, n_chol=54)),
+         ("c3", 70, dict(n_chol=300))]
+
+
+@pytest.mark.parametrize("name,nw,over", CASES)
+def test_vhs_and_one_step(name, nw, over):
+    _torch()
+    pr = Pair(name, nw=nw, ortho_every=0, **over)
+    o, cfg = pr.oracle, pr.cfg
+    g = _mixed(pr, nw)
+    x = pr.fields(0)
+    w0 = np.linspace(0.5, 1.5, nw)
+    new_o, info = o.propagate(pr.walkers0, x, cfg.dt)
+    Wg, wg, ovg = _step(g, pr.walkers0, w0, x, cfg.dt)
+    A = planar_to_complex(g.debug_read(1), (nw, cfg.M, cfg.M))
+    err = rel_fro(A, info["A"])
+    assert err < TOL_A
+    assert err > 1e-9                                         # it really is the single-precision route
+    assert np.array_equal(A, A.transpose(0, 2, 1))            # mirrored stores: exactly symmetric
+    assert rel_fro(Wg, new_o) < TOL_STEP
+    _, w_o, ov_o = o.step(pr.walkers0, w0, x, cfg.dt)
+    assert rel_max(ovg, ov_o) < TOL_OVLP
+    assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_OVLP
+    g.close()
+    pr.close()
+
+
+def test_local_energy_stays_in_double():
+    """The energy of given walkers does not go through the single-precision kernel: 1e-11 as the double path."""
+    torch = _torch()
+    pr = Pair("c2", nw=24)
+    g = _mixed(pr, 24)
+    W = torch.from_numpy(pr.walkers0).cuda()
+    E = torch.empty((24, 3), dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    g.local_energy(W, E)
+    g.sync()
+    Eo = pr.oracle.local_energy(pr.walkers0)
+    sc = energy_scale(pr.oracle, pr.walkers0, Eo)
+    for k in range(3):
+        assert rel_max(E.cpu().numpy()[:, k], Eo[:, k], scale=sc) < 1e-11
+    g.close()
+    pr.close()
+
+
+@pytest.mark.parametrize("name,nw,ortho", [("c1", 16, 0), ("c2", 64, 5)])
+def test_free_running(name, nw, ortho):
+    torch = _torch()
+    pr = Pair(name, nw=nw, ortho_every=ortho)
+    o, cfg = pr.oracle, pr.cfg
+    g = _mixed(pr, nw, ortho_every=ortho)
+    Wo, wo = pr.walkers0, np.ones(nw)
+    Wg, wg = Wo.copy(), wo.copy()
+    for s in range(10):
+        x = pr.fields(s)
+        Wg, wg, ovg = _step(g, Wg, wg, x, cfg.dt)
+        Wo, wo, ovo = o.step(Wo, wo, x, cfg.dt)
+    assert rel_fro(Wg, Wo) < TOL_RUN
+    assert rel_max(wg, wo, scale=np.maximum(np.abs(wo), 1e-3)) < TOL_RUN
+    assert rel_max(ovg, ovo) < TOL_RUN
+    E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    Wd = torch.from_numpy(Wg).cuda()
+    torch.cuda.synchronize()
+    g.local_energy(Wd, E)
+    g.sync()
+    Eo = o.local_energy(Wo)
+    sc = energy_scale(o, Wo, Eo)
+    assert rel_max(E.cpu().numpy()[:, 0], Eo[:, 0], scale=sc) < TOL_RUN
+    g.close()
+    pr.close()
+
+
+def test_mixed_precision_in_a_group_of_two():
+    """Distributed Hamiltonian + mixed precision: the tcgen05 epilogue stores into the owners' slots."""
+    torch = _torch()
+    from oracle.afqmc_oracle import AFQMCOracle
+    from paper_2406_16238_b200 import afqmc, inputs, sharded
+    nw = 6
+    cfg, h1, L, trial, walkers = inputs.make_problem_host("c1", nw=2 * nw)
+    sl = sharded.gamma_slices(cfg.n_chol, 2)
+    members = [afqmc.AFQMC(h1, torch.from_numpy(np.ascontiguousarray(L[a:b])).cuda(), trial, M=cfg.M, n_alpha=cfg.n_alpha,
+                           n_beta=cfg.n_beta, n_chol=b - a, max_walkers=nw, walker_kind=cfg.walker_kind,
+                           group_size=2, group_rank=r, mixed_precision=True) for r, (a, b) in enumerate(sl)]
+    total = members[0].shard_setup_partial() + members[1].shard_setup_partial()
+    addrs = np.stack([m.shard_get_buffers() for m in members])
+    for m in members:
+        m.shard_setup_finish(total)
+        m.shard_set_peers(addrs)
+    x = inputs.make_aux_fields(cfg, 0, 0, 2 * nw)
+    W = [torch.from_numpy(np.ascontiguousarray(walkers[r * nw:(r + 1) * nw])).cuda() for r in range(2)]
+    wt = [torch.ones(nw, dtype=torch.float64, device="cuda") for _ in range(2)]
+    xs = [torch.from_numpy(np.ascontiguousarray(x[:, a:b])).cuda() for a, b in sl]
+    torch.cuda.synchronize()
+    for m, w in zip(members, W):
+        m.shard_theta(w)
+    for m in members:
+        m.sync()
+    for m, xx in zip(members, xs):
+        m.shard_vhs(xx, cfg.dt, nw)
+    for m in members:
+        m.sync()
+    for m, w, t in zip(members, W, wt):
+        m.shard_propagate(w, t, cfg.dt)
+    for m in members:
+        m.sync()
+    o = AFQMCOracle(h1, L, trial, cfg.n_alpha, cfg.n_beta, cfg.walker_kind, taylor_order=cfg.taylor_order)
+    Wo, wo, _ = o.step(walkers, np.ones(2 * nw), x, cfg.dt)
+    Wg = np.concatenate([w.cpu().numpy() for w in W])
+    err = rel_fro(Wg, Wo)
+    assert 1e-10 < err < TOL_STEP
+    assert rel_max(np.concatenate([t.cpu().numpy() for t in wt]), wo) < TOL_OVLP
+    for m in members:
+        m.close()
+
+
+def test_mixed_precision_argument_checks():
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc, inputs
+    cfg, h1, L, trial, _ = inputs.make_problem_host("c1", nw=4, M=37, n_alpha=7, n_beta=7, n_chol=53)
+    Ld = torch.from_numpy(L).cuda()
+    kw = dict(M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=cfg.n_chol, max_walkers=4, walker_kind=0)
+    with pytest.raises(afqmc.AfqmcError) as e:
+        afqmc.AFQMC(h1, Ld, trial, mixed_precision=True, **kw)
+    assert e.value.code == -6
+    cfg, h1, L, trial, _ = inputs.make_problem_host("c1", nw=4)
+    Ld = torch.from_numpy(L).cuda()
+    kw = dict(M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=cfg.n_chol, max_walkers=4, walker_kind=0)
+    with pytest.raises(afqmc.AfqmcError) as e:
+        afqmc.AFQMC(h1, Ld, trial, mixed_precision=True, pack_chol=True, **kw)
+    assert e.value.code == -1
