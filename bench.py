@@ -439,7 +439,7 @@ def main():
             per_stage[k]["frac_of_dmma_peak"] = tf / peak_dmma
     if args.mixed_precision and "vhs" in per_stage:
         # bf16 x 3 on tcgen05: HBM bound (the split upper-triangle tiles are streamed once per step)
-        ntile = sum(1 for pb in range((cfg.M + 3) // 4) for qb in range((cfg.M + 31) // 32) if qb * 32 + 31 >= pb * 4)
+        ntile = sum(1 for pb in range((cfg.M + 7) // 8) for qb in range((cfg.M + 15) // 16) if qb * 16 + 15 >= pb * 8)
         gp = (cfg.n_chol + 63) // 64 * 64
         by = ntile * 3 * 128 * gp * 2 + nw * 2 * cfg.M * cfg.M * 8
         v = per_stage["vhs"]

@@ -61,6 +61,8 @@ struct afqmc_handle {
   int* vhs_tiles = nullptr;
   double* Lpk = nullptr;   // tile-packed upper triangle of L (pack_chol)
   void *Lb = nullptr, *Ab = nullptr;   // mixed precision: bf16 x 3 split tiles of L, split coefficients
+  int* tc_tiles = nullptr;
+  int tc_ntile = 0;
   int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
@@ -273,7 +275,7 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   if (h->Lb) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
     double* Cb[1] = {h->A};
-    const int r = run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, 1, 2 * nw, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
+    const int r = run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, 1, 2 * nw, h->tc_tiles, h->tc_ntile, M, nc, h->st);
     if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs (mixed precision): tensor map encode failed");
     h->launches += r;
   } else if (h->ws_vhs) {
@@ -708,10 +710,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->mixed_precision) {
     if (!h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "mixed_precision needs even M and n_chol");
     if (p->pack_chol) return bail(AFQMC_ERR_INVALID, "mixed_precision keeps its own split tiles: pack_chol must be 0");
-    h->Lb = dalloc(h, (vhs_tc_L_elems(h->vhs_ntile, nc) * 2 + 7) / 8);
+    {
+      std::vector<int> tl;
+      h->tc_ntile = vhs_tc_tile_list(M, &tl);
+      h->tc_tiles = (int*)dalloc(h, (tl.size() + 1) / 2 + 1);
+      if (!h->tc_tiles) return bail(AFQMC_ERR_ALLOC, "device allocation failed (tile list)");
+      if (cudaMemcpy(h->tc_tiles, tl.data(), tl.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+        return bail(AFQMC_ERR_CUDA, "tile list upload failed");
+    }
+    h->Lb = dalloc(h, (vhs_tc_L_elems(h->tc_ntile, nc) * 2 + 7) / 8);
     h->Ab = dalloc(h, (vhs_tc_cf_elems(2 * mwg, nc) * 2 + 7) / 8);
     if (!h->Lb || !h->Ab) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Cholesky tensor)");
-    h->launches += run_vhs_tc_split_L(h->L, h->Lb, h->vhs_tiles, h->vhs_ntile, M, nc, h->st);
+    h->launches += run_vhs_tc_split_L(h->L, h->Lb, h->tc_tiles, h->tc_ntile, M, nc, h->st);
   }
 
   // ---- E_shift = trial energy ---------------------------------------------------------------
@@ -1106,7 +1116,7 @@ int32_t afqmc_shard_vhs(afqmc_handle* h, const double* aux_local, double dt, int
   StageTimer tm(h, AFQMC_STAGE_VHS);
   double* Cb[kMaxGroup];
   for (int o = 0; o < G; ++o) Cb[o] = h->peer[1][o] + (size_t)h->rank * mw * 2 * MM;
-  const int r = h->Lb ? run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile, h->M, h->n_chol, h->st)
+  const int r = h->Lb ? run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, G, 2 * nw, h->tc_tiles, h->tc_ntile, h->M, h->n_chol, h->st)
                       : run_vhs_ws_scatter(h->Cf, h->Lpk ? h->Lpk : h->L, Cb, G, 2 * nw, h->vhs_tiles, h->vhs_ntile,
                                            h->M, h->n_chol, h->Lpk != nullptr, h->st);
   if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs: tensor map encode failed");

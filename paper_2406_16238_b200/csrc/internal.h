@@ -118,6 +118,7 @@ int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile
 
 // vhs_tc.cu: V_HS build in emulated single precision (bf16 x 3 on tcgen05, FP32 accumulation in TMEM)
 int vhs_tc_gamma_padded(int n_chol);
+int vhs_tc_tile_list(int M, std::vector<int>* out);   // its own 8 p x 16 q tiles touching the upper triangle
 size_t vhs_tc_L_elems(int ntile_n, int n_chol);      // bf16 elements of the split tile tensor
 size_t vhs_tc_cf_elems(int rows, int n_chol);        // bf16 elements of the split coefficient scratch
 int run_vhs_tc_split_L(const double* L, void* Lb, const int* tiles_dev, int ntile_n, int M, int n_chol,

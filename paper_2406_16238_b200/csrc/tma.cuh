@@ -29,9 +29,9 @@ struct alignas(64) TensorMap { unsigned char bytes[128]; };   // CUtensorMap, op
 int make_tensor_map_f64(TensorMap* out, const void* base, int rank, const uint64_t* dims,
                         const uint64_t* strides_bytes, const uint32_t* box);
 
-// the same for bfloat16 elements (box inner extent 64 elements = 128 bytes with SWIZZLE_128B)
+// the same for bfloat16 elements; swizzle_bytes = 64 or 128 = the byte extent of the box's inner dimension
 int make_tensor_map_bf16(TensorMap* out, const void* base, int rank, const uint64_t* dims,
-                         const uint64_t* strides_bytes, const uint32_t* box);
+                         const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes);
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);

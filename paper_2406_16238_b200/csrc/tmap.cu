@@ -30,7 +30,8 @@ EncodeTiledFn encode_fn() {
 }  // namespace
 
 static int make_tensor_map(TensorMap* out, CUtensorMapDataType dt, const void* base, int rank,
-                           const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box) {
+                           const uint64_t* dims, const uint64_t* strides_bytes, const uint32_t* box,
+                           CUtensorMapSwizzle sw = CU_TENSOR_MAP_SWIZZLE_128B) {
   static_assert(sizeof(TensorMap) == sizeof(CUtensorMap), "CUtensorMap is 128 bytes");
   EncodeTiledFn fn = encode_fn();
   if (!fn) return -1;
@@ -41,7 +42,7 @@ static int make_tensor_map(TensorMap* out, CUtensorMapDataType dt, const void* b
   for (int i = 0; i < rank - 1; ++i) gs[i] = strides_bytes[i];
   CUresult r = fn(reinterpret_cast<CUtensorMap*>(out), dt, (cuuint32_t)rank,
                   const_cast<void*>(base), gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE,
-                  CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                  sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   return (int)r;
 }
@@ -52,8 +53,10 @@ int make_tensor_map_f64(TensorMap* out, const void* base, int rank, const uint64
 }
 
 int make_tensor_map_bf16(TensorMap* out, const void* base, int rank, const uint64_t* dims,
-                         const uint64_t* strides_bytes, const uint32_t* box) {
-  return make_tensor_map(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, base, rank, dims, strides_bytes, box);
+                         const uint64_t* strides_bytes, const uint32_t* box, int swizzle_bytes) {
+  if (swizzle_bytes != 64 && swizzle_bytes != 128) return -1;
+  return make_tensor_map(out, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, base, rank, dims, strides_bytes, box,
+                         swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B);
 }
 
 }  // namespace afq

@@ -12,11 +12,11 @@
 //
 // Data: only tiles touching the upper triangle (same 4 p x 32 q tiles and tile list as vhs_ws.cu) are kept,
 // K-MAJOR (gamma contiguous) so that both operands are the canonical SWIZZLE_128B K-major UMMA layout:
-//     Lb[tile][3 planes][128 n = (pl, qj)][Gp]   bf16, Gp = n_chol rounded up to 64, zero padded   (setup)
+//     Lb[3 planes][tile][128 n = (pl, qj)][Gp]   bf16, Gp = n_chol rounded up to 64, zero padded   (setup)
 //     Ab[3 planes][Rp rows = (w, plane)][Gp]     bf16, Rp = rows rounded up to 128                 (per step)
 // 6 bytes per kept element of L: 21.5 GB at M = 1200, Nchol = 4800 (dense FP64: 55.3 GB).
 //
-// Kernel: one persistent CTA per SM, 6 warps.  Warp 0: TMA producer (one box {64 g, 128 rows, 3 planes}
+// Kernel: one persistent CTA per SM, 6 warps.  Warp 0: TMA producer (one box {32 g, 128 rows, 3 planes}
 // per operand and stage, mbarrier ring).  Warp 1: allocates tensor memory and issues tcgen05.mma
 // (M = 128, N = 128, K = 16; 4 k-steps x 6 plane pairs per stage); tcgen05.commit frees the stage and
 // publishes the accumulator.  Warps 2-5: epilogue - tcgen05.ld of the 128 x 128 FP32 accumulator (one row
@@ -33,17 +33,19 @@ namespace afq {
 
 namespace {
 
-constexpr int TC_BK = 64;                       // gamma per stage: 128 bytes of bf16 = one swizzle row
+constexpr int TC_GPAD = 64;                     // gamma extent of the split tensors is padded to this
+constexpr int TC_BK = 32;                       // gamma per stage: 64 bytes of bf16 = one SWIZZLE_64B row
 constexpr int TC_M = 128, TC_N = 128;
-constexpr int TC_PT = 4, TC_QT = 32;            // tile = 4 p x 32 q, as vhs_ws.cu
-constexpr int TC_PLANE = TC_M * 128;            // bytes of one plane of one operand in a stage (16 KB)
-constexpr int TC_OPER = 3 * TC_PLANE;           // 48 KB
-constexpr int TC_STAGE = 2 * TC_OPER;           // 96 KB
-constexpr int TC_STAGES = 2;
-constexpr int TC_ACC = 2;                       // accumulators in tensor memory (128 columns each)
-constexpr int TC_TMEM_COLS = 256;
+constexpr int TC_NT = 2;                        // N tiles per work unit: one A stage feeds both
+constexpr int TC_PT = 8, TC_QT = 16;            // tile = 8 p x 16 q: 128-byte runs of q, 64-byte mirrored runs of p
+constexpr int TC_PLANE = TC_M * TC_BK * 2;      // bytes of one plane of one 128-row operand in a stage (8 KB)
+constexpr int TC_OPER = 3 * TC_PLANE;           // 24 KB
+constexpr int TC_STAGE = (1 + TC_NT) * TC_OPER; // 72 KB: A, B tile 0, B tile 1
+constexpr int TC_STAGES = 3;
+constexpr int TC_ACC = 2;                       // accumulator sets in tensor memory (TC_NT x 128 columns each)
+constexpr int TC_TMEM_COLS = 512;
 constexpr int TC_THREADS = 192;
-constexpr size_t TC_SMEM = (size_t)TC_STAGES * TC_STAGE + 1024 + 256;
+constexpr size_t TC_SMEM = (size_t)TC_STAGES * TC_STAGE + 1024 + 256 + 1024;   // + alignment, barriers, row table
 
 // ------------------------------------------------------------------ bf16 x 3 splitting
 __device__ __forceinline__ void split3(double x, __nv_bfloat16& h, __nv_bfloat16& m, __nv_bfloat16& l) {
@@ -54,7 +56,7 @@ __device__ __forceinline__ void split3(double x, __nv_bfloat16& h, __nv_bfloat16
   l = __float2bfloat16_rn((float)r2);
 }
 
-// Lb[t][plane][n][g] from the dense L[g][p][q]; grid (ntile, Gp / 64), 256 threads
+// Lb[plane][t][n][g] from the dense L[g][p][q]; grid (ntile, Gp / 64), 256 threads
 __global__ void __launch_bounds__(256) split_L_kernel(const double* __restrict__ L, __nv_bfloat16* __restrict__ Lb,
                                                       const int* __restrict__ tiles, int M, int n_chol, int Gp) {
   __shared__ double sm[32][TC_N + 1];
@@ -74,10 +76,10 @@ __global__ void __launch_bounds__(256) split_L_kernel(const double* __restrict__
       const int n = idx / 32, gl = idx % 32;
       __nv_bfloat16 h, m, l;
       split3(sm[gl][n], h, m, l);
-      const size_t o = ((size_t)t * 3 * TC_N + n) * Gp + g0 + gl;
+      const size_t o = ((size_t)t * TC_N + n) * Gp + g0 + gl, plane = (size_t)gridDim.x * TC_N * Gp;
       Lb[o] = h;
-      Lb[o + (size_t)TC_N * Gp] = m;
-      Lb[o + (size_t)2 * TC_N * Gp] = l;
+      Lb[o + plane] = m;
+      Lb[o + 2 * plane] = l;
     }
     __syncthreads();
   }
@@ -114,17 +116,17 @@ __device__ __forceinline__ void tmem_dealloc(uint32_t base) {
   asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(base), "n"(TC_TMEM_COLS) : "memory");
 }
 
-// shared-memory matrix descriptor: K-major, SWIZZLE_128B, 8-row groups 1024 bytes apart
+// shared-memory matrix descriptor: K-major, SWIZZLE_64B (rows of 64 bytes), 8-row groups 512 bytes apart
 __device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
   uint64_t d = (uint64_t)((saddr & 0x3FFFF) >> 4);
   d |= (uint64_t)1 << 16;                 // leading byte offset (unused for swizzled K-major)
-  d |= (uint64_t)(1024 >> 4) << 32;       // stride byte offset
+  d |= (uint64_t)(512 >> 4) << 32;        // stride byte offset
   d |= (uint64_t)1 << 46;                 // descriptor version (Blackwell)
-  d |= (uint64_t)2 << 61;                 // SWIZZLE_128B
+  d |= (uint64_t)4 << 61;                 // SWIZZLE_64B
   return d;
 }
-// instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = 128
-constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(TC_N >> 3) << 17) |
+// instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = 256 (both tiles of a pair)
+constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((TC_NT * TC_N) >> 3) << 17) |
                             ((uint32_t)(TC_M >> 4) << 24);
 
 __device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
@@ -157,12 +159,28 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
   for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
 }
 
+// 32 x 32 transpose across a warp: afterwards x[i] of lane l is what x[l] of lane i was
+__device__ __forceinline__ void warp_transpose32(float (&x)[32], int lane) {
+#pragma unroll
+  for (int s = 16; s >= 1; s >>= 1) {
+    const bool up = (lane & s) != 0;
+#pragma unroll
+    for (int i = 0; i < 32; ++i) {
+      if ((i & s) == 0) {
+        const float send = up ? x[i] : x[i + s];
+        const float recv = __shfl_xor_sync(0xffffffffu, send, s);
+        if (up) x[i] = recv; else x[i + s] = recv;
+      }
+    }
+  }
+}
+
 struct TcArgs {
   double* Cb[kMaxGroup];   // output base per block of rpm rows (as vhs_ws.cu)
   int rpm;
   const int* tiles;        // [ntile_n] packed (pb << 16 | qb)
-  int M, rows, KT;         // KT = Gp / 64
-  int ntile_n, mtiles;
+  int M, rows, KT;         // KT = Gp / TC_BK
+  int ntile_n, npairs, mtiles;
 };
 
 __global__ void __launch_bounds__(TC_THREADS, 1)
@@ -175,7 +193,7 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
   uint64_t* tempty = tfull + TC_ACC;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + TC_ACC);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int ntiles = a.ntile_n * a.mtiles;
+  const int nunits = a.npairs * a.mtiles;        // work unit = (pair of N tiles, 128-row block)
 
   if (tid == 0) {
     for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
@@ -194,26 +212,27 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       prefetch_tensormap(&tmA);
       prefetch_tensormap(&tmB);
       uint32_t it = 0;
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int tl = tile / a.mtiles, mt = tile % a.mtiles;
+      for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
+        const int pr = u / a.mtiles, mt = u % a.mtiles;
         for (int kt = 0; kt < a.KT; ++kt, ++it) {
           const int s = it % TC_STAGES;
           mbar_wait(&empty[s], ((it / TC_STAGES) & 1) ^ 1);
           mbar_expect_tx(&full[s], TC_STAGE);
           unsigned char* sa = smem + (size_t)s * TC_STAGE;
           tma_load_3d(sa, &tmA, &full[s], kt * TC_BK, mt * TC_M, 0);
-          tma_load_4d(sa + TC_OPER, &tmB, &full[s], kt * TC_BK, 0, 0, tl);
+          // both tiles of the pair in one box; a tile index past the end reads as zeros
+          tma_load_4d(sa + TC_OPER, &tmB, &full[s], kt * TC_BK, 0, pr * TC_NT, 0);
         }
       }
     }
   } else if (warp == 1) {
     // ------------------------------------------------------------------ MMA issuer (lane 0)
     uint32_t it = 0, tc = 0;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++tc) {
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
       const int acc = tc % TC_ACC;
       mbar_wait(&tempty[acc], ((tc / TC_ACC) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t d = tmem_base + (uint32_t)acc * TC_N;
+      const uint32_t d = tmem_base + (uint32_t)acc * (TC_NT * TC_N);
       for (int kt = 0; kt < a.KT; ++kt, ++it) {
         const int s = it % TC_STAGES;
         mbar_wait(&full[s], (it / TC_STAGES) & 1);
@@ -227,64 +246,98 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
 #pragma unroll
             for (int q = 0; q < 6; ++q) {
               const uint64_t da = umma_desc(sa + pa[q] * TC_PLANE + k * 32);
-              const uint64_t db = umma_desc(sb + pb[q] * TC_PLANE + k * 32);
+              const uint64_t db = umma_desc(sb + pb[q] * (TC_NT * TC_PLANE) + k * 32);   // 256 rows: tile 0, tile 1
               umma_bf16(d, da, db, (kt | k | q) != 0 ? 1u : 0u);
             }
           }
           umma_commit(&empty[s]);                       // stage free when these MMAs have read it
-          if (kt == a.KT - 1) umma_commit(&tfull[acc]);  // accumulator complete
+          if (kt == a.KT - 1) umma_commit(&tfull[acc]);  // accumulators complete
         }
         __syncwarp();
       }
     }
   } else {
     // ------------------------------------------------------------------ epilogue warps 2..5
+    // A thread owns one accumulator row (tensor-memory lane) = one (walker, plane) row of A.  Tiles
+    // strictly above the diagonal are transposed across the warp 32 x 32 values at a time, so that one
+    // store instruction writes, for ONE row, two 128-byte runs of q (direct) or four 64-byte runs of p
+    // (mirrored) instead of 32 scattered 8-byte pieces.
     const int quarter = warp & 3;                 // tensor-memory lanes 32 quarter .. 32 quarter + 31
     const size_t MM = (size_t)a.M * a.M;
+    double** rowp = reinterpret_cast<double**>(tmem_slot + 4) + quarter * 32;   // this warp's 32 row bases
     uint32_t tc = 0;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++tc) {
+    int mt_cur = -1;
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
       const int acc = tc % TC_ACC;
-      const int tn = a.tiles[tile / a.mtiles], mt = tile % a.mtiles;
-      const int p0 = (tn >> 16) * TC_PT, q0 = (tn & 0xffff) * TC_QT;
+      const int pr = u / a.mtiles, mt = u % a.mtiles;
+      if (mt != mt_cur) {
+        const int r = mt * TC_M + quarter * 32 + lane;
+        __syncwarp();
+        rowp[lane] = r < a.rows ? a.Cb[r / a.rpm] + (size_t)(r % a.rpm) * MM : nullptr;
+        __syncwarp();
+        mt_cur = mt;
+      }
+      double* Cr = rowp[lane];
       mbar_wait(&tfull[acc], (tc / TC_ACC) & 1);
       tc_fence_after();
-      const uint32_t taddr = tmem_base + (uint32_t)acc * TC_N + ((uint32_t)(quarter * 32) << 16);
-      float v[TC_PT][32];
+#pragma unroll 1
+      for (int nt = 0; nt < TC_NT; ++nt) {
+        const int tl = pr * TC_NT + nt;
+        const uint32_t taddr = tmem_base + (uint32_t)(acc * TC_NT + nt) * TC_N + ((uint32_t)(quarter * 32) << 16);
+        float v[4][32];                           // v[c][j]: n = 32 c + j, p = p0 + n / 16, q = q0 + n % 16
 #pragma unroll
-      for (int c = 0; c < TC_PT; ++c) tmem_ld32(taddr + c * 32, v[c]);
-      tc_fence_before();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&tempty[acc]);    // the accumulator may be overwritten from here on
-      const int r = mt * TC_M + quarter * 32 + lane;
-      if (r >= a.rows) continue;
-      double* Cr = a.Cb[r / a.rpm] + (size_t)(r % a.rpm) * MM;
-      const bool fast = (q0 >= p0 + TC_PT) && (p0 + TC_PT <= a.M) && (q0 + TC_QT <= a.M);
-      if (fast) {
-        // strictly above the diagonal and inside the matrix: 4 rows of 32 q, and 32 mirrored rows of 4 p
-#pragma unroll
-        for (int c = 0; c < TC_PT; ++c) {
-          double2* d2 = reinterpret_cast<double2*>(Cr + (size_t)(p0 + c) * a.M + q0);
-#pragma unroll
-          for (int j = 0; j < 16; ++j) d2[j] = make_double2((double)v[c][2 * j], (double)v[c][2 * j + 1]);
+        for (int c = 0; c < 4; ++c) tmem_ld32(taddr + c * 32, v[c]);
+        if (nt == TC_NT - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty[acc]);    // the accumulators may be overwritten from here on
         }
+        if (tl >= a.ntile_n) continue;
+        const int tn = a.tiles[tl];
+        const int p0 = (tn >> 16) * TC_PT, q0 = (tn & 0xffff) * TC_QT;
+        const bool fast = (q0 >= p0 + TC_PT) && (p0 + TC_PT <= a.M) && (q0 + TC_QT <= a.M);
+        if (fast) {
+          // mirrored: block b holds q = q0 + 4 b + j / 8, p = p0 + j % 8
 #pragma unroll
-        for (int j = 0; j < 32; ++j) {
-          double2* d2 = reinterpret_cast<double2*>(Cr + (size_t)(q0 + j) * a.M + p0);
-          d2[0] = make_double2((double)v[0][j], (double)v[1][j]);
-          d2[1] = make_double2((double)v[2][j], (double)v[3][j]);
-        }
-      } else {
+          for (int b = 0; b < 4; ++b) {
+            float t[32];
 #pragma unroll
-        for (int c = 0; c < TC_PT; ++c) {
-          const int pp = p0 + c;
-          if (pp >= a.M) continue;
+            for (int j = 0; j < 32; ++j) {
+              const int n = (j % 8) * TC_QT + 4 * b + j / 8;
+              t[j] = v[n / 32][n % 32];
+            }
+            warp_transpose32(t, lane);
+            const size_t off = (size_t)(q0 + 4 * b + lane / 8) * a.M + p0 + lane % 8;
 #pragma unroll
-          for (int j = 0; j < 32; ++j) {
-            const int qq = q0 + j;
-            if (qq >= a.M || qq < pp) continue;
-            const double x = (double)v[c][j];
-            Cr[(size_t)pp * a.M + qq] = x;
-            if (qq > pp) Cr[(size_t)qq * a.M + pp] = x;
+            for (int i = 0; i < 32; ++i) {
+              double* R = rowp[i];
+              if (R) R[off] = (double)t[i];
+            }
+          }
+          // direct: block c holds p = p0 + 2 c + j / 16, q = q0 + j % 16
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            warp_transpose32(v[c], lane);
+            const size_t off = (size_t)(p0 + 2 * c + lane / 16) * a.M + q0 + lane % 16;
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              double* R = rowp[i];
+              if (R) R[off] = (double)v[c][i];
+            }
+          }
+        } else if (Cr) {
+          // tiles on the diagonal or the matrix edge: element by element from the thread's own row
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+#pragma unroll
+            for (int j = 0; j < 32; ++j) {
+              const int n = 32 * c + j;
+              const int pp = p0 + n / TC_QT, qq = q0 + n % TC_QT;
+              if (pp >= a.M || qq >= a.M || qq < pp) continue;
+              const double x = (double)v[c][j];
+              Cr[(size_t)pp * a.M + qq] = x;
+              if (qq > pp) Cr[(size_t)qq * a.M + pp] = x;
+            }
           }
         }
       }
@@ -302,7 +355,16 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
 }  // namespace
 
 // ---------------------------------------------------------------------------------- host side
-int vhs_tc_gamma_padded(int n_chol) { return (n_chol + TC_BK - 1) / TC_BK * TC_BK; }
+// (p-block, q-block) tiles of 8 x 16 elements that touch the upper triangle q >= p, row-major
+int vhs_tc_tile_list(int M, std::vector<int>* out) {
+  out->clear();
+  const int npb = (M + TC_PT - 1) / TC_PT, nqb = (M + TC_QT - 1) / TC_QT;
+  for (int pb = 0; pb < npb; ++pb)
+    for (int qb = 0; qb < nqb; ++qb)
+      if (qb * TC_QT + TC_QT - 1 >= pb * TC_PT) out->push_back((pb << 16) | qb);
+  return (int)out->size();
+}
+int vhs_tc_gamma_padded(int n_chol) { return (n_chol + TC_GPAD - 1) / TC_GPAD * TC_GPAD; }
 int vhs_tc_rows_padded(int rows) { return (rows + TC_M - 1) / TC_M * TC_M; }
 size_t vhs_tc_L_elems(int ntile_n, int n_chol) { return (size_t)ntile_n * 3 * TC_N * vhs_tc_gamma_padded(n_chol); }
 size_t vhs_tc_cf_elems(int rows, int n_chol) { return (size_t)3 * vhs_tc_rows_padded(rows) * vhs_tc_gamma_padded(n_chol); }
@@ -339,20 +401,20 @@ int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, in
     const uint64_t dims[3] = {(uint64_t)Gp, (uint64_t)Rp, 3};
     const uint64_t str[2] = {(uint64_t)Gp * 2, (uint64_t)Rp * Gp * 2};
     const uint32_t box[3] = {TC_BK, TC_M, 3};
-    if (make_tensor_map_bf16(&tmA, Ab, 3, dims, str, box) != 0) return -1;
+    if (make_tensor_map_bf16(&tmA, Ab, 3, dims, str, box, 64) != 0) return -1;
   }
   {
-    const uint64_t dims[4] = {(uint64_t)Gp, TC_N, 3, (uint64_t)ntile_n};
-    const uint64_t str[3] = {(uint64_t)Gp * 2, (uint64_t)TC_N * Gp * 2, (uint64_t)3 * TC_N * Gp * 2};
-    const uint32_t box[4] = {TC_BK, TC_N, 3, 1};
-    if (make_tensor_map_bf16(&tmB, Lb, 4, dims, str, box) != 0) return -1;
+    const uint64_t dims[4] = {(uint64_t)Gp, TC_N, (uint64_t)ntile_n, 3};
+    const uint64_t str[3] = {(uint64_t)Gp * 2, (uint64_t)TC_N * Gp * 2, (uint64_t)ntile_n * TC_N * Gp * 2};
+    const uint32_t box[4] = {TC_BK, TC_N, TC_NT, 3};
+    if (make_tensor_map_bf16(&tmB, Lb, 4, dims, str, box, 64) != 0) return -1;
   }
   TcArgs a;
   for (int r = 0; r < kMaxGroup; ++r) a.Cb[r] = r < nmember ? Cb[r] : nullptr;
   a.rpm = rows_per_member;
   a.tiles = tiles_dev; a.M = M; a.rows = rows; a.KT = Gp / TC_BK;
-  a.ntile_n = ntile_n; a.mtiles = Rp / TC_M;
-  const long nt = (long)a.ntile_n * a.mtiles;
+  a.ntile_n = ntile_n; a.npairs = (ntile_n + TC_NT - 1) / TC_NT; a.mtiles = Rp / TC_M;
+  const long nt = (long)a.npairs * a.mtiles;
   const int grid = nt < nsm ? (int)nt : nsm;
   vhs_tc_kernel<<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmB, a);
   return 2;
