@@ -10,18 +10,22 @@
 // tcgen05.mma.kind::f16 accumulates in FP32 in tensor memory, so the result carries the 24 significant bits
 // of an FP32 GEMM with FP32 accumulation.
 //
-// Data: only tiles touching the upper triangle (same 4 p x 32 q tiles and tile list as vhs_ws.cu) are kept,
-// K-MAJOR (gamma contiguous) so that both operands are the canonical SWIZZLE_128B K-major UMMA layout:
+// Data: only tiles touching the upper triangle are kept - this kernel's own tiles of 8 p x 16 q (128 elements,
+// 1200 = 150 x 8 = 75 x 16) -, K-MAJOR (gamma contiguous) and plane-major, so that two neighbouring tiles of one
+// plane form one 256-row canonical SWIZZLE_64B K-major UMMA operand in shared memory:
 //     Lb[3 planes][tile][128 n = (pl, qj)][Gp]   bf16, Gp = n_chol rounded up to 64, zero padded   (setup)
 //     Ab[3 planes][Rp rows = (w, plane)][Gp]     bf16, Rp = rows rounded up to 128                 (per step)
-// 6 bytes per kept element of L: 21.5 GB at M = 1200, Nchol = 4800 (dense FP64: 55.3 GB).
+// 6 bytes per kept element of L: 21.0 GB at M = 1200, Nchol = 4800 (dense FP64: 55.3 GB).
 //
-// Kernel: one persistent CTA per SM, 6 warps.  Warp 0: TMA producer (one box {32 g, 128 rows, 3 planes}
-// per operand and stage, mbarrier ring).  Warp 1: allocates tensor memory and issues tcgen05.mma
-// (M = 128, N = 128, K = 16; 4 k-steps x 6 plane pairs per stage); tcgen05.commit frees the stage and
-// publishes the accumulator.  Warps 2-5: epilogue - tcgen05.ld of the 128 x 128 FP32 accumulator (one row
-// per thread), conversion to double, store at [p][q] and mirrored at [q][p]; two accumulators in tensor
-// memory let the epilogue of one tile overlap the mainloop of the next.
+// Kernel: one persistent CTA per SM, 6 warps; a work unit is a PAIR of tiles x 128 rows.  Warp 0: TMA
+// producer - per stage of 32 gamma one box {32 g, 128 rows, 3 planes} of Ab and one box {32 g, 128 n, 2 tiles,
+// 3 planes} of Lb (72 KB), ring of 3 stages with mbarrier full/empty pairs.  Warp 1: allocates the 512 columns
+// of tensor memory and issues tcgen05.mma M = 128, N = 256, K = 16: 2 k-steps x 6 plane pairs per stage;
+// tcgen05.commit frees the stage and, after the last one, publishes the accumulator set.  Warps 2-5: epilogue -
+// tcgen05.ld (one accumulator row = one (walker, plane) row of A per thread), 32 x 32 warp transposes so that
+// a store instruction writes 128-byte runs of q (direct, [p][q]) or 64-byte runs of p (mirrored, [q][p]) of ONE
+// row; two accumulator sets let the epilogue of a unit overlap the mainloop of the next.  Measured and what
+// bounds it: profiles/r1v5_tc_c5.md.
 #include <cuda_bf16.h>
 
 #include <vector>
