@@ -63,6 +63,7 @@ struct afqmc_handle {
   void *Lb = nullptr, *Ab = nullptr;   // mixed precision: bf16 x 3 split tiles of L, split coefficients
   int* tc_tiles = nullptr;
   int tc_ntile = 0;
+  void *Abf = nullptr, *Tb0 = nullptr, *Tb1 = nullptr;   // mixed precision: split A and Taylor terms
   int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
@@ -314,7 +315,12 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
     h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
   }
   // a7: T_n = A T_{n-1} / n, Acc += T_n
-  {
+  if (h->Abf) {     // mixed precision: bf16 x 3 on tcgen05, FP64 running sum
+    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
+    const int r = run_taylor_tc(h->A, h->T0, h->Acc, h->Abf, h->Tb0, h->Tb1, nw, M, 2 * Nt, h->K, h->st);
+    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "taylor (mixed precision): tensor map encode failed");
+    h->launches += r;
+  } else {
     StageTimer tm(h, AFQMC_STAGE_TAYLOR);
     double *Tp = h->T0, *Tn = h->T1;
     for (int n = 1; n <= h->K; ++n) {
@@ -722,6 +728,13 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->Ab = dalloc(h, (vhs_tc_cf_elems(2 * mwg, nc) * 2 + 7) / 8);
     if (!h->Lb || !h->Ab) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Cholesky tensor)");
     h->launches += run_vhs_tc_split_L(h->L, h->Lb, h->tc_tiles, h->tc_ntile, M, nc, h->st);
+    if (taylor_tc_usable(2 * Nt)) {
+      const size_t ta = (taylor_tc_A_elems(mw, M) * 2 + 7) / 8, tt = (taylor_tc_T_elems(mw, M, 2 * Nt) * 2 + 7) / 8;
+      h->Abf = dalloc(h, ta); h->Tb0 = dalloc(h, tt); h->Tb1 = dalloc(h, tt);
+      if (!h->Abf || !h->Tb0 || !h->Tb1) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Taylor operands)");
+      cudaMemsetAsync(h->Tb0, 0, tt * 8, h->st);      // the zero padding of k and n is never written again
+      cudaMemsetAsync(h->Tb1, 0, tt * 8, h->st);
+    }
   }
 
   // ---- E_shift = trial energy ---------------------------------------------------------------

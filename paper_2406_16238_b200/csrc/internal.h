@@ -126,6 +126,13 @@ int run_vhs_tc_split_L(const double* L, void* Lb, const int* tiles_dev, int ntil
 int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, int nmember, int rows_per_member,
                const int* tiles_dev, int ntile_n, int M, int n_chol, cudaStream_t st);
 
+// taylor_tc.cu: Taylor propagation in the same emulated single precision (bf16 x 3 on tcgen05)
+size_t taylor_tc_A_elems(int nw, int M);
+size_t taylor_tc_T_elems(int nw, int M, int N2);
+bool taylor_tc_usable(int N2);
+int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, void* Tb0, void* Tb1, int nw, int M,
+                  int N2, int order, cudaStream_t st);
+
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
                    double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,

@@ -1,0 +1,292 @@
+// taylor_tc.cu - Taylor propagation T_n = A T_{n-1} / n, Acc += T_n (Eq. 12)
+// in emulated single precision on the tcgen05 tensor cores, the second half of the mixed-precision mode
+// ("single precision is used for propagations"; reading S24).  Same arithmetic as
+// vhs_tc.cu: operands split into three bfloat16 numbers, six plane pairs, FP32 accumulation in tensor memory.
+//
+// The complex product is ONE real GEMM per walker: with T stored as real columns (re, im interleaved, N2 = 2 Nt)
+//     A T = [Ar | Ai] * [T ; J T],   (J T)[k][2j] = -T[k][2j+1],  (J T)[k][2j+1] = T[k][2j],
+// i.e. K = 2 Kp (Kp = M rounded up to 32, zero padded), both operands K-major:
+//     Abf[w][3 planes][M rows][2 Kp]      bf16   [Ar row | Ai row]          (split_A_kernel, once per step)
+//     Tb [w][3 planes][Np rows][2 Kp]     bf16   [T^T row | (J T)^T row]    (Np = N2 rounded up to 16)
+// The epilogue of order n scales by 1/n, adds the term to the FP64 running sum Acc (walker layout) and writes
+// the split, transposed term straight into the Tb of order n + 1 (lanes = consecutive k: 64-byte runs).
+//
+// Kernel: persistent CTA per SM, work unit = (walker, 128 rows of A); warp 0 TMA producer (boxes {32 k, 128
+// rows, 3 planes} of Abf and {32 k, Np rows, 3 planes} of Tb), warp 1 tcgen05.mma M = 128, N = Np, K = 16
+// (2 k-steps x 6 plane pairs per stage), warps 2-5 epilogue; two accumulators in tensor memory.
+#include "internal.h"
+#include "tc.cuh"
+#include "tma.cuh"
+
+namespace afq {
+
+namespace {
+
+constexpr int TY_BK = 32;
+constexpr int TY_M = 128;
+constexpr int TY_APLANE = TY_M * TY_BK * 2;     // 8 KB
+constexpr int TY_AOPER = 3 * TY_APLANE;         // 24 KB
+constexpr int TY_ACC = 2;
+constexpr int TY_TMEM_COLS = 512;
+constexpr int TY_THREADS = 192;
+constexpr int TY_SMEM_CAP = 232448;
+
+// Abf[w][plane][m][reim * Kp + q] from A[w][reim][m][q]; grid (M, nw)
+__global__ void __launch_bounds__(256) split_A_kernel(const double* __restrict__ A, __nv_bfloat16* __restrict__ Abf,
+                                                      int M, int Kp) {
+  const int m = blockIdx.x, w = blockIdx.y;
+  const size_t MM = (size_t)M * M, plane = (size_t)M * 2 * Kp;
+  __nv_bfloat16* out = Abf + (size_t)w * 3 * plane + (size_t)m * 2 * Kp;
+  for (int idx = threadIdx.x; idx < 2 * Kp; idx += blockDim.x) {
+    const int reim = idx / Kp, q = idx % Kp;
+    const double x = q < M ? A[((size_t)w * 2 + reim) * MM + (size_t)m * M + q] : 0.0;
+    __nv_bfloat16 h, mm, l;
+    split3(x, h, mm, l);
+    out[idx] = h;
+    out[idx + plane] = mm;
+    out[idx + 2 * plane] = l;
+  }
+}
+
+// Tb[w][plane][n][k] = T[w][k][n], Tb[w][plane][n][Kp + k] = (J T)[k][n]; zero for n >= N2 or k >= M.
+// grid (Kp / 32, nw), 256 threads; T is [nw][M][N2] doubles (the walker layout)
+__global__ void __launch_bounds__(256) split_T_kernel(const double* __restrict__ T, __nv_bfloat16* __restrict__ Tb,
+                                                      int M, int N2, int Np, int Kp) {
+  extern __shared__ double tsm[];                 // [32][N2 + 1]
+  const int k0 = blockIdx.x * 32, w = blockIdx.y;
+  const int ld = N2 + 1;
+  for (int idx = threadIdx.x; idx < 32 * N2; idx += blockDim.x) {
+    const int kl = idx / N2, n = idx % N2;
+    tsm[kl * ld + n] = (k0 + kl < M) ? T[((size_t)w * M + k0 + kl) * N2 + n] : 0.0;
+  }
+  __syncthreads();
+  const size_t plane = (size_t)Np * 2 * Kp;
+  __nv_bfloat16* out = Tb + (size_t)w * 3 * plane;
+  for (int idx = threadIdx.x; idx < 32 * Np; idx += blockDim.x) {
+    const int n = idx / 32, kl = idx % 32;
+    double t = 0.0, jt = 0.0;
+    if (n < N2) {
+      t = tsm[kl * ld + n];
+      jt = (n & 1) ? tsm[kl * ld + n - 1] : -tsm[kl * ld + n + 1];
+    }
+    __nv_bfloat16 h, m, l;
+    split3(t, h, m, l);
+    size_t o = (size_t)n * 2 * Kp + k0 + kl;
+    out[o] = h; out[o + plane] = m; out[o + 2 * plane] = l;
+    split3(jt, h, m, l);
+    o += Kp;
+    out[o] = h; out[o + plane] = m; out[o + 2 * plane] = l;
+  }
+}
+
+struct TyArgs {
+  double* Acc;             // [nw][M][N2] running sum, FP64
+  __nv_bfloat16* Tnext;    // Tb of the next order, or nullptr for the last one
+  double alpha;            // 1 / n
+  int M, N2, Np, Kp, nw;
+  int KT, mtiles, stages;
+  uint32_t idesc;
+  int b_plane;             // bytes of one plane of the B operand in a stage (Np * 64)
+  int stage_bytes;
+};
+
+__global__ void __launch_bounds__(TY_THREADS, 1)
+taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB, const TyArgs a) {
+  extern __shared__ unsigned char smem_raw[];
+  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  const int S = a.stages;
+  uint64_t* full = reinterpret_cast<uint64_t*>(smem + (size_t)S * a.stage_bytes);
+  uint64_t* empty = full + S;
+  uint64_t* tfull = empty + S;
+  uint64_t* tempty = tfull + TY_ACC;
+  uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + TY_ACC);
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int nunits = a.nw * a.mtiles;            // work unit = (walker, 128 rows of A)
+
+  if (tid == 0) {
+    for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
+    for (int s = 0; s < TY_ACC; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
+    fence_barrier_init();
+  }
+  if (warp == 1) tmem_alloc<TY_TMEM_COLS>(tmem_slot);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ------------------------------------------------------------------ TMA producer
+    if (lane == 0) {
+      prefetch_tensormap(&tmA);
+      prefetch_tensormap(&tmB);
+      uint32_t it = 0;
+      for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
+        const int w = u / a.mtiles, mt = u % a.mtiles;
+        for (int kt = 0; kt < a.KT; ++kt, ++it) {
+          const int s = it % S;
+          mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
+          mbar_expect_tx(&full[s], (uint32_t)a.stage_bytes);
+          unsigned char* sa = smem + (size_t)s * a.stage_bytes;
+          tma_load_4d(sa, &tmA, &full[s], kt * TY_BK, mt * TY_M, 0, w);      // rows past M read as zeros
+          tma_load_4d(sa + TY_AOPER, &tmB, &full[s], kt * TY_BK, 0, 0, w);
+        }
+      }
+    }
+  } else if (warp == 1) {
+    // ------------------------------------------------------------------ MMA issuer (lane 0)
+    uint32_t it = 0, tc = 0;
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
+      const int acc = tc % TY_ACC;
+      mbar_wait(&tempty[acc], ((tc / TY_ACC) & 1) ^ 1);
+      tc_fence_after();
+      const uint32_t d = tmem_base + (uint32_t)acc * 256;
+      for (int kt = 0; kt < a.KT; ++kt, ++it) {
+        const int s = it % S;
+        mbar_wait(&full[s], (it / S) & 1);
+        tc_fence_after();
+        if (lane == 0) {
+          const uint32_t sa = smem_u32(smem + (size_t)s * a.stage_bytes), sb = sa + TY_AOPER;
+          const int pa[6] = {2, 0, 1, 1, 0, 0}, pb[6] = {0, 2, 1, 0, 1, 0};   // lh hl mm mh hm hh
+#pragma unroll
+          for (int k = 0; k < TY_BK / 16; ++k) {
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+              const uint64_t da = umma_desc(sa + pa[q] * TY_APLANE + k * 32);
+              const uint64_t db = umma_desc(sb + pb[q] * a.b_plane + k * 32);
+              umma_bf16(d, da, db, a.idesc, (kt | k | q) != 0 ? 1u : 0u);
+            }
+          }
+          umma_commit(&empty[s]);
+          if (kt == a.KT - 1) umma_commit(&tfull[acc]);
+        }
+        __syncwarp();
+      }
+    }
+  } else {
+    // ------------------------------------------------------------------ epilogue warps 2..5
+    // thread = one row m of the term: scale, add to the FP64 running sum, write the split transposed term
+    // (and J times it) into the B operand of the next order: lanes are consecutive k = m.
+    const int quarter = warp & 3;
+    const size_t bplane = (size_t)a.Np * 2 * a.Kp;
+    const float alpha = (float)a.alpha;
+    uint32_t tc = 0;
+    for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
+      const int acc = tc % TY_ACC;
+      const int w = u / a.mtiles, mt = u % a.mtiles;
+      const int m = mt * TY_M + quarter * 32 + lane;
+      mbar_wait(&tfull[acc], (tc / TY_ACC) & 1);
+      tc_fence_after();
+      const uint32_t taddr = tmem_base + (uint32_t)acc * 256 + ((uint32_t)(quarter * 32) << 16);
+      double* accrow = a.Acc + ((size_t)w * a.M + m) * a.N2;
+      __nv_bfloat16* tn = a.Tnext ? a.Tnext + (size_t)w * 3 * bplane + m : nullptr;
+      const int nchunks = (a.N2 + 31) / 32;
+#pragma unroll 1
+      for (int c = 0; c < nchunks; ++c) {
+        float v[32];
+        tmem_ld32(taddr + c * 32, v);
+        if (c == nchunks - 1) {
+          tc_fence_before();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty[acc]);
+        }
+        if (m >= a.M) continue;
+#pragma unroll
+        for (int j = 0; j < 32; ++j) {
+          const int n = 32 * c + j;
+          if (n >= a.N2) continue;
+          const float t = v[j] * alpha;
+          accrow[n] += (double)t;
+          if (tn) {
+            // an FP32 number is exactly three bfloat16 numbers
+            const __nv_bfloat16 h = __float2bfloat16_rn(t);
+            const float r1 = t - __bfloat162float(h);
+            const __nv_bfloat16 mm = __float2bfloat16_rn(r1);
+            const __nv_bfloat16 l = __float2bfloat16_rn(r1 - __bfloat162float(mm));
+            __nv_bfloat16* o = tn + (size_t)n * 2 * a.Kp;
+            o[0] = h; o[bplane] = mm; o[2 * bplane] = l;
+            // (J T)[k][n ^ 1] = (n odd ? -t : +t)
+            __nv_bfloat16* oj = tn + (size_t)(n ^ 1) * 2 * a.Kp + a.Kp;
+            if (n & 1) { oj[0] = __hneg(h); oj[bplane] = __hneg(mm); oj[2 * bplane] = __hneg(l); }
+            else { oj[0] = h; oj[bplane] = mm; oj[2 * bplane] = l; }
+          }
+        }
+      }
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) {
+    tc_fence_after();
+    tmem_dealloc<TY_TMEM_COLS>(tmem_base);
+  }
+}
+
+int round_up(int v, int m) { return (v + m - 1) / m * m; }
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------- host side
+size_t taylor_tc_A_elems(int nw, int M) { return (size_t)nw * 3 * M * 2 * round_up(M, TY_BK); }
+size_t taylor_tc_T_elems(int nw, int M, int N2) { return (size_t)nw * 3 * round_up(N2, 16) * 2 * round_up(M, TY_BK); }
+bool taylor_tc_usable(int N2) { return N2 % 2 == 0 && round_up(N2, 16) <= 256; }
+
+// Acc (holding T_0 on entry) += sum_{n=1..order} A^n T_0 / n!, A planar [nw][2][M][M], T0 / Acc [nw][M][N2].
+// Abf, Tb0, Tb1 are scratch of taylor_tc_A_elems / taylor_tc_T_elems bf16 each.  Returns launches or -1.
+int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, void* Tb0, void* Tb1, int nw, int M,
+                  int N2, int order, cudaStream_t st) {
+  if (!taylor_tc_usable(N2)) return -1;
+  const int Kp = round_up(M, TY_BK), Np = round_up(N2, 16);
+  const int b_plane = Np * TY_BK * 2, stage = TY_AOPER + 3 * b_plane;
+  int S = (TY_SMEM_CAP - 1024 - 256) / stage;
+  if (S > 8) S = 8;
+  if (S < 2) return -1;
+  const size_t smem = (size_t)S * stage + 1024 + 256;
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(taylor_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TY_SMEM_CAP);
+    cudaFuncSetAttribute(split_T_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 257 * 8);
+    attr = true;
+  }
+  static int nsm = 0;
+  if (!nsm) {
+    int dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
+    if (nsm <= 0) nsm = 148;
+  }
+  int launches = 0;
+  split_A_kernel<<<dim3(M, nw), 256, 0, st>>>(A, (__nv_bfloat16*)Abf, M, Kp);
+  split_T_kernel<<<dim3(Kp / 32, nw), 256, (size_t)32 * (N2 + 1) * 8, st>>>(T0, (__nv_bfloat16*)Tb0, M, N2, Np, Kp);
+  launches += 2;
+  TensorMap tmA, tmB[2];
+  {
+    const uint64_t dims[4] = {(uint64_t)2 * Kp, (uint64_t)M, 3, (uint64_t)nw};
+    const uint64_t str[3] = {(uint64_t)2 * Kp * 2, (uint64_t)M * 2 * Kp * 2, (uint64_t)3 * M * 2 * Kp * 2};
+    const uint32_t box[4] = {TY_BK, TY_M, 3, 1};
+    if (make_tensor_map_bf16(&tmA, Abf, 4, dims, str, box, 64) != 0) return -1;
+  }
+  void* tb[2] = {Tb0, Tb1};
+  for (int i = 0; i < 2; ++i) {
+    const uint64_t dims[4] = {(uint64_t)2 * Kp, (uint64_t)Np, 3, (uint64_t)nw};
+    const uint64_t str[3] = {(uint64_t)2 * Kp * 2, (uint64_t)Np * 2 * Kp * 2, (uint64_t)3 * Np * 2 * Kp * 2};
+    const uint32_t box[4] = {TY_BK, (uint32_t)Np, 3, 1};
+    if (make_tensor_map_bf16(&tmB[i], tb[i], 4, dims, str, box, 64) != 0) return -1;
+  }
+  TyArgs a;
+  a.Acc = Acc; a.M = M; a.N2 = N2; a.Np = Np; a.Kp = Kp; a.nw = nw;
+  a.KT = 2 * Kp / TY_BK; a.mtiles = (M + TY_M - 1) / TY_M; a.stages = S;
+  a.idesc = umma_idesc_bf16(TY_M, Np); a.b_plane = b_plane; a.stage_bytes = stage;
+  const long nu = (long)nw * a.mtiles;
+  const int grid = nu < nsm ? (int)nu : nsm;
+  for (int n = 1; n <= order; ++n) {
+    const int cur = (n - 1) & 1;
+    a.alpha = 1.0 / n;
+    a.Tnext = n < order ? (__nv_bfloat16*)tb[cur ^ 1] : nullptr;
+    taylor_tc_kernel<<<grid, TY_THREADS, smem, st>>>(tmA, tmB[cur], a);
+    ++launches;
+  }
+  return launches;
+}
+
+}  // namespace afq

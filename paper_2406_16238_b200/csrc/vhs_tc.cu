@@ -32,6 +32,7 @@
 
 #include "internal.h"
 #include "tma.cuh"
+#include "tc.cuh"
 
 namespace afq {
 
@@ -49,16 +50,9 @@ constexpr int TC_STAGES = 3;
 constexpr int TC_ACC = 2;                       // accumulator sets in tensor memory (TC_NT x 128 columns each)
 constexpr int TC_TMEM_COLS = 512;
 constexpr int TC_THREADS = 192;
+// instruction descriptor: M = 128, N = 256 (both tiles of a pair)
+constexpr uint32_t kIdesc = umma_idesc_bf16(TC_M, TC_NT * TC_N);
 constexpr size_t TC_SMEM = (size_t)TC_STAGES * TC_STAGE + 1024 + 256 + 1024;   // + alignment, barriers, row table
-
-// ------------------------------------------------------------------ bf16 x 3 splitting
-__device__ __forceinline__ void split3(double x, __nv_bfloat16& h, __nv_bfloat16& m, __nv_bfloat16& l) {
-  h = __float2bfloat16_rn((float)x);
-  const double r1 = x - (double)__bfloat162float(h);
-  m = __float2bfloat16_rn((float)r1);
-  const double r2 = r1 - (double)__bfloat162float(m);
-  l = __float2bfloat16_rn((float)r2);
-}
 
 // Lb[plane][t][n][g] from the dense L[g][p][q]; grid (ntile, Gp / 64), 256 threads
 __global__ void __launch_bounds__(256) split_L_kernel(const double* __restrict__ L, __nv_bfloat16* __restrict__ Lb,
@@ -105,80 +99,6 @@ __global__ void __launch_bounds__(256) split_cf_kernel(const double* __restrict_
   }
 }
 
-// ------------------------------------------------------------------ tcgen05 building blocks
-__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;\n" ::: "memory"); }
-__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;\n" ::: "memory"); }
-
-// whole warp: allocate TC_TMEM_COLS columns, base address written to *slot (shared memory)
-__device__ __forceinline__ void tmem_alloc(uint32_t* slot) {
-  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;\n" ::"r"(smem_u32(slot)),
-               "n"(TC_TMEM_COLS)
-               : "memory");
-  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;\n" ::: "memory");
-}
-__device__ __forceinline__ void tmem_dealloc(uint32_t base) {
-  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;\n" ::"r"(base), "n"(TC_TMEM_COLS) : "memory");
-}
-
-// shared-memory matrix descriptor: K-major, SWIZZLE_64B (rows of 64 bytes), 8-row groups 512 bytes apart
-__device__ __forceinline__ uint64_t umma_desc(uint32_t saddr) {
-  uint64_t d = (uint64_t)((saddr & 0x3FFFF) >> 4);
-  d |= (uint64_t)1 << 16;                 // leading byte offset (unused for swizzled K-major)
-  d |= (uint64_t)(512 >> 4) << 32;        // stride byte offset
-  d |= (uint64_t)1 << 46;                 // descriptor version (Blackwell)
-  d |= (uint64_t)4 << 61;                 // SWIZZLE_64B
-  return d;
-}
-// instruction descriptor: D = F32, A = B = BF16, both K-major, M = 128, N = 256 (both tiles of a pair)
-constexpr uint32_t kIdesc = (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)((TC_NT * TC_N) >> 3) << 17) |
-                            ((uint32_t)(TC_M >> 4) << 24);
-
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t accumulate) {
-  asm volatile(
-      "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\n"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n}\n" ::"r"(d_tmem),
-      "l"(adesc), "l"(bdesc), "r"(kIdesc), "r"(accumulate)
-      : "memory");
-}
-// arrive on an mbarrier when every tcgen05.mma issued so far by this thread has completed
-__device__ __forceinline__ void umma_commit(uint64_t* bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n" ::"r"(smem_u32(bar))
-               : "memory");
-}
-// this thread's lane of tensor memory, 32 consecutive FP32 columns
-__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
-  uint32_t r[32];
-  asm volatile(
-      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
-      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
-      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];\n"
-      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
-        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]), "=r"(r[16]),
-        "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]), "=r"(r[24]),
-        "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
-      : "r"(taddr)
-      : "memory");
-  asm volatile("tcgen05.wait::ld.sync.aligned;\n" ::: "memory");
-#pragma unroll
-  for (int i = 0; i < 32; ++i) v[i] = __uint_as_float(r[i]);
-}
-
-// 32 x 32 transpose across a warp: afterwards x[i] of lane l is what x[l] of lane i was
-__device__ __forceinline__ void warp_transpose32(float (&x)[32], int lane) {
-#pragma unroll
-  for (int s = 16; s >= 1; s >>= 1) {
-    const bool up = (lane & s) != 0;
-#pragma unroll
-    for (int i = 0; i < 32; ++i) {
-      if ((i & s) == 0) {
-        const float send = up ? x[i] : x[i + s];
-        const float recv = __shfl_xor_sync(0xffffffffu, send, s);
-        if (up) x[i] = recv; else x[i + s] = recv;
-      }
-    }
-  }
-}
-
 struct TcArgs {
   double* Cb[kMaxGroup];   // output base per block of rpm rows (as vhs_ws.cu)
   int rpm;
@@ -204,7 +124,7 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
     for (int s = 0; s < TC_ACC; ++s) { mbar_init(&tfull[s], 1); mbar_init(&tempty[s], 4); }
     fence_barrier_init();
   }
-  if (warp == 1) tmem_alloc(tmem_slot);
+  if (warp == 1) tmem_alloc<TC_TMEM_COLS>(tmem_slot);
   tc_fence_before();
   __syncthreads();
   tc_fence_after();
@@ -251,7 +171,7 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
             for (int q = 0; q < 6; ++q) {
               const uint64_t da = umma_desc(sa + pa[q] * TC_PLANE + k * 32);
               const uint64_t db = umma_desc(sb + pb[q] * (TC_NT * TC_PLANE) + k * 32);   // 256 rows: tile 0, tile 1
-              umma_bf16(d, da, db, (kt | k | q) != 0 ? 1u : 0u);
+              umma_bf16(d, da, db, kIdesc, (kt | k | q) != 0 ? 1u : 0u);
             }
           }
           umma_commit(&empty[s]);                       // stage free when these MMAs have read it
@@ -352,7 +272,7 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
   __syncthreads();
   if (warp == 1) {
     tc_fence_after();
-    tmem_dealloc(tmem_base);
+    tmem_dealloc<TC_TMEM_COLS>(tmem_base);
   }
 }
 
