@@ -13,7 +13,8 @@
 //
 // Kernel: persistent CTA per SM, work unit = (walker, 128 rows of A); warp 0 TMA producer (boxes {32 k, 128
 // rows, 3 planes} of Abf and {32 k, Np rows, 3 planes} of Tb), warp 1 tcgen05.mma M = 128, N = Np, K = 16
-// (2 k-steps x 6 plane pairs per stage), warps 2-5 epilogue; two accumulators in tensor memory.
+// (2 k-steps x 6 plane pairs per stage; hh into its own accumulator), warps 2-5 epilogue; two accumulator
+// sets in tensor memory when Np <= 128.
 #include "internal.h"
 #include "tc.cuh"
 #include "tma.cuh"
@@ -86,6 +87,7 @@ struct TyArgs {
   int M, N2, Np, Kp, nw;
   int KT, mtiles, stages;
   uint32_t idesc;
+  int nacc, d2off;         // accumulator sets in tensor memory (2 if Np <= 128), column offset of D2 in a set
   int b_plane;             // bytes of one plane of the B operand in a stage (Np * 64)
   int stage_bytes;
 };
@@ -136,10 +138,11 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
     // ------------------------------------------------------------------ MMA issuer (lane 0)
     uint32_t it = 0, tc = 0;
     for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
-      const int acc = tc % TY_ACC;
-      mbar_wait(&tempty[acc], ((tc / TY_ACC) & 1) ^ 1);
+      const int acc = tc % a.nacc;
+      mbar_wait(&tempty[acc], ((tc / a.nacc) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t d = tmem_base + (uint32_t)acc * 256;
+      // D1: the hh plane pair; D2: the five small ones (truncating accumulation, see vhs_tc.cu)
+      const uint32_t d1 = tmem_base + (uint32_t)acc * 256, d2 = d1 + a.d2off;
       for (int kt = 0; kt < a.KT; ++kt, ++it) {
         const int s = it % S;
         mbar_wait(&full[s], (it / S) & 1);
@@ -153,7 +156,8 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
             for (int q = 0; q < 6; ++q) {
               const uint64_t da = umma_desc(sa + pa[q] * TY_APLANE + k * 32);
               const uint64_t db = umma_desc(sb + pb[q] * a.b_plane + k * 32);
-              umma_bf16(d, da, db, a.idesc, (kt | k | q) != 0 ? 1u : 0u);
+              if (q == 5) umma_bf16(d1, da, db, a.idesc, (kt | k) != 0 ? 1u : 0u);
+              else umma_bf16(d2, da, db, a.idesc, (kt | k | q) != 0 ? 1u : 0u);
             }
           }
           umma_commit(&empty[s]);
@@ -171,10 +175,10 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
     const float alpha = (float)a.alpha;
     uint32_t tc = 0;
     for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
-      const int acc = tc % TY_ACC;
+      const int acc = tc % a.nacc;
       const int w = u / a.mtiles, mt = u % a.mtiles;
       const int m = mt * TY_M + quarter * 32 + lane;
-      mbar_wait(&tfull[acc], (tc / TY_ACC) & 1);
+      mbar_wait(&tfull[acc], (tc / a.nacc) & 1);
       tc_fence_after();
       const uint32_t taddr = tmem_base + (uint32_t)acc * 256 + ((uint32_t)(quarter * 32) << 16);
       double* accrow = a.Acc + ((size_t)w * a.M + m) * a.N2;
@@ -182,8 +186,11 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
       const int nchunks = (a.N2 + 31) / 32;
 #pragma unroll 1
       for (int c = 0; c < nchunks; ++c) {
-        float v[32];
+        float v[32], v2[32];
         tmem_ld32(taddr + c * 32, v);
+        tmem_ld32(taddr + a.d2off + c * 32, v2);
+#pragma unroll
+        for (int j = 0; j < 32; ++j) v[j] += v2[j];
         if (c == nchunks - 1) {
           tc_fence_before();
           __syncwarp();
@@ -277,6 +284,7 @@ int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, voi
   a.Acc = Acc; a.M = M; a.N2 = N2; a.Np = Np; a.Kp = Kp; a.nw = nw;
   a.KT = 2 * Kp / TY_BK; a.mtiles = (M + TY_M - 1) / TY_M; a.stages = S;
   a.idesc = umma_idesc_bf16(TY_M, Np); a.b_plane = b_plane; a.stage_bytes = stage;
+  a.nacc = Np <= 128 ? 2 : 1; a.d2off = Np <= 128 ? 128 : 256;
   const long nu = (long)nw * a.mtiles;
   const int grid = nu < nsm ? (int)nu : nsm;
   for (int n = 1; n <= order; ++n) {

@@ -24,7 +24,9 @@
 // tcgen05.commit frees the stage and, after the last one, publishes the accumulator set.  Warps 2-5: epilogue -
 // tcgen05.ld (one accumulator row = one (walker, plane) row of A per thread), 32 x 32 warp transposes so that
 // a store instruction writes 128-byte runs of q (direct, [p][q]) or 64-byte runs of p (mirrored, [q][p]) of ONE
-// row; two accumulator sets let the epilogue of a unit overlap the mainloop of the next.  Measured and what
+// row.  The hh plane pair has its own accumulator (the tensor core truncates when it adds: see the MMA
+// loop), so the 512 columns hold ONE set of two N = 256 accumulators and the MMA warp waits while the
+// epilogue drains it (about 2 % of a unit; TMA keeps filling the ring meanwhile).  Measured and what
 // bounds it: profiles/r1v5_tc_c5.md.
 #include <cuda_bf16.h>
 
@@ -47,7 +49,8 @@ constexpr int TC_PLANE = TC_M * TC_BK * 2;      // bytes of one plane of one 128
 constexpr int TC_OPER = 3 * TC_PLANE;           // 24 KB
 constexpr int TC_STAGE = (1 + TC_NT) * TC_OPER; // 72 KB: A, B tile 0, B tile 1
 constexpr int TC_STAGES = 3;
-constexpr int TC_ACC = 2;                       // accumulator sets in tensor memory (TC_NT x 128 columns each)
+constexpr int TC_ACC = 1;                       // accumulator sets in tensor memory; a set = TWO accumulators of
+                                                // TC_NT x 128 columns: D1 for the hh plane pair, D2 for the other five
 constexpr int TC_TMEM_COLS = 512;
 constexpr int TC_THREADS = 192;
 // instruction descriptor: M = 128, N = 256 (both tiles of a pair)
@@ -156,7 +159,10 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       const int acc = tc % TC_ACC;
       mbar_wait(&tempty[acc], ((tc / TC_ACC) & 1) ^ 1);
       tc_fence_after();
-      const uint32_t d = tmem_base + (uint32_t)acc * (TC_NT * TC_N);
+      // The tensor core adds into its FP32 accumulator with truncation.  Adding the five small plane pairs
+      // (<= 2^-8 of hh) to the same accumulator would cost a truncation of the LARGE sum each time; kept apart,
+      // the large sum sees one update per 16 gamma and the bias drops six-fold.  The epilogue adds D1 + D2.
+      const uint32_t d1 = tmem_base + (uint32_t)acc * (2 * TC_NT * TC_N), d2 = d1 + TC_NT * TC_N;
       for (int kt = 0; kt < a.KT; ++kt, ++it) {
         const int s = it % TC_STAGES;
         mbar_wait(&full[s], (it / TC_STAGES) & 1);
@@ -171,7 +177,8 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
             for (int q = 0; q < 6; ++q) {
               const uint64_t da = umma_desc(sa + pa[q] * TC_PLANE + k * 32);
               const uint64_t db = umma_desc(sb + pb[q] * (TC_NT * TC_PLANE) + k * 32);   // 256 rows: tile 0, tile 1
-              umma_bf16(d, da, db, kIdesc, (kt | k | q) != 0 ? 1u : 0u);
+              if (q == 5) umma_bf16(d1, da, db, kIdesc, (kt | k) != 0 ? 1u : 0u);
+              else umma_bf16(d2, da, db, kIdesc, (kt | k | q) != 0 ? 1u : 0u);
             }
           }
           umma_commit(&empty[s]);                       // stage free when these MMAs have read it
@@ -207,10 +214,16 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
 #pragma unroll 1
       for (int nt = 0; nt < TC_NT; ++nt) {
         const int tl = pr * TC_NT + nt;
-        const uint32_t taddr = tmem_base + (uint32_t)(acc * TC_NT + nt) * TC_N + ((uint32_t)(quarter * 32) << 16);
+        const uint32_t taddr = tmem_base + (uint32_t)(acc * 2 * TC_NT + nt) * TC_N + ((uint32_t)(quarter * 32) << 16);
         float v[4][32];                           // v[c][j]: n = 32 c + j, p = p0 + n / 16, q = q0 + n % 16
 #pragma unroll
-        for (int c = 0; c < 4; ++c) tmem_ld32(taddr + c * 32, v[c]);
+        for (int c = 0; c < 4; ++c) {
+          float v2[32];
+          tmem_ld32(taddr + c * 32, v[c]);
+          tmem_ld32(taddr + TC_NT * TC_N + c * 32, v2);
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[c][j] += v2[j];
+        }
         if (nt == TC_NT - 1) {
           tc_fence_before();
           __syncwarp();
