@@ -25,7 +25,9 @@
  *
  * Errors: every int32_t entry point returns AFQMC_OK or a negative code; nothing throws or
  * aborts across the ABI.  afqmc_last_error() gives a message for the last failure on that
- * handle (or for a failed afqmc_create when passed NULL).  A walker whose overlap with the
+* handle (or for a failed afqmc_create when passed NULL).  A handle lives on the CUDA device that holds
+ * L_chol; every entry point switches to that device for the duration of the call, so handles on
+ * different devices can be driven from one host thread.  A walker whose overlap with the
  * trial is zero or non-finite is NOT an error: its weight becomes exactly 0 (Eq. 15,
  * reading S10).  One handle per host thread; no global mutable state besides the create
  * error string.

@@ -17,6 +17,7 @@ struct afqmc_handle {
   int M = 0, Nt = 0, nblk = 1, off[2] = {0, 0}, ns[2] = {0, 0};
   int n_chol = 0, maxw = 0, K = 6, rhf = 1;
   double sf = 2.0;
+  int dev = 0;                 // CUDA device of the handle (that of L_chol); every entry point switches to it
   cudaStream_t st = nullptr;
   bool own_stream = false;
   const double* L = nullptr;
@@ -81,6 +82,23 @@ struct afqmc_handle {
 static std::string g_create_err;
 
 namespace {
+
+// switch to the handle's device for the duration of an API call
+struct DevGuard {
+  int prev = -1;
+  bool sw = false;
+  explicit DevGuard(int dev) {
+    cudaGetDevice(&prev);
+    if (prev != dev) { cudaSetDevice(dev); sw = true; }
+  }
+  ~DevGuard() { if (sw) cudaSetDevice(prev); }
+};
+
+int device_of(const void* p) {
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, p) != cudaSuccess) { cudaGetLastError(); return -1; }
+  return (at.type == cudaMemoryTypeDevice || at.type == cudaMemoryTypeManaged) ? at.device : -1;
+}
 
 bool is_device_ptr(const void* p) {
   cudaPointerAttributes at;
@@ -476,6 +494,7 @@ const char* afqmc_last_error(const afqmc_handle* h) { return h ? h->err.c_str() 
 
 void afqmc_destroy(afqmc_handle* h) {
   if (!h) return;
+  DevGuard dg_(h->dev);
   cudaStreamSynchronize(h->st);
   for (void* p : h->allocs)
     if (p) cudaFree(p);
@@ -508,9 +527,12 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (G > 1 && (p->M % 2 != 0 || p->n_chol % 2 != 0))
     return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "a distributed Hamiltonian needs even M and an even local n_chol (TMA strides)");
 
+  const int ldev = device_of(L_chol);
+  DevGuard dg_(ldev >= 0 ? ldev : 0);
   afqmc_handle* h = new (std::nothrow) afqmc_handle();
   if (!h) return fail(nullptr, AFQMC_ERR_ALLOC, "host allocation failed");
   h->p = *p;
+  h->dev = ldev >= 0 ? ldev : 0;
   h->M = p->M; h->n_chol = p->n_chol; h->maxw = p->max_walkers;
   h->G = G; h->rank = p->group_rank; h->mwg = G * p->max_walkers;
   h->shard_ready = G == 1;
@@ -764,6 +786,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
 
 int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
@@ -790,6 +813,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
 
 int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, int32_t nw) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !E_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
@@ -813,6 +837,7 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
 int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi, int32_t nw,
                                  int32_t* map_out) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !xi) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
@@ -839,6 +864,7 @@ int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights
 
 int32_t afqmc_estimators(afqmc_handle* h, const double* weights, const void* E, double* est_out, int32_t nw) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (!weights || !E || !est_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
   const bool hostWt = !is_device_ptr(weights), hostE = !is_device_ptr(E), hostO = !is_device_ptr(est_out);
@@ -858,6 +884,7 @@ int32_t afqmc_estimators(afqmc_handle* h, const double* weights, const void* E, 
 int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, const double* xi,
                         double dt, int32_t nw, int32_t n_steps, int32_t pop_every, void* E_out, double* est_out) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (h->G > 1) return fail(h, AFQMC_ERR_UNSUPPORTED, "distributed-Hamiltonian handle: use the afqmc_shard_* phases");
   if (!walkers || !weights || !aux_fields) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
@@ -914,6 +941,7 @@ int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const d
 
 int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (!ovlp_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
   if (h->last_nw <= 0) return fail(h, AFQMC_ERR_INVALID, "no step has been taken");
   const bool host = !is_device_ptr(ovlp_out);
@@ -924,6 +952,7 @@ int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out) {
 
 int32_t afqmc_get_constants(afqmc_handle* h, double* out3) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (!out3) return fail(h, AFQMC_ERR_INVALID, "null argument");
   out3[0] = h->E_const; out3[1] = h->e_shift; out3[2] = h->e_trial;
   return AFQMC_OK;
@@ -931,6 +960,7 @@ int32_t afqmc_get_constants(afqmc_handle* h, double* out3) {
 
 int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   const double* src = nullptr;
   int64_t n = 0;
   const long MM = (long)h->M * h->M;
@@ -953,18 +983,21 @@ int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
 
 int64_t afqmc_set_block_graph(afqmc_handle* h, int32_t on) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (on >= 0) h->graph_on = on != 0;
   return h->graph_replays;
 }
 
 int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   h->prof = on != 0;
   return AFQMC_OK;
 }
 
 int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   if (!ms_out) return fail(h, AFQMC_ERR_INVALID, "null argument");
   cudaError_t e = cudaStreamSynchronize(h->st);
   if (e != cudaSuccess) return fail(h, AFQMC_ERR_CUDA, std::string("get_stage_times: ") + cudaGetErrorString(e));
@@ -993,6 +1026,7 @@ int64_t afqmc_launch_count(const afqmc_handle* h) { return h ? h->launches : -1;
 // ------------------------------------------------------------------ distributed Hamiltonian
 #define SHARD_CHECK(h, need_ready)                                                                     \
   if (!h) return AFQMC_ERR_INVALID;                                                                    \
+  DevGuard dg_(h->dev);                                                                                \
   if (h->G <= 1) return fail(h, AFQMC_ERR_INVALID, "not a distributed-Hamiltonian handle (group_size <= 1)"); \
   if (need_ready && !h->shard_ready) return fail(h, AFQMC_ERR_INVALID, "afqmc_shard_setup_finish has not been called"); \
   if (need_ready && !h->peers_set) return fail(h, AFQMC_ERR_INVALID, "afqmc_shard_set_peers has not been called");
@@ -1089,6 +1123,20 @@ int32_t afqmc_shard_set_peers(afqmc_handle* h, const uint64_t* addrs) {
       if (!addrs[(size_t)r * 4 + k] || (addrs[(size_t)r * 4 + k] & 15)) return fail(h, AFQMC_ERR_INVALID, "null or misaligned peer buffer");
       h->peer[k][r] = (double*)(uintptr_t)addrs[(size_t)r * 4 + k];
     }
+  // members on other devices of this process: the kernels store into their buffers, so peer access must
+  // be on (buffers imported through CUDA IPC were opened with cudaIpcMemLazyEnablePeerAccess already)
+  for (int r = 0; r < h->G; ++r) {
+    const int pd = device_of(h->peer[1][r]);
+    if (pd >= 0 && pd != h->dev) {
+      int can = 0;
+      cudaDeviceCanAccessPeer(&can, h->dev, pd);
+      if (!can) return fail(h, AFQMC_ERR_UNSUPPORTED, "no peer access between the devices of the group");
+      const cudaError_t e = cudaDeviceEnablePeerAccess(pd, 0);
+      if (e != cudaSuccess && e != cudaErrorPeerAccessAlreadyEnabled)
+        return fail(h, AFQMC_ERR_CUDA, std::string("cudaDeviceEnablePeerAccess: ") + cudaGetErrorString(e));
+      cudaGetLastError();
+    }
+  }
   h->peers_set = true;
   return AFQMC_OK;
 }
@@ -1184,6 +1232,7 @@ int32_t afqmc_shard_energy_finish(afqmc_handle* h, void* E_out, int32_t nw) {
 
 int32_t afqmc_sync(afqmc_handle* h) {
   if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
   cudaError_t e = cudaStreamSynchronize(h->st);
   if (e != cudaSuccess) return fail(h, AFQMC_ERR_CUDA, std::string("sync: ") + cudaGetErrorString(e));
   return check_cuda(h, "afqmc_sync");

@@ -166,10 +166,9 @@ template <int NP8, int GW, int SPLIT>
 int launch_ex(const ExArgs& a, cudaStream_t st) {
   using Cfg = ExCfg<NP8, GW, SPLIT>;
   auto kern = exchange_kernel<NP8, GW, SPLIT>;
-  static bool done = false;
-  if (!done) {
+  static uint64_t done = 0;
+  if (first_use_on_device(&done)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-    done = true;
   }
   dim3 grid(a.nw, (a.n_chol + Cfg::G - 1) / Cfg::G);
   kern<<<grid, kThreads, Cfg::SMEM, st>>>(a);

@@ -289,18 +289,11 @@ template <int WM, int WN, int MI, int NI>
 int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
   using Cfg = XwsCfg<WM, WN, MI, NI>;
   auto kern = exchange_ws_kernel<WM, WN, MI, NI>;
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
-    attr = true;
   }
-  static int nsm = 0;
-  if (!nsm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    if (nsm <= 0) nsm = 148;
-  }
+  const int nsm = sm_count_current();
   TensorMap tmA, tmB;
   {
     const uint64_t dims[3] = {(uint64_t)e.M, (uint64_t)e.Nt, (uint64_t)e.n_chol};

@@ -7,10 +7,9 @@ template <int BM, int BN, int WM, int WN, bool A_KM, bool B_NK, bool CPLX, int S
 static int launch_cfg(const GemmArgs& a, cudaStream_t st) {
   using Cfg = GemmCfg<BM, BN, WM, WN, A_KM, B_NK, CPLX, STAGES>;
   auto kern = gemm_dmma_kernel<BM, BN, WM, WN, A_KM, B_NK, CPLX, STAGES>;
-  static bool attr_done = false;
-  if (!attr_done) {
+  static uint64_t attr_done = 0;
+  if (first_use_on_device(&attr_done)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
-    attr_done = true;
   }
   dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch * a.splitK);
   kern<<<grid, kThreads, Cfg::SMEM, st>>>(a);

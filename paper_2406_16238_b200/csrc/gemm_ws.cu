@@ -20,16 +20,7 @@ namespace {
 constexpr int kProdT = 128;
 constexpr int kSmemCap = 232448;
 
-int sm_count() {
-  static int nsm = 0;
-  if (!nsm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    if (nsm <= 0) nsm = 148;
-  }
-  return nsm;
-}
+int sm_count() { return sm_count_current(); }
 
 // ------------------------------------------------------------------------------------ KN
 struct KnArgs {
@@ -197,10 +188,9 @@ template <int MI, int NI, bool CPLX>
 int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, cudaStream_t st) {
   using Cfg = KnCfg<MI, NI, CPLX>;
   auto kern = gemm_ws_kn_kernel<MI, NI, CPLX>;
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemCap);
-    attr = true;
   }
   int S = (kSmemCap - 1024 - 256) / Cfg::STAGE_BYTES;
   if (S > 8) S = 8;
@@ -414,10 +404,9 @@ int gemm_ws_nk_split(int M, int N, int K, int max_split) {
 int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double* C, long ldc, long sCsplit,
                    int M, int N, int K, int split, cudaStream_t st) {
   if (!(even(lda) && even(ldb) && al16(A) && al16(B))) return -1;
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(gemm_ws_nk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemCap);
-    attr = true;
   }
   TensorMap tmA, tmB;
   {

@@ -15,6 +15,37 @@ constexpr int kMaxOcc = 64;     // largest occupied block (columns per spin) sup
 constexpr int kMaxTaylor = 16;
 constexpr int kMaxGroup = 8;    // members of a distributed-Hamiltonian group
 
+// Per-device one-off work (cudaFuncSetAttribute is per device; handles may live on different devices of one
+// process): true the first time it is called with this mask on the current device.
+inline bool first_use_on_device(uint64_t* mask) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  const uint64_t b = 1ull << (dev & 63);
+  if (*mask & b) return false;
+  *mask |= b;
+  return true;
+}
+// largest dynamic shared-memory size requested so far on the current device; true if `bytes` exceeds it
+inline bool grow_on_device(size_t* cur /* [64] */, size_t bytes) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (bytes <= cur[dev & 63]) return false;
+  cur[dev & 63] = bytes;
+  return true;
+}
+// SM count of the current device (cached per device)
+inline int sm_count_current() {
+  static int n[64] = {0};
+  int dev = 0;
+  cudaGetDevice(&dev);
+  int& v = n[dev & 63];
+  if (!v) {
+    cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
+    if (v <= 0) v = 148;
+  }
+  return v;
+}
+
 enum GemmKind { GEMM_KN = 0, GEMM_NK = 1, GEMM_KMKN = 2, GEMM_CPLX_KN = 3 };
 
 // gemm.cu

@@ -419,10 +419,9 @@ int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st) {
   int nsmax = a.ns[0];
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = ot_smem(nsmax);
-  static size_t cur = 0;
-  if (sm > cur) {
+  static size_t cur[64] = {0};
+  if (grow_on_device(cur, sm)) {
     cudaFuncSetAttribute(overlap_theta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    cur = sm;
   }
   overlap_theta_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);
   return 1;
@@ -442,10 +441,9 @@ int run_cholqr_pass(const QRArgs& a, int nw, cudaStream_t st) {
   int nsmax = a.ns[0];
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = (size_t)2 * nsmax * nsmax * 16 + (size_t)kRows * (nsmax | 1) * 16 + 64;
-  static size_t cur = 0;
-  if (sm > cur) {
+  static size_t cur[64] = {0};
+  if (grow_on_device(cur, sm)) {
     cudaFuncSetAttribute(cholqr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
-    cur = sm;
   }
   cholqr_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);
   return 1;

@@ -249,19 +249,12 @@ int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, voi
   if (S > 8) S = 8;
   if (S < 2) return -1;
   const size_t smem = (size_t)S * stage + 1024 + 256;
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(taylor_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TY_SMEM_CAP);
     cudaFuncSetAttribute(split_T_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 257 * 8);
-    attr = true;
   }
-  static int nsm = 0;
-  if (!nsm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    if (nsm <= 0) nsm = 148;
-  }
+  const int nsm = sm_count_current();
   int launches = 0;
   split_A_kernel<<<dim3(M, nw), 256, 0, st>>>(A, (__nv_bfloat16*)Abf, M, Kp);
   split_T_kernel<<<dim3(Kp / 32, nw), 256, (size_t)32 * (N2 + 1) * 8, st>>>(T0, (__nv_bfloat16*)Tb0, M, N2, Np, Kp);

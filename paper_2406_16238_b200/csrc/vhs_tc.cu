@@ -320,18 +320,11 @@ int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, in
   if (nmember < 1 || nmember > kMaxGroup || rows_per_member < 1) return -1;
   const int rows = nmember * rows_per_member;
   const int Gp = vhs_tc_gamma_padded(n_chol), Rp = vhs_tc_rows_padded(rows);
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(vhs_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
-    attr = true;
   }
-  static int nsm = 0;
-  if (!nsm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    if (nsm <= 0) nsm = 148;
-  }
+  const int nsm = sm_count_current();
   split_cf_kernel<<<dim3((Gp + 255) / 256, Rp), 256, 0, st>>>(Cf, (__nv_bfloat16*)Ab, rows, n_chol, Rp, Gp);
   TensorMap tmA, tmB;
   {

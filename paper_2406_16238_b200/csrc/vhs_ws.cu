@@ -233,19 +233,12 @@ int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int
                        const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st) {
   if (nmember < 1 || nmember > kMaxGroup || rows_per_member < 1) return -1;
   const int rows = nmember * rows_per_member;
-  static bool attr = false;
-  if (!attr) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
     cudaFuncSetAttribute(vhs_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
     cudaFuncSetAttribute(vhs_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
-    attr = true;
   }
-  static int nsm = 0;
-  if (!nsm) {
-    int dev = 0;
-    cudaGetDevice(&dev);
-    cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-    if (nsm <= 0) nsm = 148;
-  }
+  const int nsm = sm_count_current();
   TensorMap tmA, tmB;
   {
     const uint64_t dims[2] = {(uint64_t)n_chol, (uint64_t)rows};
