@@ -56,6 +56,8 @@ struct afqmc_handle {
   double *hmod_part = nullptr, *setup_buf = nullptr, *e1zero = nullptr, *Etmp = nullptr, *scal_sum = nullptr;
   double Ec_part = 0.0, e2trial_part = 0.0, e1b_trial = 0.0;
   double* peer[4][kMaxGroup] = {};              // [theta, a, scal, e][member]
+  double *Obuf = nullptr, *Aop = nullptr;       // overlap / inverse operands of the DMMA overlap-Theta route
+  bool ot_gemm = false;
   int fb_split = 1;
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   bool ws_vhs = false;
@@ -213,6 +215,7 @@ OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, in
   a.M = h->M; a.Nt = h->Nt; a.nblk = h->nblk;
   for (int b = 0; b < 2; ++b) { a.off[b] = h->off[b]; a.ns[b] = h->ns[b]; }
   a.want_theta = want_theta; a.want_e1 = want_e1;
+  a.trialT = h->ot_gemm ? h->trialT : nullptr; a.Obuf = h->Obuf; a.Aop = h->Aop;
   return a;
 }
 
@@ -693,6 +696,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mwg * 2);
   }
   h->Xe = dalloc(h, (size_t)nc * mwg * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
+  h->Obuf = dalloc(h, (size_t)mw * Nt * 2 * Nt); h->Aop = dalloc(h, (size_t)mw * 4 * Nt * Nt);
+  if (!h->Obuf || !h->Aop) return bail(AFQMC_ERR_ALLOC, "device allocation failed (overlap operands)");
+  h->ot_gemm = h->ws && getenv("AFQMC_OT_KERNEL") == nullptr;   // AFQMC_OT_KERNEL=1: the one-kernel route (tests)
   if (G > 1) {
     h->theta_buf = h->ThT;
     h->a_slots = dalloc(h, (size_t)G * mw * 2 * MM);

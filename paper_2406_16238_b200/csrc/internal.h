@@ -63,6 +63,10 @@ struct OTArgs {                 // overlap / Theta / one-body energy, one CTA pe
   int M, Nt, nblk;
   int off[2], ns[2];
   int want_theta, want_e1;
+  // DMMA route (all three set): trial^T [Nt][M], scratch O [nw][Nt][Nt] complex, scratch Aop [nw][2Nt][2Nt]
+  const double* trialT;
+  double* Obuf;
+  double* Aop;
 };
 int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st);
 

@@ -7,6 +7,8 @@
 //   a10    re-orthonormalisation by two Cholesky-QR passes
 //
 // One CTA per (spin block, walker); these stages are <= 1 % of the flops of a step.
+#include <cstring>
+
 #include "internal.h"
 
 namespace afq {
@@ -197,6 +199,114 @@ __global__ void __launch_bounds__(256) overlap_theta_kernel(OTArgs a) {
     block_sum<2>(e1, red);
     if (tid == 0) reinterpret_cast<double2*>(a.e1)[(size_t)w * a.nblk + blk] = make_double2(e1[0], e1[1]);
   }
+}
+
+// ------------------------------------------------------------------------------ a1 / a2 on DMMA
+// The same stage as overlap_theta_kernel with its two contractions on the tensor cores:
+//   O = psi^T phi          batched KN GEMM (gemm_ws.cu), all blocks at once: Obuf[w][Nt][2 Nt]
+//   gj_kernel              per (block, walker): Gauss-Jordan inverse + det of the diagonal block, and the
+//                          inverse written as the real (2 Nt) x (2 Nt) operand
+//                              Aop[(plane, i)][(j, plane')] = [[Re Oinv^T, -Im Oinv^T], [Im Oinv^T, Re Oinv^T]]
+//   Theta^T = Aop W^T      batched NK GEMM: ThT[w][(plane, i)][q] = sum_k Aop[(plane, i)][k] W[q][k]
+//   e1_kernel              one-body energy sum hrot . Theta
+__global__ void __launch_bounds__(256) gj_kernel(OTArgs a) {
+  extern __shared__ __align__(16) unsigned char smraw[];
+  const int blk = blockIdx.x, w = blockIdx.y;
+  const int ns = a.ns[blk], off = a.off[blk], Nt = a.Nt;
+  const int tid = threadIdx.x;
+  const int ld2 = 2 * ns;
+  double2* Aug = reinterpret_cast<double2*>(smraw);             // [ns][2 ns]
+  double2* fcol = Aug + (size_t)ns * ld2;                       // [ns]
+  __shared__ int s_piv;
+  __shared__ double2 s_det;
+  const double2* O = reinterpret_cast<const double2*>(a.Obuf) + (size_t)w * Nt * Nt;
+  for (int idx = tid; idx < ns * ns; idx += blockDim.x) {
+    const int i = idx / ns, j = idx % ns;
+    Aug[i * ld2 + j] = O[(size_t)(off + i) * Nt + off + j];
+    Aug[i * ld2 + ns + j] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+  }
+  if (tid == 0) s_det = make_double2(1.0, 0.0);
+  __syncthreads();
+  for (int c = 0; c < ns; ++c) {
+    if (tid < 32) {
+      double best = -1.0;
+      int bi = c;
+      for (int r = c + tid; r < ns; r += 32) {
+        double2 v = Aug[r * ld2 + c];
+        double m = v.x * v.x + v.y * v.y;
+        if (!(m <= best)) { best = m; bi = r; }   // NaN counts as a candidate so it propagates
+      }
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        double ob = __shfl_down_sync(0xffffffffu, best, o);
+        int oi = __shfl_down_sync(0xffffffffu, bi, o);
+        if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
+      }
+      if (tid == 0) s_piv = bi;
+    }
+    __syncthreads();
+    const int piv = s_piv;
+    if (piv != c) {
+      for (int j = tid; j < ld2; j += blockDim.x) {
+        double2 u = Aug[c * ld2 + j];
+        Aug[c * ld2 + j] = Aug[piv * ld2 + j];
+        Aug[piv * ld2 + j] = u;
+      }
+      if (tid == 0) s_det = make_double2(-s_det.x, -s_det.y);
+    }
+    __syncthreads();
+    const double2 pv = Aug[c * ld2 + c];
+    __syncthreads();
+    const double2 ipv = cinv(pv);
+    if (tid == 0) s_det = cmul(s_det, pv);
+    for (int j = tid; j < ld2; j += blockDim.x) Aug[c * ld2 + j] = cmul(Aug[c * ld2 + j], ipv);
+    for (int r = tid; r < ns; r += blockDim.x)
+      if (r != c) fcol[r] = Aug[r * ld2 + c];
+    __syncthreads();
+    for (int idx = tid; idx < ns * ld2; idx += blockDim.x) {
+      const int r = idx / ld2, j = idx % ld2;
+      if (r != c) {
+        const double2 f = fcol[r], pc = Aug[c * ld2 + j];
+        double2 v = Aug[idx];
+        v.x -= f.x * pc.x - f.y * pc.y;
+        v.y -= f.x * pc.y + f.y * pc.x;
+        Aug[idx] = v;
+      }
+    }
+    __syncthreads();
+  }
+  if (tid == 0) reinterpret_cast<double2*>(a.det)[(size_t)w * a.nblk + blk] = s_det;
+  if (!a.want_theta) return;
+  // rows (plane, off + i) of Aop, all 2 Nt columns (zero outside this spin block)
+  const int K2 = 2 * Nt;
+  double* Aop = a.Aop + (size_t)w * K2 * K2;
+  for (int idx = tid; idx < ns * Nt; idx += blockDim.x) {
+    const int i = idx / Nt, jc = idx % Nt;           // jc: column of the walker, all blocks
+    double2 o = make_double2(0.0, 0.0);
+    if (jc >= off && jc < off + ns) o = Aug[(jc - off) * ld2 + ns + i];   // Oinv[j][i]
+    double* r0 = Aop + (size_t)(off + i) * K2 + 2 * jc;               // plane re
+    double* r1 = Aop + (size_t)(Nt + off + i) * K2 + 2 * jc;          // plane im
+    r0[0] = o.x; r0[1] = -o.y;
+    r1[0] = o.y; r1[1] = o.x;
+  }
+}
+
+// e1[w][blk] = sum_{i in block, q} hrot[off + i][q] * Theta^T[w][.][off + i][q]; grid (nblk, nw)
+__global__ void __launch_bounds__(256) e1_kernel(OTArgs a) {
+  __shared__ double red[8 * 2];
+  const int blk = blockIdx.x, w = blockIdx.y;
+  const int ns = a.ns[blk], off = a.off[blk], M = a.M, Nt = a.Nt;
+  const double* tr = a.ThT + ((size_t)(w * 2 + 0) * Nt + off) * M;
+  const double* ti = a.ThT + ((size_t)(w * 2 + 1) * Nt + off) * M;
+  const double* hr = a.hrot + (size_t)off * M;
+  double e1[2] = {0.0, 0.0};
+  for (long idx = threadIdx.x; idx < (long)ns * M; idx += blockDim.x) {
+    const double h = hr[idx];
+    e1[0] = fma(h, tr[idx], e1[0]);
+    e1[1] = fma(h, ti[idx], e1[1]);
+  }
+  block_sum<2>(e1, red);
+  if (threadIdx.x == 0) reinterpret_cast<double2*>(a.e1)[(size_t)w * a.nblk + blk] = make_double2(e1[0], e1[1]);
 }
 
 // ------------------------------------------------------------------------------ a4
@@ -415,7 +525,43 @@ static size_t ot_smem(int ns) {
   return (size_t)ns * 2 * ns * 16 + (size_t)kRows * ldp * 16 + (size_t)ns * 16 + (size_t)kRows * ns * 8 + 32 * 8 + 64;
 }
 
+// the DMMA route; returns launches or -1 if a GEMM cannot be served (caller falls back to the one-kernel route)
+static int run_overlap_theta_gemm(const OTArgs& a, int nw, cudaStream_t st) {
+  const int M = a.M, Nt = a.Nt, K2 = 2 * Nt;
+  int launches = 0;
+  // O[w] = trial^T (Nt x M, shared) * W[w] (M x 2 Nt)
+  int r = run_gemm_ws_kn(a.trialT, M, 0, 0, false, a.W, K2, (long)M * K2, a.Obuf, nullptr, K2, (long)Nt * K2, Nt, K2, M,
+                         nw, 1.0, 0, st);
+  if (r < 0) return -1;
+  launches += r;
+  int nsmax = a.ns[0];
+  if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
+  const size_t sm = (size_t)nsmax * 2 * nsmax * 16 + (size_t)nsmax * 16 + 64;
+  static size_t cur[64] = {0};
+  if (grow_on_device(cur, sm)) cudaFuncSetAttribute(gj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  gj_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);
+  ++launches;
+  if (!a.want_theta) return launches;
+  // ThT[w] (2 Nt x M) = Aop[w] (2 Nt x 2 Nt, k contiguous) * W[w]^T (W: M x 2 Nt, k contiguous)
+  GemmArgs g;
+  memset(&g, 0, sizeof(g));
+  g.A = a.Aop; g.lda = K2; g.sA = (long)K2 * K2;
+  g.B = a.W; g.ldb = K2; g.sB = (long)M * K2;
+  g.C = a.ThT; g.ldc = M; g.sC = (long)K2 * M;
+  g.M = K2; g.N = M; g.K = K2; g.batch = nw; g.splitK = 1; g.alpha = 1.0;
+  launches += run_gemm(GEMM_NK, g, st);
+  if (a.want_e1) {
+    e1_kernel<<<dim3(a.nblk, nw), 256, 0, st>>>(a);
+    ++launches;
+  }
+  return launches;
+}
+
 int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st) {
+  if (a.Obuf && a.Aop && a.trialT) {
+    const int r = run_overlap_theta_gemm(a, nw, st);
+    if (r > 0) return r;
+  }
   int nsmax = a.ns[0];
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = ot_smem(nsmax);
