@@ -90,8 +90,8 @@ typedef struct {
  *   L_chol DEVICE [n_chol][M][M], each L_g symmetric; BORROWED read-only until afqmc_destroy
  *          (it is the dominant resident array, 55 GB in the largest configuration).  With
  *          pack_chol = 1 it is borrowed only for the duration of afqmc_create: the handle keeps
- *          Lrot and a tile-packed copy of the upper triangles ([tiles][n_chol][4][32] doubles,
- *          0.53x the dense size at M = 1200) and every later call gives the same bits as with
+ *          Lrot and a tile-packed copy of the upper triangles ([tiles][n_chol][8][16] doubles,
+ *          0.51x the dense size at M = 1200) and every later call gives the same bits as with
  *          the dense tensor, so the caller may free L_chol afterwards.
  *   trial  EITHER [M][Nt] real, COPIED.
  *   out    receives the handle; NULL on failure. */

@@ -67,6 +67,8 @@ struct afqmc_handle {
   int* tc_tiles = nullptr;
   int tc_ntile = 0;
   void *Abf = nullptr, *Tb0 = nullptr, *Tb1 = nullptr;   // mixed precision: split A and Taylor terms
+  void *Lrb = nullptr, *Tfb = nullptr;                    // mixed precision: split Lrot and Theta^T (force bias)
+  int fb_tc_nsplit = 1;
   int vhs_ntile = 0;
   long step_count = 0;
   int last_nw = 0;
@@ -257,7 +259,15 @@ int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw)
 void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw) {
   const int M = h->M, Nt = h->Nt, nc = h->n_chol;
   // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
-  {
+  int nsplit = h->fb_split;
+  if (h->Lrb) {     // mixed precision: the shift xbar may be ANY complex vector (Eqs. 12, 16 hold for every
+                    // xbar), so single precision here changes the sampling efficiency only, not the estimator
+    StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
+    nsplit = h->fb_tc_nsplit;
+    const int r = run_fb_tc(h->ThT, h->Tfb, h->Lrb, h->Xp, nc, (long)2 * h->mwg * nc, 2 * nw, nc, Nt * M, nsplit, h->st);
+    if (r < 0) { h->err = "force bias (mixed precision): tensor map encode failed"; }
+    else h->launches += r;
+  } else {
     StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
     GemmArgs g = gemm_args();
     g.A = h->ThT; g.lda = (long)Nt * M; g.B = h->Lrot; g.ldb = (long)Nt * M;
@@ -273,7 +283,7 @@ void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw
   {
     StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
     ShiftArgs s;
-    s.Xp = h->Xp; s.sXp = (long)2 * h->mwg * nc; s.nsplit = h->fb_split; s.m = h->m; s.x = x;
+    s.Xp = h->Xp; s.sXp = (long)2 * h->mwg * nc; s.nsplit = nsplit; s.m = h->m; s.x = x;
     s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
     s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
     h->launches += run_field_shift(s, nw, h->st);
@@ -756,6 +766,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->Ab = dalloc(h, (vhs_tc_cf_elems(2 * mwg, nc) * 2 + 7) / 8);
     if (!h->Lb || !h->Ab) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Cholesky tensor)");
     h->launches += run_vhs_tc_split_L(h->L, h->Lb, h->tc_tiles, h->tc_ntile, M, nc, h->st);
+    {   // force bias: split Lrot once; Theta^T is split per step
+      h->fb_tc_nsplit = fb_tc_split(2 * mwg, nc, Nt * M, 16);
+      if (h->fb_tc_nsplit > h->fb_split) {
+        dfree_one(h, h->Xp);
+        h->Xp = dalloc(h, (size_t)h->fb_tc_nsplit * 2 * mwg * nc);
+        if (!h->Xp) return bail(AFQMC_ERR_ALLOC, "device allocation failed (force-bias partials)");
+      }
+      h->Lrb = dalloc(h, (fb_tc_L_elems(nc, Nt * M) * 2 + 7) / 8);
+      h->Tfb = dalloc(h, (fb_tc_T_elems(2 * mwg, Nt * M) * 2 + 7) / 8);
+      if (!h->Lrb || !h->Tfb) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split half-rotated tensor)");
+      h->launches += run_fb_tc_split_L(h->Lrot, h->Lrb, nc, Nt * M, h->st);
+    }
     if (taylor_tc_usable(2 * Nt)) {
       const size_t ta = (taylor_tc_A_elems(mw, M) * 2 + 7) / 8, tt = (taylor_tc_T_elems(mw, M, 2 * Nt) * 2 + 7) / 8;
       h->Abf = dalloc(h, ta); h->Tb0 = dalloc(h, tt); h->Tb1 = dalloc(h, tt);

@@ -146,7 +146,7 @@ int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_de
 // V_HS of a walker is stored straight into its owner's receive slot, possibly peer memory)
 int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int nmember, int rows_per_member,
                        const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st);
-// tile-packed upper triangle of L (the paper's pack_chol): [ntile_n][n_chol][4][32]
+// tile-packed upper triangle of L (the paper's pack_chol): [ntile_n][n_chol][8][16]
 size_t vhs_ws_packed_doubles(int ntile_n, int n_chol);
 int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
                    cudaStream_t st);
@@ -160,6 +160,14 @@ int run_vhs_tc_split_L(const double* L, void* Lb, const int* tiles_dev, int ntil
                        cudaStream_t st);
 int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, int nmember, int rows_per_member,
                const int* tiles_dev, int ntile_n, int M, int n_chol, cudaStream_t st);
+
+// force bias on the same tcgen05 kernel (plain epilogue, split over K = Nt M)
+size_t fb_tc_L_elems(int n_chol, int K);
+size_t fb_tc_T_elems(int rows, int K);
+int fb_tc_split(int rows, int n_chol, int K, int max_split);
+int run_fb_tc_split_L(const double* Lrot, void* Lrb, int n_chol, int K, cudaStream_t st);
+int run_fb_tc(const double* ThT, void* Tbuf, const void* Lrb, double* Xp, long ldc, long sCsplit, int rows, int n_chol,
+              int K, int split, cudaStream_t st);
 
 // taylor_tc.cu: Taylor propagation in the same emulated single precision (bf16 x 3 on tcgen05)
 size_t taylor_tc_A_elems(int nw, int M);

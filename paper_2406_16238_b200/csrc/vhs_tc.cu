@@ -108,8 +108,28 @@ struct TcArgs {
   const int* tiles;        // [ntile_n] packed (pb << 16 | qb)
   int M, rows, KT;         // KT = Gp / TC_BK
   int ntile_n, npairs, mtiles;
+  // EPI = 1 (plain row-major output, split over K): C[ks][row][n], n < N
+  double* C;
+  long ldc, sCsplit;
+  int N, nsplit, KTs;      // KTs: k stages per slice
 };
 
+template <int EPI>
+__device__ __forceinline__ void unit_decode(const TcArgs& a, int u, int& pr, int& mt, int& kbeg, int& kend) {
+  if (EPI == 1) {
+    const int ks = u % a.nsplit, rest = u / a.nsplit;
+    mt = rest % a.mtiles; pr = rest / a.mtiles;
+    kbeg = ks * a.KTs; kend = min(a.KT, kbeg + a.KTs);
+  } else {
+    pr = u / a.mtiles; mt = u % a.mtiles;
+    kbeg = 0; kend = a.KT;
+  }
+}
+
+// EPI = 0: V_HS - symmetric scatter of the tiles of the tile list (direct + mirrored stores).
+// EPI = 1: plain GEMM C[row][n] = sum_k A[row][k] B[n][k] over 256-column blocks of B rows, split over K
+//          (force bias X = Theta^T . Lrot: K = Nt M is long, N = n_chol short).
+template <int EPI>
 __global__ void __launch_bounds__(TC_THREADS, 1)
 vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB, const TcArgs a) {
   extern __shared__ unsigned char smem_raw[];
@@ -120,7 +140,8 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
   uint64_t* tempty = tfull + TC_ACC;
   uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(tempty + TC_ACC);
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int nunits = a.npairs * a.mtiles;        // work unit = (pair of N tiles, 128-row block)
+  // work unit = (pair of N tiles, 128-row block[, K slice])
+  const int nunits = a.npairs * a.mtiles * (EPI == 1 ? a.nsplit : 1);
 
   if (tid == 0) {
     for (int s = 0; s < TC_STAGES; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], 1); }
@@ -140,8 +161,9 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       prefetch_tensormap(&tmB);
       uint32_t it = 0;
       for (int u = blockIdx.x; u < nunits; u += gridDim.x) {
-        const int pr = u / a.mtiles, mt = u % a.mtiles;
-        for (int kt = 0; kt < a.KT; ++kt, ++it) {
+        int pr, mt, kbeg, kend;
+        unit_decode<EPI>(a, u, pr, mt, kbeg, kend);
+        for (int kt = kbeg; kt < kend; ++kt, ++it) {
           const int s = it % TC_STAGES;
           mbar_wait(&empty[s], ((it / TC_STAGES) & 1) ^ 1);
           mbar_expect_tx(&full[s], TC_STAGE);
@@ -163,7 +185,9 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       // (<= 2^-8 of hh) to the same accumulator would cost a truncation of the LARGE sum each time; kept apart,
       // the large sum sees one update per 16 gamma and the bias drops six-fold.  The epilogue adds D1 + D2.
       const uint32_t d1 = tmem_base + (uint32_t)acc * (2 * TC_NT * TC_N), d2 = d1 + TC_NT * TC_N;
-      for (int kt = 0; kt < a.KT; ++kt, ++it) {
+      int pr_, mt_, kbeg, kend;
+      unit_decode<EPI>(a, u, pr_, mt_, kbeg, kend);
+      for (int kt = kbeg; kt < kend; ++kt, ++it) {
         const int s = it % TC_STAGES;
         mbar_wait(&full[s], (it / TC_STAGES) & 1);
         tc_fence_after();
@@ -177,12 +201,12 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
             for (int q = 0; q < 6; ++q) {
               const uint64_t da = umma_desc(sa + pa[q] * TC_PLANE + k * 32);
               const uint64_t db = umma_desc(sb + pb[q] * (TC_NT * TC_PLANE) + k * 32);   // 256 rows: tile 0, tile 1
-              if (q == 5) umma_bf16(d1, da, db, kIdesc, (kt | k) != 0 ? 1u : 0u);
-              else umma_bf16(d2, da, db, kIdesc, (kt | k | q) != 0 ? 1u : 0u);
+              if (q == 5) umma_bf16(d1, da, db, kIdesc, ((kt - kbeg) | k) != 0 ? 1u : 0u);
+              else umma_bf16(d2, da, db, kIdesc, ((kt - kbeg) | k | q) != 0 ? 1u : 0u);
             }
           }
           umma_commit(&empty[s]);                       // stage free when these MMAs have read it
-          if (kt == a.KT - 1) umma_commit(&tfull[acc]);  // accumulators complete
+          if (kt == kend - 1) umma_commit(&tfull[acc]);  // accumulators complete
         }
         __syncwarp();
       }
@@ -200,8 +224,14 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
     int mt_cur = -1;
     for (int u = blockIdx.x; u < nunits; u += gridDim.x, ++tc) {
       const int acc = tc % TC_ACC;
-      const int pr = u / a.mtiles, mt = u % a.mtiles;
-      if (mt != mt_cur) {
+      int pr, mt, kbeg, kend;
+      unit_decode<EPI>(a, u, pr, mt, kbeg, kend);
+      if (EPI == 1) {
+        const int r = mt * TC_M + quarter * 32 + lane;
+        __syncwarp();
+        rowp[lane] = r < a.rows ? a.C + (size_t)(kbeg / a.KTs) * a.sCsplit + (size_t)r * a.ldc : nullptr;
+        __syncwarp();
+      } else if (mt != mt_cur) {
         const int r = mt * TC_M + quarter * 32 + lane;
         __syncwarp();
         rowp[lane] = r < a.rows ? a.Cb[r / a.rpm] + (size_t)(r % a.rpm) * MM : nullptr;
@@ -230,6 +260,22 @@ vhs_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
           if (lane == 0) mbar_arrive(&tempty[acc]);    // the accumulators may be overwritten from here on
         }
         if (tl >= a.ntile_n) continue;
+        if (EPI == 1) {
+          // plain rows: after the transpose of block c, lane l holds column 128 tl + 32 c + l of row i
+#pragma unroll
+          for (int c = 0; c < 4; ++c) {
+            warp_transpose32(v[c], lane);
+            const int n = tl * TC_N + 32 * c + lane;
+            if (n < a.N) {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                double* R = rowp[i];
+                if (R) R[n] = (double)v[c][i];
+              }
+            }
+          }
+          continue;
+        }
         const int tn = a.tiles[tl];
         const int p0 = (tn >> 16) * TC_PT, q0 = (tn & 0xffff) * TC_QT;
         const bool fast = (q0 >= p0 + TC_PT) && (p0 + TC_PT <= a.M) && (q0 + TC_QT <= a.M);
@@ -322,7 +368,8 @@ int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, in
   const int Gp = vhs_tc_gamma_padded(n_chol), Rp = vhs_tc_rows_padded(rows);
   static uint64_t attr = 0;
   if (first_use_on_device(&attr)) {
-    cudaFuncSetAttribute(vhs_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+    cudaFuncSetAttribute(vhs_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+    cudaFuncSetAttribute(vhs_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
   }
   const int nsm = sm_count_current();
   split_cf_kernel<<<dim3((Gp + 255) / 256, Rp), 256, 0, st>>>(Cf, (__nv_bfloat16*)Ab, rows, n_chol, Rp, Gp);
@@ -346,7 +393,74 @@ int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, in
   a.ntile_n = ntile_n; a.npairs = (ntile_n + TC_NT - 1) / TC_NT; a.mtiles = Rp / TC_M;
   const long nt = (long)a.npairs * a.mtiles;
   const int grid = nt < nsm ? (int)nt : nsm;
-  vhs_tc_kernel<<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmB, a);
+  a.C = nullptr; a.ldc = 0; a.sCsplit = 0; a.N = 0; a.nsplit = 1; a.KTs = a.KT;
+  vhs_tc_kernel<0><<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmB, a);
+  return 2;
+}
+
+// ---- force bias on the same kernel: X[s][row][g] = sum_{k in slice s} ThT[row][k] Lrot[g][k] -------------
+int fb_tc_rows_padded(int n_chol) { return (n_chol + TC_NT * TC_N - 1) / (TC_NT * TC_N) * (TC_NT * TC_N); }
+size_t fb_tc_L_elems(int n_chol, int K) { return (size_t)3 * fb_tc_rows_padded(n_chol) * vhs_tc_gamma_padded(K); }
+size_t fb_tc_T_elems(int rows, int K) { return (size_t)3 * vhs_tc_rows_padded(rows) * vhs_tc_gamma_padded(K); }
+
+// K slices so that (pairs x row blocks x slices) fills the SMs; every slice is non-empty
+int fb_tc_split(int rows, int n_chol, int K, int max_split) {
+  const int nsm = sm_count_current();
+  const int KT = vhs_tc_gamma_padded(K) / TC_BK;
+  const long base = (long)(fb_tc_rows_padded(n_chol) / (TC_NT * TC_N)) * (vhs_tc_rows_padded(rows) / TC_M);
+  int best = 1;
+  double best_cost = 1e300;
+  for (int s = 1; s <= max_split; ++s) {
+    const int KTs = (KT + s - 1) / s;
+    if ((long)KTs * (s - 1) >= KT && s > 1) continue;
+    const double cost = (double)((base * s + nsm - 1) / nsm) * (KTs + 8);
+    if (cost < best_cost) { best_cost = cost; best = s; }
+  }
+  return best;
+}
+
+// Lrb[3][rows padded to 256][Kp] from Lrot [n_chol][K] (setup)
+int run_fb_tc_split_L(const double* Lrot, void* Lrb, int n_chol, int K, cudaStream_t st) {
+  const int Kp = vhs_tc_gamma_padded(K), Rp = fb_tc_rows_padded(n_chol);
+  split_cf_kernel<<<dim3((Kp + 255) / 256 > 64 ? 64 : (Kp + 255) / 256, Rp), 256, 0, st>>>(Lrot, (__nv_bfloat16*)Lrb, n_chol, K,
+                                                                                          Rp, Kp);
+  return 1;
+}
+
+int run_fb_tc(const double* ThT, void* Tbuf, const void* Lrb, double* Xp, long ldc, long sCsplit, int rows, int n_chol,
+              int K, int split, cudaStream_t st) {
+  const int Kp = vhs_tc_gamma_padded(K), Rp = vhs_tc_rows_padded(rows), Np = fb_tc_rows_padded(n_chol);
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr)) {
+    cudaFuncSetAttribute(vhs_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+    cudaFuncSetAttribute(vhs_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
+  }
+  const int nsm = sm_count_current();
+  split_cf_kernel<<<dim3((Kp + 255) / 256 > 64 ? 64 : (Kp + 255) / 256, Rp), 256, 0, st>>>(ThT, (__nv_bfloat16*)Tbuf, rows, K, Rp,
+                                                                                          Kp);
+  TensorMap tmA, tmB;
+  {
+    const uint64_t dims[3] = {(uint64_t)Kp, (uint64_t)Rp, 3};
+    const uint64_t str[2] = {(uint64_t)Kp * 2, (uint64_t)Rp * Kp * 2};
+    const uint32_t box[3] = {TC_BK, TC_M, 3};
+    if (make_tensor_map_bf16(&tmA, Tbuf, 3, dims, str, box, 64) != 0) return -1;
+  }
+  const int ntile = Np / TC_N;
+  {
+    const uint64_t dims[4] = {(uint64_t)Kp, TC_N, (uint64_t)ntile, 3};
+    const uint64_t str[3] = {(uint64_t)Kp * 2, (uint64_t)TC_N * Kp * 2, (uint64_t)Np * Kp * 2};
+    const uint32_t box[4] = {TC_BK, TC_N, TC_NT, 3};
+    if (make_tensor_map_bf16(&tmB, Lrb, 4, dims, str, box, 64) != 0) return -1;
+  }
+  TcArgs a;
+  for (int r = 0; r < kMaxGroup; ++r) a.Cb[r] = nullptr;
+  a.rpm = 1; a.tiles = nullptr; a.M = 0; a.rows = rows; a.KT = Kp / TC_BK;
+  a.ntile_n = ntile; a.npairs = ntile / TC_NT; a.mtiles = Rp / TC_M;
+  a.C = Xp; a.ldc = ldc; a.sCsplit = sCsplit; a.N = n_chol;
+  a.nsplit = split < 1 ? 1 : split; a.KTs = (a.KT + a.nsplit - 1) / a.nsplit;
+  const long nt = (long)a.npairs * a.mtiles * a.nsplit;
+  const int grid = nt < nsm ? (int)nt : nsm;
+  vhs_tc_kernel<1><<<grid, TC_THREADS, TC_SMEM, st>>>(tmA, tmB, a);
   return 2;
 }
 

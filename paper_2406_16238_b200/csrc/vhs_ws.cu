@@ -7,10 +7,10 @@
 // the L bytes of the dense contraction, same result (each element of A is written once, from
 // the upper-triangle entry of L).
 //
-// Tile: 128 rows (w, plane) x (4 p x 32 q).  Producer: per 16-gamma stage one box of Cf
-// (k-major, 128 x 16) and eight boxes {16 q, 1 p, 16 gamma} of L, all SWIZZLE_128B.  Consumers:
-// 8 warps of 64 x 32 (8 x 4 DMMA blocks); a warp owns one q-octet and the 4 p rows, so the
-// mirrored store is 32 contiguous bytes per (row, q).
+// Tile: 128 rows (w, plane) x (8 p x 16 q) (1200 = 150 x 8 = 75 x 16: no ragged tile at the headline size).
+// Producer: per 16-gamma stage one box of Cf (k-major, 128 x 16) and eight boxes {16 q, 1 p, 16 gamma} of L,
+// all SWIZZLE_128B.  Consumers: 8 warps of 64 x 32 (8 x 4 DMMA blocks); a warp owns one q-octet and 4 p rows,
+// so the mirrored store is 32 contiguous bytes per (row, q).
 #include <vector>
 
 #include "internal.h"
@@ -21,7 +21,7 @@ namespace afq {
 namespace {
 
 constexpr int kProd = 128;
-constexpr int BMv = 128, PT = 4, QT = 32, BKv = 16;
+constexpr int BMv = 128, PT = 8, QT = 16, BKv = 16;
 constexpr int NCWv = 8, NCTv = NCWv * 32, THREADSv = NCTv + kProd;
 constexpr int A_BYTES = BMv * 128, B_BOX = BKv * 128, B_BYTES = PT * (QT / 16) * B_BOX;
 constexpr int STAGE_BYTESv = A_BYTES + B_BYTES;    // 32 KB
@@ -87,13 +87,13 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
   reg_alloc<240>();
   constexpr int MI = 8, NI = 4;
   const int g = lane >> 2, t = lane & 3;
-  const int wm = warp & 1, wn = warp >> 1;       // wn: q-octet 0..3 of the 32-wide tile
+  const int wm = warp & 1, wn = warp >> 1;       // wn: (q-octet, p-half) of the 8 p x 16 q tile
   const int p = rperm(g);
   // A (k-major, 16-byte loads): chunk (4 kp + t) of row 8 b + p
   const uint32_t la0 = (uint32_t)(p * 128 + ((t ^ p) << 4));
   const uint32_t la1 = (uint32_t)(p * 128 + (((t ^ p) ^ 4) << 4));
   // B (n-major, 8-byte loads): box (j, qb) row k = 8 kp + 2 t + par, element q = 8 h + g
-  const int qb = wn >> 1, hh = wn & 1;
+  const int hh = wn & 1, ph = wn >> 1;            // q-octet 0..1 of the 16-q box, p rows 4 ph .. 4 ph + 3
   const int chunk = 4 * hh + (g >> 1);
   uint32_t lb[2][2];                              // [kp][par]
 #pragma unroll
@@ -101,7 +101,7 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
 #pragma unroll
     for (int par = 0; par < 2; ++par) {
       const int k = 8 * kp + 2 * t + par;
-      lb[kp][par] = (uint32_t)(qb * B_BOX + k * 128 + ((chunk ^ (k & 7)) << 4) + (g & 1) * 8);
+      lb[kp][par] = (uint32_t)(4 * ph * B_BOX + k * 128 + ((chunk ^ (k & 7)) << 4) + (g & 1) * 8);
     }
   const uint32_t smem_u = smem_u32(smem);
   const uint32_t aoff = (uint32_t)(wm * MI) * 1024u;
@@ -147,10 +147,11 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
     }
 
     // ---- epilogue: direct store at [p][q] (q >= p) and mirrored store at [q][p] (q > p)
-    const int ql = q0 + 8 * wn;                    // first q of this warp's octet
-    if (ql + 7 < p0) continue;                     // entirely below the diagonal: nothing to keep
+    const int ql = q0 + 8 * hh;                    // first q of this warp's octet
+    const int pw = p0 + 4 * ph;                    // first of this warp's 4 p rows
+    if (ql + 7 < pw) continue;                     // entirely below the diagonal: nothing to keep
     const int q = ql + 2 * t;                      // this lane's q, q + 1
-    const bool fast = (ql >= p0 + PT) && (p0 + PT <= a.M) && (ql + 8 <= a.M);
+    const bool fast = (ql >= pw + 4) && (pw + 4 <= a.M) && (ql + 8 <= a.M);
 #pragma unroll
     for (int i = 0; i < MI; ++i) {
       const int r = mt * BMv + 8 * (wm * MI + i) + p;
@@ -159,17 +160,17 @@ vhs_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ Ten
       if (fast) {
 #pragma unroll
         for (int j = 0; j < NI; ++j)
-          *reinterpret_cast<double2*>(Cr + (size_t)(p0 + j) * a.M + q) = make_double2(acc[i][j][0], acc[i][j][1]);
+          *reinterpret_cast<double2*>(Cr + (size_t)(pw + j) * a.M + q) = make_double2(acc[i][j][0], acc[i][j][1]);
 #pragma unroll
         for (int e = 0; e < 2; ++e) {
-          double* d = Cr + (size_t)(q + e) * a.M + p0;
+          double* d = Cr + (size_t)(q + e) * a.M + pw;
           *reinterpret_cast<double2*>(d) = make_double2(acc[i][0][e], acc[i][1][e]);
           *reinterpret_cast<double2*>(d + 2) = make_double2(acc[i][2][e], acc[i][3][e]);
         }
       } else {
 #pragma unroll
         for (int j = 0; j < NI; ++j) {
-          const int pp = p0 + j;
+          const int pp = pw + j;
           if (pp >= a.M) continue;
 #pragma unroll
           for (int e = 0; e < 2; ++e) {
