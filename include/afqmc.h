@@ -71,9 +71,9 @@ typedef struct {
                         /* shares one Cholesky tensor, 0 or 1 = none, at most 8; with G > 1 L_chol, */
                         /* n_chol describe THIS member's gamma slice and max_walkers its own walkers */
   int32_t group_rank;   /* this member's index in the group, 0 .. G-1                             */
-  int32_t mixed_precision; /* 0: everything in double.  1: the V_HS build (a5) and the Taylor terms     */
-                        /* (a7), the cost of a step without energy, in EMULATED single precision on */
-                        /* the tcgen05 tensor                                                        */
+  int32_t mixed_precision; /* 0: everything in double.  1: the propagation - force bias (a3), V_HS      */
+                        /* build (a5), one-body half steps (a6, a8), Taylor terms (a7) - in         */
+                        /* EMULATED single precision on the tcgen05 tensor                          */
                         /* cores - operands split into three bfloat16 numbers, six partial products, */
                         /* FP32 accumulation in tensor memory -, everything else incl. the local     */
                         /* energy in double ("mixed precision").  The handle keeps the */

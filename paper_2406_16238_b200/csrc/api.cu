@@ -67,6 +67,7 @@ struct afqmc_handle {
   int* tc_tiles = nullptr;
   int tc_ntile = 0;
   void *Abf = nullptr, *Tb0 = nullptr, *Tb1 = nullptr;   // mixed precision: split A and Taylor terms
+  void* E1b = nullptr;                                    // mixed precision: split one-body propagator
   void *Lrb = nullptr, *Tfb = nullptr;                    // mixed precision: split Lrot and Theta^T (force bias)
   int fb_tc_nsplit = 1;
   int vhs_ntile = 0;
@@ -207,6 +208,7 @@ void build_E1(afqmc_handle* h, double dt) {
     std::swap(P, Q);
   }
   h->launches += run_scale_copy(h->E1, P, 1.0, MM, h->st);
+  if (h->E1b) h->launches += taylor_tc_prepare_E1(h->E1, h->E1b, M, h->st);
   h->dt_cached = dt;
 }
 
@@ -290,6 +292,7 @@ void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw
   }
 }
 
+int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
 int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
 
 int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double dt, int nw) {
@@ -326,59 +329,9 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   return propagate_device(h, W, wt, h->cfb, h->cmf, dt, nw);
 }
 
-// a6-a10 with A = V_HS in h->A and the overlap determinants of the incoming walkers in h->det_old
-int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw) {
+// a9-a10: overlap of the propagated walkers, phaseless weight update, re-orthonormalisation on schedule
+int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw) {
   const int M = h->M, Nt = h->Nt;
-  const long MM = (long)M * M;
-  if (!(h->dt_cached == dt)) build_E1(h, dt);
-  // a6: T0 = Acc = E1 phi
-  const long wstride = (long)M * 2 * Nt;
-  {
-    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
-    GemmArgs g = gemm_args();
-    g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
-    g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
-    g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 2, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
-  }
-  // a7: T_n = A T_{n-1} / n, Acc += T_n
-  if (h->Abf) {     // mixed precision: bf16 x 3 on tcgen05, FP64 running sum
-    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
-    const int r = run_taylor_tc(h->A, h->T0, h->Acc, h->Abf, h->Tb0, h->Tb1, nw, M, 2 * Nt, h->K, h->st);
-    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "taylor (mixed precision): tensor map encode failed");
-    h->launches += r;
-  } else {
-    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
-    double *Tp = h->T0, *Tn = h->T1;
-    for (int n = 1; n <= h->K; ++n) {
-      GemmArgs g = gemm_args();
-      g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
-      g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
-      g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
-      int r = -1;
-      if (h->ws)
-        r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
-                           M, nw, 1.0 / n, 1, h->st);
-      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
-      std::swap(Tp, Tn);
-    }
-  }
-  // a8: phi = E1 Acc, written into the caller's walkers
-  {
-    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
-    GemmArgs g = gemm_args();
-    g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
-    g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
-    int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 0, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
-  }
   // a9: new overlap and weights
   {
     StageTimer tm(h, AFQMC_STAGE_OVERLAP_NEW);
@@ -406,6 +359,87 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
     h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
   }
   return AFQMC_OK;
+}
+
+// a6-a10 with A = V_HS in h->A and the overlap determinants of the incoming walkers in h->det_old
+int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw) {
+  const int M = h->M, Nt = h->Nt;
+  const long MM = (long)M * M;
+  if (!(h->dt_cached == dt)) build_E1(h, dt);
+  if (h->Abf) {
+    // mixed precision: a6, a7, a8 as bf16 x 3 GEMMs on tcgen05; the running sum of the Taylor terms is FP64
+    const int N2 = 2 * Nt;
+    int r = 0, bad = 0;
+    {
+      StageTimer tm(h, AFQMC_STAGE_ONE_BODY);       // Acc = T_0 = phi + (E1 - 1) phi; the split T_0 goes straight to Tb1
+      h->launches += taylor_tc_prepare_T(W, h->Tb0, nw, M, N2, h->st);
+      r = taylor_tc_apply(h->E1b, true, h->Tb0, h->Tb1, h->Acc, true, W, 1.0, nw, M, N2, h->st);
+      bad |= r < 0; h->launches += r > 0 ? r : 0;
+    }
+    {
+      StageTimer tm(h, AFQMC_STAGE_TAYLOR);         // Acc += A^n T_0 / n!
+      h->launches += taylor_tc_prepare_A(h->A, h->Abf, nw, M, h->st);
+      void* tb[2] = {h->Tb1, h->Tb0};
+      for (int n = 1; n <= h->K; ++n) {
+        const int cur = (n - 1) & 1;
+        r = taylor_tc_apply(h->Abf, false, tb[cur], n < h->K ? tb[cur ^ 1] : nullptr, h->Acc, false, nullptr, 1.0 / n, nw, M, N2,
+                            h->st);
+        bad |= r < 0; h->launches += r > 0 ? r : 0;
+      }
+    }
+    {
+      StageTimer tm(h, AFQMC_STAGE_ONE_BODY);       // phi = Acc + (E1 - 1) Acc, into the caller's walkers
+      h->launches += taylor_tc_prepare_T(h->Acc, h->Tb0, nw, M, N2, h->st);
+      r = taylor_tc_apply(h->E1b, true, h->Tb0, nullptr, W, true, h->Acc, 1.0, nw, M, N2, h->st);
+      bad |= r < 0; h->launches += r > 0 ? r : 0;
+    }
+    if (bad) return fail(h, AFQMC_ERR_CUDA, "propagation (mixed precision): tensor map encode failed");
+    return finish_step_device(h, W, wt, cfb, cmf, dt, nw);
+  }
+  // a6: T0 = Acc = E1 phi
+  const long wstride = (long)M * 2 * Nt;
+  {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = W; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
+    g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 2, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+  }
+  // a7: T_n = A T_{n-1} / n, Acc += T_n
+  {
+    StageTimer tm(h, AFQMC_STAGE_TAYLOR);
+    double *Tp = h->T0, *Tn = h->T1;
+    for (int n = 1; n <= h->K; ++n) {
+      GemmArgs g = gemm_args();
+      g.A = h->A; g.A2 = h->A + MM; g.lda = M; g.sA = 2 * MM; g.B = Tp; g.ldb = 2 * Nt; g.sB = wstride;
+      g.C = Tn; g.C2 = h->Acc; g.mode = 1; g.ldc = 2 * Nt; g.sC = wstride;
+      g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw; g.alpha = 1.0 / n;
+      int r = -1;
+      if (h->ws)
+        r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
+                           M, nw, 1.0 / n, 1, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
+      std::swap(Tp, Tn);
+    }
+  }
+  // a8: phi = E1 Acc, written into the caller's walkers
+  {
+    StageTimer tm(h, AFQMC_STAGE_ONE_BODY);
+    GemmArgs g = gemm_args();
+    g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
+    g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
+    int r = -1;
+    if (h->ws)
+      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
+                         nw, 1.0, 0, h->st);
+    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+  }
+  return finish_step_device(h, W, wt, cfb, cmf, dt, nw);
 }
 
 // Comb on device buffers: map -> h->pmap, weights in place, walkers and stored overlaps permuted.
@@ -781,7 +815,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     if (taylor_tc_usable(2 * Nt)) {
       const size_t ta = (taylor_tc_A_elems(mw, M) * 2 + 7) / 8, tt = (taylor_tc_T_elems(mw, M, 2 * Nt) * 2 + 7) / 8;
       h->Abf = dalloc(h, ta); h->Tb0 = dalloc(h, tt); h->Tb1 = dalloc(h, tt);
-      if (!h->Abf || !h->Tb0 || !h->Tb1) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Taylor operands)");
+      h->E1b = dalloc(h, (taylor_tc_A_elems(1, M) * 2 + 7) / 8);
+      if (!h->Abf || !h->Tb0 || !h->Tb1 || !h->E1b) return bail(AFQMC_ERR_ALLOC, "device allocation failed (split Taylor operands)");
       cudaMemsetAsync(h->Tb0, 0, tt * 8, h->st);      // the zero padding of k and n is never written again
       cudaMemsetAsync(h->Tb1, 0, tt * 8, h->st);
     }

@@ -173,8 +173,11 @@ int run_fb_tc(const double* ThT, void* Tbuf, const void* Lrb, double* Xp, long l
 size_t taylor_tc_A_elems(int nw, int M);
 size_t taylor_tc_T_elems(int nw, int M, int N2);
 bool taylor_tc_usable(int N2);
-int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, void* Tb0, void* Tb1, int nw, int M,
-                  int N2, int order, cudaStream_t st);
+int taylor_tc_prepare_A(const double* A, void* Abf, int nw, int M, cudaStream_t st);
+int taylor_tc_prepare_E1(const double* E1, void* E1b, int M, cudaStream_t st);
+int taylor_tc_prepare_T(const double* T, void* Tb, int nw, int M, int N2, cudaStream_t st);
+int taylor_tc_apply(const void* Aplanes, bool real_shared, const void* Tb, void* Tnext, double* Out, bool assign,
+                    const double* Src, double alpha, int nw, int M, int N2, cudaStream_t st);
 
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,

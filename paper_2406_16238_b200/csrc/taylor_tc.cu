@@ -49,6 +49,24 @@ __global__ void __launch_bounds__(256) split_A_kernel(const double* __restrict__
   }
 }
 
+// E1b[plane][m][q] (row stride 2 Kp, second half unused) from E1[m][q] - delta_mq: the one-body half step is
+// applied as phi + (E1 - 1) phi with the identity part kept in FP64, so that the truncating FP32 accumulation
+// acts on the small correction only (E1 = expm(-dt/2 h_mod) is 1 + O(dt)); grid M
+__global__ void __launch_bounds__(256) split_E1_kernel(const double* __restrict__ E1, __nv_bfloat16* __restrict__ E1b,
+                                                       int M, int Kp) {
+  const int m = blockIdx.x;
+  const size_t plane = (size_t)M * 2 * Kp;
+  __nv_bfloat16* out = E1b + (size_t)m * 2 * Kp;
+  for (int q = threadIdx.x; q < Kp; q += blockDim.x) {
+    const double x = q < M ? E1[(size_t)m * M + q] - (q == m ? 1.0 : 0.0) : 0.0;
+    __nv_bfloat16 h, mm, l;
+    split3(x, h, mm, l);
+    out[q] = h;
+    out[q + plane] = mm;
+    out[q + 2 * plane] = l;
+  }
+}
+
 // Tb[w][plane][n][k] = T[w][k][n], Tb[w][plane][n][Kp + k] = (J T)[k][n]; zero for n >= N2 or k >= M.
 // grid (Kp / 32, nw), 256 threads; T is [nw][M][N2] doubles (the walker layout)
 __global__ void __launch_bounds__(256) split_T_kernel(const double* __restrict__ T, __nv_bfloat16* __restrict__ Tb,
@@ -84,6 +102,9 @@ struct TyArgs {
   double* Acc;             // [nw][M][N2] running sum, FP64
   __nv_bfloat16* Tnext;    // Tb of the next order, or nullptr for the last one
   double alpha;            // 1 / n
+  int assign;              // Acc = term instead of Acc += term
+  const double* Src;       // assign only: Acc = Src + term (the operator is 1 + Aop; nullptr: none)
+  int a_shared;            // the A operand is one matrix for all walkers
   int M, N2, Np, Kp, nw;
   int KT, mtiles, stages;
   uint32_t idesc;
@@ -129,7 +150,7 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
           mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
           mbar_expect_tx(&full[s], (uint32_t)a.stage_bytes);
           unsigned char* sa = smem + (size_t)s * a.stage_bytes;
-          tma_load_4d(sa, &tmA, &full[s], kt * TY_BK, mt * TY_M, 0, w);      // rows past M read as zeros
+          tma_load_4d(sa, &tmA, &full[s], kt * TY_BK, mt * TY_M, 0, a.a_shared ? 0 : w);   // rows past M: zeros
           tma_load_4d(sa + TY_AOPER, &tmB, &full[s], kt * TY_BK, 0, 0, w);
         }
       }
@@ -201,8 +222,18 @@ taylor_tc_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ 
         for (int j = 0; j < 32; ++j) {
           const int n = 32 * c + j;
           if (n >= a.N2) continue;
-          const float t = v[j] * alpha;
-          accrow[n] += (double)t;
+          float t = v[j] * alpha;
+          if (a.assign) {
+            if (a.Src) {
+              const double full = a.Src[((size_t)w * a.M + m) * a.N2 + n] + (double)t;
+              accrow[n] = full;
+              t = (float)full;                     // what the next order sees
+            } else {
+              accrow[n] = (double)t;
+            }
+          } else {
+            accrow[n] += (double)t;
+          }
           if (tn) {
             // an FP32 number is exactly three bfloat16 numbers
             const __nv_bfloat16 h = __float2bfloat16_rn(t);
@@ -238,10 +269,34 @@ size_t taylor_tc_A_elems(int nw, int M) { return (size_t)nw * 3 * M * 2 * round_
 size_t taylor_tc_T_elems(int nw, int M, int N2) { return (size_t)nw * 3 * round_up(N2, 16) * 2 * round_up(M, TY_BK); }
 bool taylor_tc_usable(int N2) { return N2 % 2 == 0 && round_up(N2, 16) <= 256; }
 
-// Acc (holding T_0 on entry) += sum_{n=1..order} A^n T_0 / n!, A planar [nw][2][M][M], T0 / Acc [nw][M][N2].
-// Abf, Tb0, Tb1 are scratch of taylor_tc_A_elems / taylor_tc_T_elems bf16 each.  Returns launches or -1.
-int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, void* Tb0, void* Tb1, int nw, int M,
-                  int N2, int order, cudaStream_t st) {
+// Abf <- planar complex A [nw][2][M][M]
+int taylor_tc_prepare_A(const double* A, void* Abf, int nw, int M, cudaStream_t st) {
+  split_A_kernel<<<dim3(M, nw), 256, 0, st>>>(A, (__nv_bfloat16*)Abf, M, round_up(M, TY_BK));
+  return 1;
+}
+// E1b (layout of ONE walker of Abf, real half only) <- real E1 [M][M]
+int taylor_tc_prepare_E1(const double* E1, void* E1b, int M, cudaStream_t st) {
+  split_E1_kernel<<<M, 256, 0, st>>>(E1, (__nv_bfloat16*)E1b, M, round_up(M, TY_BK));
+  return 1;
+}
+// Tb <- T [nw][M][N2] (walker layout): [T^T | (J T)^T] rows
+int taylor_tc_prepare_T(const double* T, void* Tb, int nw, int M, int N2, cudaStream_t st) {
+  static uint64_t attr = 0;
+  if (first_use_on_device(&attr))
+    cudaFuncSetAttribute(split_T_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 257 * 8);
+  const int Kp = round_up(M, TY_BK);
+  split_T_kernel<<<dim3(Kp / 32, nw), 256, (size_t)32 * (N2 + 1) * 8, st>>>(T, (__nv_bfloat16*)Tb, M, N2,
+                                                                            round_up(N2, 16), Kp);
+  return 1;
+}
+
+// Out (+)= alpha * Aop * T per walker, where T is given by its split planes Tb and
+//   real_shared = false: Aop = the walker's complex A (Abf of taylor_tc_prepare_A), K = 2 Kp
+//   real_shared = true : Aop = one real matrix for all walkers (E1b of taylor_tc_prepare_E1), K = Kp
+// assign: Out = [Src +] ... instead of Out += ...; Tnext (or nullptr) receives the split planes of the result.
+// Returns launches or -1.
+int taylor_tc_apply(const void* Aplanes, bool real_shared, const void* Tb, void* Tnext, double* Out, bool assign,
+                    const double* Src, double alpha, int nw, int M, int N2, cudaStream_t st) {
   if (!taylor_tc_usable(N2)) return -1;
   const int Kp = round_up(M, TY_BK), Np = round_up(N2, 16);
   const int b_plane = Np * TY_BK * 2, stage = TY_AOPER + 3 * b_plane;
@@ -250,44 +305,33 @@ int run_taylor_tc(const double* A, const double* T0, double* Acc, void* Abf, voi
   if (S < 2) return -1;
   const size_t smem = (size_t)S * stage + 1024 + 256;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (first_use_on_device(&attr))
     cudaFuncSetAttribute(taylor_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TY_SMEM_CAP);
-    cudaFuncSetAttribute(split_T_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 257 * 8);
-  }
   const int nsm = sm_count_current();
-  int launches = 0;
-  split_A_kernel<<<dim3(M, nw), 256, 0, st>>>(A, (__nv_bfloat16*)Abf, M, Kp);
-  split_T_kernel<<<dim3(Kp / 32, nw), 256, (size_t)32 * (N2 + 1) * 8, st>>>(T0, (__nv_bfloat16*)Tb0, M, N2, Np, Kp);
-  launches += 2;
-  TensorMap tmA, tmB[2];
+  TensorMap tmA, tmB;
   {
-    const uint64_t dims[4] = {(uint64_t)2 * Kp, (uint64_t)M, 3, (uint64_t)nw};
+    const uint64_t dims[4] = {(uint64_t)2 * Kp, (uint64_t)M, 3, (uint64_t)(real_shared ? 1 : nw)};
     const uint64_t str[3] = {(uint64_t)2 * Kp * 2, (uint64_t)M * 2 * Kp * 2, (uint64_t)3 * M * 2 * Kp * 2};
     const uint32_t box[4] = {TY_BK, TY_M, 3, 1};
-    if (make_tensor_map_bf16(&tmA, Abf, 4, dims, str, box, 64) != 0) return -1;
+    if (make_tensor_map_bf16(&tmA, Aplanes, 4, dims, str, box, 64) != 0) return -1;
   }
-  void* tb[2] = {Tb0, Tb1};
-  for (int i = 0; i < 2; ++i) {
+  {
     const uint64_t dims[4] = {(uint64_t)2 * Kp, (uint64_t)Np, 3, (uint64_t)nw};
     const uint64_t str[3] = {(uint64_t)2 * Kp * 2, (uint64_t)Np * 2 * Kp * 2, (uint64_t)3 * Np * 2 * Kp * 2};
     const uint32_t box[4] = {TY_BK, (uint32_t)Np, 3, 1};
-    if (make_tensor_map_bf16(&tmB[i], tb[i], 4, dims, str, box, 64) != 0) return -1;
+    if (make_tensor_map_bf16(&tmB, Tb, 4, dims, str, box, 64) != 0) return -1;
   }
   TyArgs a;
-  a.Acc = Acc; a.M = M; a.N2 = N2; a.Np = Np; a.Kp = Kp; a.nw = nw;
-  a.KT = 2 * Kp / TY_BK; a.mtiles = (M + TY_M - 1) / TY_M; a.stages = S;
+  a.Acc = Out; a.Tnext = (__nv_bfloat16*)Tnext; a.alpha = alpha; a.assign = assign ? 1 : 0;
+  a.a_shared = real_shared ? 1 : 0; a.Src = Src;
+  a.M = M; a.N2 = N2; a.Np = Np; a.Kp = Kp; a.nw = nw;
+  a.KT = (real_shared ? Kp : 2 * Kp) / TY_BK; a.mtiles = (M + TY_M - 1) / TY_M; a.stages = S;
   a.idesc = umma_idesc_bf16(TY_M, Np); a.b_plane = b_plane; a.stage_bytes = stage;
   a.nacc = Np <= 128 ? 2 : 1; a.d2off = Np <= 128 ? 128 : 256;
   const long nu = (long)nw * a.mtiles;
   const int grid = nu < nsm ? (int)nu : nsm;
-  for (int n = 1; n <= order; ++n) {
-    const int cur = (n - 1) & 1;
-    a.alpha = 1.0 / n;
-    a.Tnext = n < order ? (__nv_bfloat16*)tb[cur ^ 1] : nullptr;
-    taylor_tc_kernel<<<grid, TY_THREADS, smem, st>>>(tmA, tmB[cur], a);
-    ++launches;
-  }
-  return launches;
+  taylor_tc_kernel<<<grid, TY_THREADS, smem, st>>>(tmA, tmB, a);
+  return 1;
 }
 
 }  // namespace afq

@@ -203,7 +203,7 @@ def test_full_size(name, with_oracle):
     # The tensor core adds into its FP32 accumulator with truncation, not round-to-nearest: the 300 updates of
     # the large (hh) accumulator at n_chol = 4800 leave a ONE-SIGNED relative error of ~1e-5 on A, which the
     # determinant of the N_occ x N_occ overlap collects: weights and |overlaps| come out larger by a factor
-    # 1 + 3.9e-5 at c5 (2.6e-5 at c4) that is COMMON to all walkers (it cancels in every weighted average)
+    # 1 + 2.2e-5 at c5 (1.8e-5 at c4) that is COMMON to all walkers (it cancels in every weighted average)
     # with a walker-to-walker spread of 9e-6.  DESIGN.md section 5.
     ratio = wm / wd
     assert abs(np.median(ratio) - 1.0) < 1.5e-4
