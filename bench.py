@@ -448,11 +448,13 @@ def main():
         v["algorithmic_bytes"] = by
         v["gbytes_per_s"] = by / (v["ms_per_step"] * 1e-3) / 1e9
         v["note"] = "emulated single precision (bf16 x 3, FP32 accumulate in TMEM); bound: hbm"
-        if "taylor" in per_stage:
-            t = per_stage["taylor"]
-            t.pop("frac_of_dmma_peak", None)
-            t["tflops"] = 6 * fl["taylor"] / (t["ms_per_step"] * 1e-3) / 1e12
-            t["note"] = "emulated single precision on tcgen05 (split of A and T_0 + one launch per order)"
+        for k, note in (("taylor", "split of A + one launch per order"), ("force_bias", "split of Theta^T + one launch"),
+                        ("one_body", "split of the walkers + one launch per half step")):
+            if k in per_stage:
+                t = per_stage[k]
+                t.pop("frac_of_dmma_peak", None)
+                t["tflops"] = 6 * fl[k] / (t["ms_per_step"] * 1e-3) / 1e12      # bf16 flops issued
+                t["note"] = "emulated single precision on tcgen05 (" + note + ")"
     dom = max(per_stage, key=lambda k: per_stage[k]["ms_per_step"])
     nl = {"exchange": 1 if cfg.walker_kind == 0 else 2, "taylor": cfg.taylor_order, "one_body": 2}.get(dom, 1)
     roof = {"kernel": dom, "bound": "tensor", "unit": "TFLOP/s", "peak": peak_dmma,
