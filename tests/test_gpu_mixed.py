@@ -220,3 +220,45 @@ def test_full_size(name, with_oracle):
         assert rel_max(wm[idx], wo) < 1.5e-4
     g.close()
     pr.close()
+
+
+def _random_cases(n, seed):
+    """Seeded random shapes: even M and n_chol (TMA strides), RHF and UHF, occupied blocks 1..48, 1..140 rows."""
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        M = 2 * int(rng.integers(12, 80))
+        uhf = bool(rng.integers(0, 2))
+        na = int(rng.integers(1, min(48, M // 2)))
+        nb = int(rng.integers(1, na + 1)) if uhf else na
+        nchol = 2 * int(rng.integers(5, 120))
+        nw = int(rng.integers(1, 71))
+        out.append(("c2" if uhf else "c1", nw, dict(M=M, n_alpha=na, n_beta=nb, n_chol=nchol)))
+    return out
+
+
+@pytest.mark.parametrize("name,nw,over", _random_cases(10, 20240607) + [
+    ("c2", 3, dict(M=160, n_alpha=64, n_beta=50, n_chol=40)),     # N2 = 228 > 128: one accumulator set in TMEM
+    ("c2", 2, dict(M=150, n_alpha=40, n_beta=33, n_chol=30)),     # N2 = 146
+])
+def test_random_shapes(name, nw, over):
+    """Tile edges of the tcgen05 kernels: ragged 8 x 16 tiles, odd tile counts (a pair with one tile), gamma and
+    k padding, 1..140 rows, N2 from 2 to 228 columns."""
+    _torch()
+    pr = Pair(name, nw=nw, ortho_every=0, **over)
+    o, cfg = pr.oracle, pr.cfg
+    g = _mixed(pr, nw)
+    x = pr.fields(0)
+    w0 = np.linspace(0.5, 1.5, nw)
+    new_o, info = o.propagate(pr.walkers0, x, cfg.dt)
+    Wg, wg, ovg = _step(g, pr.walkers0, w0, x, cfg.dt)
+    A = planar_to_complex(g.debug_read(1), (nw, cfg.M, cfg.M))
+    assert rel_fro(A, info["A"]) < TOL_A
+    X = planar_to_complex(g.debug_read(0), (nw, cfg.n_chol))
+    assert rel_fro(X, info["X"]) < TOL_A
+    assert rel_fro(Wg, new_o) < TOL_STEP
+    _, w_o, ov_o = o.step(pr.walkers0, w0, x, cfg.dt)
+    assert rel_max(ovg, ov_o) < TOL_OVLP
+    assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_OVLP
+    g.close()
+    pr.close()

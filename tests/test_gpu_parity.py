@@ -168,6 +168,46 @@ def test_free_running_parity(name, nw):
     pr.close()
 
 
+# --------------------------------------------------------------------------- random shapes
+def _random_cases(n, seed):
+    rng = np.random.default_rng(seed)
+    out = []
+    for _ in range(n):
+        M = int(rng.integers(8, 150))
+        uhf = bool(rng.integers(0, 2))
+        na = int(rng.integers(1, min(60, M)))
+        nb = int(rng.integers(1, na + 1)) if uhf else na
+        nchol = int(rng.integers(3, 200))
+        nw = int(rng.integers(1, 40))
+        out.append(("c2" if uhf else "c1", nw, dict(M=M, n_alpha=na, n_beta=nb, n_chol=nchol)))
+    return out
+
+
+@pytest.mark.parametrize("name,nw,over", _random_cases(14, 20240611))
+def test_random_shapes(name, nw, over):
+    """Seeded random shapes (odd and even M and n_chol, RHF and UHF, 1..59 occupied columns): one step and the
+    local energy, stage tolerances as above.  Odd M / n_chol take the cp.async kernels, even ones the TMA kernels."""
+    _torch()
+    pr = Pair(name, nw=nw, ortho_every=0, **over)
+    o, g, cfg = pr.oracle, pr.gpu, pr.cfg
+    x = pr.fields(0)
+    w0 = np.linspace(0.5, 1.5, nw)
+    new_o, info = o.propagate(pr.walkers0, x, cfg.dt)
+    Wg, wg, ovg = gpu_step(pr, pr.walkers0, w0, x, cfg.dt)
+    assert rel_fro(planar_to_complex(g.debug_read(0), (nw, cfg.n_chol)), info["X"]) < TOL_STAGE * 10
+    assert rel_fro(planar_to_complex(g.debug_read(1), (nw, cfg.M, cfg.M)), info["A"]) < 1e-11
+    assert rel_fro(Wg, new_o) < TOL_STEP
+    _, w_o, ov_o = o.step(pr.walkers0, w0, x, cfg.dt)
+    assert rel_max(ovg, ov_o) < TOL_STEP
+    assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_STEP
+    E_o = o.local_energy(new_o)
+    E_g = gpu_energy(pr, new_o)
+    sc = energy_scale(o, new_o, E_o)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10
+    pr.close()
+
+
 # --------------------------------------------------------------------------- full sizes
 @pytest.mark.parametrize("name,idx,device_L", [("c3", (0, 129, 255), False),
                                                ("c4", (0, 77, 127), True),
