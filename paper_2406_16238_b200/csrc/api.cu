@@ -258,7 +258,7 @@ int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw)
 
 // One walker step on device buffers (rows a1-a10), stream ordered, no synchronisation.
 // a3 + a4 for the nw walkers whose Theta^T sits in h->ThT (with this handle's Cholesky vectors)
-void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw) {
+int force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw) {
   const int M = h->M, Nt = h->Nt, nc = h->n_chol;
   // a3: X[(w,part)][g] = sum_k ThT[(w,part)][k] Lrot[g][k], split over k
   int nsplit = h->fb_split;
@@ -267,8 +267,8 @@ void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw
     StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
     nsplit = h->fb_tc_nsplit;
     const int r = run_fb_tc(h->ThT, h->Tfb, h->Lrb, h->Xp, nc, (long)2 * h->mwg * nc, 2 * nw, nc, Nt * M, nsplit, h->st);
-    if (r < 0) { h->err = "force bias (mixed precision): tensor map encode failed"; }
-    else h->launches += r;
+    if (r < 0) return fail(h, AFQMC_ERR_CUDA, "force bias (mixed precision): tensor map encode failed");
+    h->launches += r;
   } else {
     StageTimer tm(h, AFQMC_STAGE_FORCE_BIAS);
     GemmArgs g = gemm_args();
@@ -290,6 +290,7 @@ void force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw
     s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
     h->launches += run_field_shift(s, nw, h->st);
   }
+  return AFQMC_OK;
 }
 
 int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
@@ -305,7 +306,10 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
     StageTimer tm(h, AFQMC_STAGE_OVERLAP_THETA);
     h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 0), nw, h->st);
   }
-  force_bias_shift_device(h, x, dt, nw);
+  {
+    const int rc = force_bias_shift_device(h, x, dt, nw);
+    if (rc != AFQMC_OK) return rc;
+  }
   // a5: A[(w,part)][pq] = sum_g Cf[(w,part)][g] L[g][pq]
   if (h->Lb) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
@@ -1228,7 +1232,10 @@ int32_t afqmc_shard_vhs(afqmc_handle* h, const double* aux_local, double dt, int
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
   const int G = h->G, mw = h->maxw, nwg = G * nw;
   const long MM = (long)h->M * h->M;
-  force_bias_shift_device(h, aux_local, dt, nwg);
+  {
+    const int rc = force_bias_shift_device(h, aux_local, dt, nwg);
+    if (rc != AFQMC_OK) return rc;
+  }
   {
     StageTimer tm(h, AFQMC_STAGE_SHARD_EXCHANGE);
     for (int o = 0; o < G; ++o) {

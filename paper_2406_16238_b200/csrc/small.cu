@@ -292,8 +292,8 @@ __global__ void __launch_bounds__(256) gj_kernel(OTArgs a) {
 }
 
 // e1[w][blk] = sum_{i in block, q} hrot[off + i][q] * Theta^T[w][.][off + i][q]; grid (nblk, nw)
-__global__ void __launch_bounds__(256) e1_kernel(OTArgs a) {
-  __shared__ double red[8 * 2];
+__global__ void __launch_bounds__(1024) e1_kernel(OTArgs a) {
+  __shared__ double red[32 * 2];
   const int blk = blockIdx.x, w = blockIdx.y;
   const int ns = a.ns[blk], off = a.off[blk], M = a.M, Nt = a.Nt;
   const double* tr = a.ThT + ((size_t)(w * 2 + 0) * Nt + off) * M;
@@ -551,7 +551,7 @@ static int run_overlap_theta_gemm(const OTArgs& a, int nw, cudaStream_t st) {
   g.M = K2; g.N = M; g.K = K2; g.batch = nw; g.splitK = 1; g.alpha = 1.0;
   launches += run_gemm(GEMM_NK, g, st);
   if (a.want_e1) {
-    e1_kernel<<<dim3(a.nblk, nw), 256, 0, st>>>(a);
+    e1_kernel<<<dim3(a.nblk, nw), 1024, 0, st>>>(a);
     ++launches;
   }
   return launches;
