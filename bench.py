@@ -466,6 +466,18 @@ def main():
             "ms_per_launch": per_stage[dom]["ms_per_step"] / nl,
             "share_of_step": per_stage[dom]["ms_per_step"] / (tmax / K),
             "traffic": NCU_TRAFFIC.get((cfg.name, dom))}
+    # the profiling guide's rule for a dtype without a measured peak: another dtype's measured peak x the
+    # nominal ratio (bf16 burst figure of MEASURED_PEAKS.json x 40 / 2250 for FP64); a weaker denominator
+    # than the DMMA rate measured above, kept beside it for comparison
+    try:
+        with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as f:
+            mp = json.load(f)
+        rule = float(mp["bf16_tflops"]) * 40.0 / 2250.0
+        roof["peak_by_guide_rule"] = rule
+        roof["frac_by_guide_rule"] = (roof["achieved"] / rule) if roof["achieved"] else None
+        roof["hbm_gbs_measured"] = mp.get("hbm_gbs")
+    except (OSError, KeyError, ValueError):
+        pass
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
