@@ -197,6 +197,9 @@ def test_full_size(name, with_oracle):
     x = pr.fields(0)
     w0 = np.linspace(0.5, 1.5, nw)
     Wm, wm, ovm = _step(g, pr.walkers0, w0, x, cfg.dt)
+    for rep in range(12):                  # thousands of pipeline stages per SM and call: same bits every time
+        W2, w2, _ = _step(g, pr.walkers0, w0, x, cfg.dt)
+        assert W2.tobytes() == Wm.tobytes() and w2.tobytes() == wm.tobytes(), rep
     Wd, wd, ovd = _step(pr.gpu, pr.walkers0, w0, x, cfg.dt)
     err = rel_fro(Wm, Wd)
     assert 1e-10 < err < TOL_STEP_FULL
@@ -261,4 +264,32 @@ def test_random_shapes(name, nw, over):
     assert rel_max(ovg, ov_o) < TOL_OVLP
     assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_OVLP
     g.close()
+    pr.close()
+
+
+@pytest.mark.parametrize("mixed", [False, True])
+def test_bitwise_reproducible(mixed):
+    """No atomics, fixed-order reductions, hardware-ordered pipelines: the same call gives the same bits.  A
+    race in a shared-memory ring or in the tensor-memory hand-over would show up here as a flipped bit
+    (the WAR race of DESIGN.md section 7 was found this way at full size)."""
+    torch = _torch()
+    pr = Pair("c3", nw=40, oracle=False, n_chol=600)
+    cfg = pr.cfg
+    g = _mixed(pr, 40) if mixed else pr.gpu
+    x = torch.from_numpy(pr.fields(0)).cuda()
+    ref = None
+    for rep in range(25):
+        W = torch.from_numpy(pr.walkers0).cuda()
+        wt = torch.ones(40, dtype=torch.float64, device="cuda")
+        E = torch.empty((40, 3), dtype=torch.complex128, device="cuda")
+        torch.cuda.synchronize()
+        g.step(W, wt, x, cfg.dt)
+        g.local_energy(W, E)
+        g.sync()
+        out = (W.cpu().numpy().tobytes(), wt.cpu().numpy().tobytes(), E.cpu().numpy().tobytes())
+        if ref is None:
+            ref = out
+        assert out == ref, rep
+    if mixed:
+        g.close()
     pr.close()
