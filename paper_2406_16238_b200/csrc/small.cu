@@ -213,64 +213,68 @@ __global__ void __launch_bounds__(256) gj_kernel(OTArgs a) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const int blk = blockIdx.x, w = blockIdx.y;
   const int ns = a.ns[blk], off = a.off[blk], Nt = a.Nt;
-  const int tid = threadIdx.x;
+  const int tid = threadIdx.x, tx = tid & 31, ty = tid >> 5;
   const int ld2 = 2 * ns;
   double2* Aug = reinterpret_cast<double2*>(smraw);             // [ns][2 ns]
   double2* fcol = Aug + (size_t)ns * ld2;                       // [ns]
   __shared__ int s_piv;
   __shared__ double2 s_det;
   const double2* O = reinterpret_cast<const double2*>(a.Obuf) + (size_t)w * Nt * Nt;
-  for (int idx = tid; idx < ns * ns; idx += blockDim.x) {
-    const int i = idx / ns, j = idx % ns;
-    Aug[i * ld2 + j] = O[(size_t)(off + i) * Nt + off + j];
-    Aug[i * ld2 + ns + j] = make_double2(i == j ? 1.0 : 0.0, 0.0);
-  }
+  for (int i = ty; i < ns; i += 8)
+    for (int j = tx; j < ns; j += 32) {
+      Aug[i * ld2 + j] = O[(size_t)(off + i) * Nt + off + j];
+      Aug[i * ld2 + ns + j] = make_double2(i == j ? 1.0 : 0.0, 0.0);
+    }
   if (tid == 0) s_det = make_double2(1.0, 0.0);
   __syncthreads();
+  // Gauss-Jordan with row pivoting on [O | I]: four barriers per column (pivot found / column c and the pivot
+  // read / rows swapped and scaled / rows eliminated); thread (ty, tx) owns rows ty, ty + 8, ... and columns
+  // tx, tx + 32, ... of the elimination, so no index arithmetic with divisions is needed.
   for (int c = 0; c < ns; ++c) {
-    if (tid < 32) {
+    if (ty == 0) {
       double best = -1.0;
       int bi = c;
-      for (int r = c + tid; r < ns; r += 32) {
-        double2 v = Aug[r * ld2 + c];
-        double m = v.x * v.x + v.y * v.y;
+      for (int r = c + tx; r < ns; r += 32) {
+        const double2 v = Aug[r * ld2 + c];
+        const double m = v.x * v.x + v.y * v.y;
         if (!(m <= best)) { best = m; bi = r; }   // NaN counts as a candidate so it propagates
       }
 #pragma unroll
       for (int o = 16; o > 0; o >>= 1) {
-        double ob = __shfl_down_sync(0xffffffffu, best, o);
-        int oi = __shfl_down_sync(0xffffffffu, bi, o);
+        const double ob = __shfl_down_sync(0xffffffffu, best, o);
+        const int oi = __shfl_down_sync(0xffffffffu, bi, o);
         if (ob > best || (ob == best && oi < bi)) { best = ob; bi = oi; }
       }
-      if (tid == 0) s_piv = bi;
+      if (tx == 0) s_piv = bi;
     }
     __syncthreads();
     const int piv = s_piv;
-    if (piv != c) {
-      for (int j = tid; j < ld2; j += blockDim.x) {
-        double2 u = Aug[c * ld2 + j];
-        Aug[c * ld2 + j] = Aug[piv * ld2 + j];
-        Aug[piv * ld2 + j] = u;
-      }
-      if (tid == 0) s_det = make_double2(-s_det.x, -s_det.y);
-    }
-    __syncthreads();
-    const double2 pv = Aug[c * ld2 + c];
+    const double2 pv = Aug[piv * ld2 + c];         // read by everyone before anyone writes (barrier below)
+    // the eliminated rows need their column-c entries as they are now (row piv will sit in row c after the swap)
+    for (int r = tid; r < ns; r += blockDim.x)
+      if (r != c) fcol[r] = r == piv ? Aug[c * ld2 + c] : Aug[r * ld2 + c];
     __syncthreads();
     const double2 ipv = cinv(pv);
-    if (tid == 0) s_det = cmul(s_det, pv);
-    for (int j = tid; j < ld2; j += blockDim.x) Aug[c * ld2 + j] = cmul(Aug[c * ld2 + j], ipv);
-    for (int r = tid; r < ns; r += blockDim.x)
-      if (r != c) fcol[r] = Aug[r * ld2 + c];
+    if (tid == 0) {
+      double2 d = cmul(s_det, pv);
+      s_det = piv != c ? make_double2(-d.x, -d.y) : d;
+    }
+    // swap rows c and piv and scale the new row c by 1 / pivot, one column per thread
+    for (int j = tid; j < ld2; j += blockDim.x) {
+      const double2 top = Aug[piv * ld2 + j];
+      if (piv != c) Aug[piv * ld2 + j] = Aug[c * ld2 + j];
+      Aug[c * ld2 + j] = cmul(top, ipv);
+    }
     __syncthreads();
-    for (int idx = tid; idx < ns * ld2; idx += blockDim.x) {
-      const int r = idx / ld2, j = idx % ld2;
-      if (r != c) {
-        const double2 f = fcol[r], pc = Aug[c * ld2 + j];
-        double2 v = Aug[idx];
+    for (int r = ty; r < ns; r += 8) {
+      if (r == c) continue;
+      const double2 f = fcol[r];
+      for (int j = tx; j < ld2; j += 32) {
+        const double2 pc = Aug[c * ld2 + j];
+        double2 v = Aug[r * ld2 + j];
         v.x -= f.x * pc.x - f.y * pc.y;
         v.y -= f.x * pc.y + f.y * pc.x;
-        Aug[idx] = v;
+        Aug[r * ld2 + j] = v;
       }
     }
     __syncthreads();
