@@ -201,6 +201,9 @@ def test_full_size(name, with_oracle):
         W2, w2, _ = _step(g, pr.walkers0, w0, x, cfg.dt)
         assert W2.tobytes() == Wm.tobytes() and w2.tobytes() == wm.tobytes(), rep
     Wd, wd, ovd = _step(pr.gpu, pr.walkers0, w0, x, cfg.dt)
+    for rep in range(12):                  # and the double path likewise
+        W2, w2, _ = _step(pr.gpu, pr.walkers0, w0, x, cfg.dt)
+        assert W2.tobytes() == Wd.tobytes() and w2.tobytes() == wd.tobytes(), rep
     err = rel_fro(Wm, Wd)
     assert 1e-10 < err < TOL_STEP_FULL
     # The tensor core adds into its FP32 accumulator with truncation, not round-to-nearest: the 300 updates of
