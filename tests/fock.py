@@ -57,6 +57,21 @@ class Fock:
                                 H = H + 0.5 * eri[p, s, q, r] * (ap_aq @ self.c[s2 * M + r] @ self.c[s1 * M + s])
         return H
 
+    def hamiltonian_eri(self, h, eri):
+        """Eq. (2) for a given (possibly complex) h and four-index tensor eri[p, s, q, r] = (ps|qr)."""
+        M = self.M
+        H = self.one_body(h).astype(np.complex128)
+        for s1 in range(2):
+            for s2 in range(2):
+                for p in range(M):
+                    for q in range(M):
+                        ap_aq = self.cd[s1 * M + p] @ self.cd[s2 * M + q]
+                        for r in range(M):
+                            for s in range(M):
+                                if eri[p, s, q, r] != 0:
+                                    H = H + 0.5 * eri[p, s, q, r] * (ap_aq @ self.c[s2 * M + r] @ self.c[s1 * M + s])
+        return H
+
     def det_state(self, phi_a, phi_b):
         """prod_i (sum_p phi_a[p,i] a+_{p,up}) prod_j (sum_p phi_b[p,j] a+_{p,dn}) |0>."""
         M = self.M
