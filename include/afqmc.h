@@ -80,6 +80,14 @@ typedef struct {
                         /* split upper-triangle tiles (6 bytes per kept element) and, as with        */
                         /* pack_chol, stops borrowing L_chol when afqmc_create returns.  Needs even  */
                         /* M and n_chol.  Results agree with the double path to ~1e-6 relative.      */
+  int32_t complex_chol; /* 1: complex Cholesky vectors.  L_chol is DEVICE complex128     */
+                        /* [n_chol][M][M] with (ps|qr) = sum_g L^g_ps conj(L^g_rq) a (ps|qr) = (qr|ps)      */
+                        /* symmetric tensor, h1 is EITHER complex128 [M][M] Hermitian, the trial stays real. */
+                        /* The handle works with the 2 n_chol Hermitian matrices A_g = (L_g + L_g^+)/2,      */
+                        /* B_g = (L_g - L_g^+)/(2i): aux_fields is [nw][2 n_chol] (fields of the A_g first), */
+                        /* L_chol is not referenced after afqmc_create.  Not combinable with pack_chol,      */
+                        /* mixed_precision or group_size > 1.                                                */
+  int32_t reserved;     /* 0                                                                                   */
 } afqmc_params;
 
 /* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;

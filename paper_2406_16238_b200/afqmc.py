@@ -35,7 +35,8 @@ class AfqmcParams(C.Structure):
                 ("walker_kind", C.c_int32), ("taylor_order", C.c_int32),
                 ("ortho_every", C.c_int32), ("e_shift_auto", C.c_int32),
                 ("e_shift", C.c_double), ("stream", C.c_void_p), ("pack_chol", C.c_int32),
-                ("group_size", C.c_int32), ("group_rank", C.c_int32), ("mixed_precision", C.c_int32)]
+                ("group_size", C.c_int32), ("group_rank", C.c_int32), ("mixed_precision", C.c_int32),
+                ("complex_chol", C.c_int32), ("reserved", C.c_int32)]
 
 
 def _load():
@@ -128,7 +129,7 @@ class AFQMC:
 
     def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
                  walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False,
-                 group_size=0, group_rank=0, mixed_precision=False):
+                 group_size=0, group_rank=0, mixed_precision=False, complex_chol=False):
         p = AfqmcParams()
         p.struct_size = C.sizeof(AfqmcParams)
         p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
@@ -140,8 +141,9 @@ class AFQMC:
         p.pack_chol = 1 if pack_chol else 0
         p.group_size, p.group_rank = int(group_size), int(group_rank)
         p.mixed_precision = 1 if mixed_precision else 0
+        p.complex_chol = 1 if complex_chol else 0
         # L_chol is borrowed by the library (only during create when pack_chol is set)
-        self._keep = (h1, None if (pack_chol or mixed_precision) else L_chol, trial)
+        self._keep = (h1, None if (pack_chol or mixed_precision or complex_chol) else L_chol, trial)
         self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers
         self.Nt = n_alpha if walker_kind == 0 else n_alpha + n_beta
         h = C.c_void_p()

@@ -1,5 +1,6 @@
 // api.cu - the C ABI of libafqmc (include/afqmc.h): handle, setup, and the stream-ordered
 // sequence of kernels that makes one walker step / one local-energy evaluation.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -66,6 +67,13 @@ struct afqmc_handle {
   void *Lb = nullptr, *Ab = nullptr;   // mixed precision: bf16 x 3 split tiles of L, split coefficients
   int* tc_tiles = nullptr;
   int tc_ntile = 0;
+  // complex Cholesky vectors (cplx.cu): n_chol counts the 4n real planes, nf = 2n fields
+  bool cplx = false;
+  int nf = 0;
+  double *Ks = nullptr, *hrot_i = nullptr, *Lrot_sum = nullptr, *E1c = nullptr, *e1i = nullptr, *Xe_s = nullptr;
+  double* expart_c[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [set i / set r+i][spin block]
+  int exgroups_c[2] = {0, 0};
+  std::vector<double> hm_host;                  // h_mod, planar (re, im), for the host expm
   void *Abf = nullptr, *Tb0 = nullptr, *Tb1 = nullptr;   // mixed precision: split A and Taylor terms
   void* E1b = nullptr;                                    // mixed precision: split one-body propagator
   void *Lrb = nullptr, *Tfb = nullptr;                    // mixed precision: split Lrot and Theta^T (force bias)
@@ -181,7 +189,57 @@ GemmArgs gemm_args() {
 
 // E1 = expm(-dt/2 h_mod) by scaling and squaring of a degree-16 Taylor polynomial (Horner),
 // every product on the DMMA GEMM.  (The oracle uses an eigendecomposition instead: reading S6.)
+// complex Hermitian h_mod (complex Cholesky vectors): E1 = expm(-dt/2 h_mod) on the HOST by scaling and squaring
+// of a degree-18 Taylor polynomial, plain O(M^3) complex products (cached per dt; the oracle uses eigh), then
+// uploaded as two planes.  Fine for the M of a few hundred this path is meant for.
+static void cmatmul(const std::vector<double>& A, const std::vector<double>& B, std::vector<double>& C, int M) {
+  const size_t MM = (size_t)M * M;
+  std::fill(C.begin(), C.end(), 0.0);
+  for (int i = 0; i < M; ++i)
+    for (int k = 0; k < M; ++k) {
+      const double ar = A[(size_t)i * M + k], ai = A[MM + (size_t)i * M + k];
+      if (ar == 0.0 && ai == 0.0) continue;
+      const double* br = &B[(size_t)k * M];
+      const double* bi = &B[MM + (size_t)k * M];
+      double* cr = &C[(size_t)i * M];
+      double* ci = &C[MM + (size_t)i * M];
+      for (int j = 0; j < M; ++j) {
+        cr[j] += ar * br[j] - ai * bi[j];
+        ci[j] += ar * bi[j] + ai * br[j];
+      }
+    }
+}
+
+void build_E1_complex(afqmc_handle* h, double dt) {
+  const int M = h->M;
+  const size_t MM = (size_t)M * M;
+  std::vector<double> X(2 * MM), P(2 * MM, 0.0), Q(2 * MM);
+  double n1 = 0.0;
+  for (int c = 0; c < M; ++c) {
+    double cs = 0.0;
+    for (int r = 0; r < M; ++r) cs += hypot(h->hm_host[(size_t)r * M + c], h->hm_host[MM + (size_t)r * M + c]);
+    if (cs > n1) n1 = cs;
+  }
+  double nrm = 0.5 * fabs(dt) * n1;
+  int s = 0;
+  while (nrm > 0.25 && s < 40) { nrm *= 0.5; ++s; }
+  const double f = -0.5 * dt / std::ldexp(1.0, s);
+  for (size_t i = 0; i < 2 * MM; ++i) X[i] = f * h->hm_host[i];
+  for (int i = 0; i < M; ++i) P[(size_t)i * M + i] = 1.0;
+  for (int k = 18; k >= 1; --k) {               // Horner: P <- 1 + X P / k
+    cmatmul(X, P, Q, M);
+    for (size_t i = 0; i < 2 * MM; ++i) Q[i] /= k;
+    for (int i = 0; i < M; ++i) Q[(size_t)i * M + i] += 1.0;
+    P.swap(Q);
+  }
+  for (int i = 0; i < s; ++i) { cmatmul(P, P, Q, M); P.swap(Q); }
+  cudaMemcpyAsync(h->E1c, P.data(), 2 * MM * 8, cudaMemcpyHostToDevice, h->st);
+  cudaStreamSynchronize(h->st);                 // P is a local
+  h->dt_cached = dt;
+}
+
 void build_E1(afqmc_handle* h, double dt) {
+  if (h->cplx) { build_E1_complex(h, dt); return; }
   StageTimer tm(h, AFQMC_STAGE_E1_BUILD);
   const int M = h->M;
   const long MM = (long)M * M;
@@ -248,7 +306,49 @@ int energy_from_theta(afqmc_handle* h, const double* e1, double* E_out, int nw) 
   return AFQMC_OK;
 }
 
+// complex Cholesky vectors: three runs of the exchange kernel (Re planes, Im planes, their sum), cplx.cu
+int local_energy_complex_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
+  const int nf = h->nf;
+  {
+    StageTimer tm(h, AFQMC_STAGE_E_THETA);
+    OTArgs a = ot_args(h, W, h->det_old, 1, 1);
+    h->launches += run_overlap_theta(a, nw, h->st);           // e1 <- Re(h)rot . Theta
+    a.hrot = h->hrot_i; a.e1 = h->e1i;
+    h->launches += run_e1(a, nw, h->st);                      // e1i <- Im(h)rot . Theta
+  }
+  const size_t lsz = (size_t)nf * h->Nt * h->M;
+  const double* lrot[3] = {h->Lrot, h->Lrot + lsz, h->Lrot_sum};
+  double* xe[3] = {h->Xe, h->Xe + (size_t)nf * h->mwg * 2, h->Xe_s};
+  for (int k = 0; k < 3; ++k)
+    for (int b = 0; b < h->nblk; ++b) {
+      StageTimer tm(h, AFQMC_STAGE_EXCHANGE);
+      ExArgs e;
+      e.Lrot = lrot[k]; e.ThT = h->ThT; e.expart = k == 0 ? h->expart[b] : h->expart_c[k - 1][b]; e.X = xe[k];
+      e.M = h->M; e.Nt = h->Nt; e.n_chol = nf; e.nw = nw;
+      e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
+      if (h->ws) {
+        const int r = run_exchange_ws(e, h->st);
+        if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
+        h->launches += r;
+      } else {
+        h->launches += run_exchange(e, h->st);
+      }
+    }
+  StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
+  CEnergyArgs c;
+  c.Xr = xe[0]; c.Xi = xe[1];
+  for (int b = 0; b < 2; ++b) {
+    c.expart[0][b] = h->expart[b]; c.expart[1][b] = h->expart_c[0][b]; c.expart[2][b] = h->expart_c[1][b];
+    c.ngroups[b] = h->exgroups_c[b];
+  }
+  c.e1r = h->e1; c.e1i = h->e1i; c.E_out = E_out;
+  c.nf = nf; c.nw = nw; c.nblk = h->nblk; c.spin_factor = h->sf;
+  h->launches += run_energy_cplx(c, h->st);
+  return AFQMC_OK;
+}
+
 int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
+  if (h->cplx) return local_energy_complex_device(h, W, E_out, nw);
   {
     StageTimer tm(h, AFQMC_STAGE_E_THETA);
     h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
@@ -282,7 +382,14 @@ int force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw)
     h->launches += r > 0 ? r : run_gemm(GEMM_NK, g, h->st);
   }
   // a4: shifted fields, scalars, V_HS coefficients
-  {
+  if (h->cplx) {
+    StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
+    CShiftArgs c;
+    c.Xp = h->Xp; c.sXp = (long)2 * h->mwg * nc; c.nsplit = nsplit; c.m = h->m; c.x = x;
+    c.X = h->X; c.Cf = h->Cf; c.cfb = h->cfb; c.cmf = h->cmf; c.nf = h->nf;
+    c.spin_factor = h->sf; c.sqrt_dt = sqrt(dt);
+    h->launches += run_field_shift_cplx(c, nw, h->st);
+  } else {
     StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
     ShiftArgs s;
     s.Xp = h->Xp; s.sXp = (long)2 * h->mwg * nc; s.nsplit = nsplit; s.m = h->m; s.x = x;
@@ -409,10 +516,18 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
     g.C = h->T0; g.C2 = h->Acc; g.mode = 2; g.ldc = 2 * Nt; g.sC = wstride;
     g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
     int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 2, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+    if (h->cplx) {       // complex E1 (planar): the planar-complex GEMM of the Taylor terms with a shared operand
+      g.A = h->E1c; g.A2 = h->E1c + MM;
+      if (h->ws)
+        r = run_gemm_ws_kn(h->E1c, M, MM, 0, true, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
+                           nw, 1.0, 2, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
+    } else {
+      if (h->ws)
+        r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
+                           nw, 1.0, 2, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+    }
   }
   // a7: T_n = A T_{n-1} / n, Acc += T_n
   {
@@ -438,10 +553,18 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
     g.A = h->E1; g.lda = M; g.sA = 0; g.B = h->Acc; g.ldb = 2 * Nt; g.sB = wstride;
     g.C = W; g.ldc = 2 * Nt; g.sC = wstride; g.M = M; g.N = 2 * Nt; g.K = M; g.batch = nw;
     int r = -1;
-    if (h->ws)
-      r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
-                         nw, 1.0, 0, h->st);
-    h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+    if (h->cplx) {
+      g.A = h->E1c; g.A2 = h->E1c + MM;
+      if (h->ws)
+        r = run_gemm_ws_kn(h->E1c, M, MM, 0, true, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
+                           nw, 1.0, 0, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
+    } else {
+      if (h->ws)
+        r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
+                           nw, 1.0, 0, h->st);
+      h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
+    }
   }
   return finish_step_device(h, W, wt, cfb, cmf, dt, nw);
 }
@@ -465,7 +588,7 @@ int block_body_device(afqmc_handle* h, double* W, double* wt, const double* aux,
                       int n_steps, int pop_every, double* E, double* est) {
   int j = 0;
   for (int s = 0; s < n_steps; ++s) {
-    const int rc = step_device(h, W, wt, aux + (size_t)s * nw * h->n_chol, dt, nw);
+    const int rc = step_device(h, W, wt, aux + (size_t)s * nw * h->nf, dt, nw);
     if (rc != AFQMC_OK) return rc;
     if (pop_every > 0 && (s + 1) % pop_every == 0) population_control_device(h, W, wt, xi + j++, nw);
   }
@@ -563,14 +686,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (!h1 || !L_chol || !trial || !p || !out) return fail(nullptr, AFQMC_ERR_INVALID, "null argument");
   if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
   if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
-      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
+      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->complex_chol != 0 && p->complex_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
     return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
   if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
   if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
   if (p->n_alpha > p->M || p->n_beta > p->M) return fail(nullptr, AFQMC_ERR_DIMS, "more occupied orbitals than basis functions");
   if (p->taylor_order > kMaxTaylor) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "taylor_order > 16");
   if (p->n_alpha > kMaxOcc || p->n_beta > kMaxOcc) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "occupied block > 64 columns");
-  if ((long)p->n_chol * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
+  const bool cplx = p->complex_chol == 1;
+  const int nvec = cplx ? 4 * p->n_chol : p->n_chol;      // real planes the kernels run over
+  if ((long)nvec * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
+  if (cplx && (p->pack_chol || p->mixed_precision || p->group_size > 1))
+    return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "complex_chol cannot be combined with pack_chol, mixed_precision or a group");
   if (!is_device_ptr(L_chol)) return fail(nullptr, AFQMC_ERR_INVALID, "L_chol must be a device pointer");
   const int G = p->group_size > 0 ? p->group_size : 1;
   if (G > kMaxGroup) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "group_size > 8");
@@ -584,7 +711,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (!h) return fail(nullptr, AFQMC_ERR_ALLOC, "host allocation failed");
   h->p = *p;
   h->dev = ldev >= 0 ? ldev : 0;
-  h->M = p->M; h->n_chol = p->n_chol; h->maxw = p->max_walkers;
+  h->M = p->M; h->n_chol = nvec; h->maxw = p->max_walkers;
+  h->cplx = cplx; h->nf = cplx ? 2 * p->n_chol : p->n_chol;
   h->G = G; h->rank = p->group_rank; h->mwg = G * p->max_walkers;
   h->shard_ready = G == 1;
   h->K = p->taylor_order ? p->taylor_order : 6;
@@ -616,10 +744,23 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   };
 
   // ---- host copies of the small inputs, checks, P_tot ------------------------------------
-  std::vector<double> th((size_t)M * Nt), hh((size_t)MM);
-  if (cudaMemcpy(th.data(), trial, th.size() * 8, cudaMemcpyDefault) != cudaSuccess ||
-      cudaMemcpy(hh.data(), h1, hh.size() * 8, cudaMemcpyDefault) != cudaSuccess)
-    return bail(AFQMC_ERR_CUDA, "copy of h1/trial failed");
+  std::vector<double> th((size_t)M * Nt), hh((size_t)MM), hi;
+  if (cudaMemcpy(th.data(), trial, th.size() * 8, cudaMemcpyDefault) != cudaSuccess)
+    return bail(AFQMC_ERR_CUDA, "copy of the trial failed");
+  if (cplx) {                                  // complex Hermitian h1: planes
+    std::vector<double> hc((size_t)2 * MM);
+    if (cudaMemcpy(hc.data(), h1, hc.size() * 8, cudaMemcpyDefault) != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "copy of h1 failed");
+    hi.resize(MM);
+    for (long i = 0; i < MM; ++i) { hh[i] = hc[2 * i]; hi[i] = hc[2 * i + 1]; }
+    // the planes of the 2n Hermitian matrices replace the caller's tensor from here on
+    h->Ks = dalloc(h, (size_t)nvec * MM);
+    if (!h->Ks) return bail(AFQMC_ERR_ALLOC, "device allocation failed (Hermitian planes)");
+    h->launches += run_hermitian_planes(L_chol, h->Ks, M, p->n_chol, h->st);
+    h->L = h->Ks;
+  } else if (cudaMemcpy(hh.data(), h1, hh.size() * 8, cudaMemcpyDefault) != cudaSuccess) {
+    return bail(AFQMC_ERR_CUDA, "copy of h1 failed");
+  }
   for (int b = 0; b < h->nblk; ++b)
     for (int i = 0; i < h->ns[b]; ++i)
       for (int j = i; j < h->ns[b]; ++j) {
@@ -704,9 +845,11 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
       return bail(AFQMC_ERR_CUDA, std::string("setup kernels failed: ") + cudaGetErrorString(cudaPeekAtLastError()));
     double s = 0.0;
-    for (int g = 0; g < nc; ++g) s += mh[g] * mh[g];
+    const int nm = cplx ? h->nf : nc;          // complex: tr(Im K P) = 0, only the nf real planes carry m
+    for (int g = 0; g < nm; ++g) s += mh[g] * mh[g];
     h->E_const = -0.5 * s;
     h->Ec_part = h->E_const;
+    if (cplx) h->hm_host.assign(hm.begin(), hm.end());
     double n1 = 0.0;
     for (int c = 0; c < M; ++c) {
       double cs = 0.0;
@@ -714,6 +857,48 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
       if (cs > n1) n1 = cs;
     }
     h->hmod_norm1 = n1;
+  }
+  if (cplx) {
+    // Im h_mod = Im h1 - 1/2 (Z - Z^T) + sum_g m_g Im K_g,  Z = sum_g (Re K_g)^T (Im K_g)   (cplx.cu, header)
+    const int nf = h->nf;
+    const double* Ki = h->Ks + (size_t)nf * MM;
+    const int tiles = ((M + 127) / 128) * ((M + 127) / 128);
+    int split = (296 + tiles - 1) / tiles;
+    if (split > 32) split = 32;
+    if (split < 1) split = 1;
+    double* part = dalloc(h, (size_t)split * MM);
+    h->hrot_i = dalloc(h, (size_t)Nt * M);
+    h->Lrot_sum = dalloc(h, (size_t)nf * Nt * M);
+    h->E1c = dalloc(h, (size_t)2 * MM);
+    if (!part || !h->hrot_i || !h->Lrot_sum || !h->E1c) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex setup)");
+    GemmArgs g = gemm_args();
+    g.A = h->Ks; g.lda = M; g.B = Ki; g.ldb = M; g.C = part; g.ldc = M;
+    g.M = M; g.N = M; g.K = nf * M; g.splitK = split; g.sCsplit = MM;
+    h->launches += run_gemm(GEMM_KMKN, g, h->st);
+    h->launches += run_sum_mL(Ki, h->m, mL, M, nf, h->st);
+    std::vector<double> zp((size_t)split * MM), mli((size_t)MM);
+    cudaMemcpyAsync(zp.data(), part, zp.size() * 8, cudaMemcpyDeviceToHost, h->st);
+    cudaMemcpyAsync(mli.data(), mL, MM * 8, cudaMemcpyDeviceToHost, h->st);
+    // hrot_i = trial^T Im h1 (Xs is free scratch here); Lrot_sum = Lrot_re + Lrot_im for the cross term of tr(TT)
+    cudaMemcpyAsync(h->Xs, hi.data(), MM * 8, cudaMemcpyHostToDevice, h->st);
+    GemmArgs g2 = gemm_args();
+    g2.A = h->trialT; g2.lda = M; g2.B = h->Xs; g2.ldb = M; g2.C = h->hrot_i; g2.ldc = M;
+    g2.M = Nt; g2.N = M; g2.K = M;
+    h->launches += run_gemm(GEMM_KN, g2, h->st);
+    h->launches += run_add(h->Lrot_sum, h->Lrot, h->Lrot + (size_t)nf * Nt * M, (long)nf * Nt * M, h->st);
+    if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "complex setup kernels failed");
+    h->hm_host.resize((size_t)2 * MM);
+    for (int r = 0; r < M; ++r)
+      for (int c = 0; c < M; ++c) {
+        double z = 0.0, zt = 0.0;
+        for (int k = 0; k < split; ++k) {
+          z += zp[(size_t)k * MM + (size_t)r * M + c];
+          zt += zp[(size_t)k * MM + (size_t)c * M + r];
+        }
+        h->hm_host[MM + (size_t)r * M + c] = hi[(size_t)r * M + c] - 0.5 * (z - zt) + mli[(size_t)r * M + c];
+      }
+    dfree_one(h, part);
   }
   dfree_one(h, dP);
   dfree_one(h, mL);
@@ -772,7 +957,21 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
       !h->Xe || !h->e1 || !h->stW || !h->stWt || !h->stX || !h->stE)
     return bail(AFQMC_ERR_ALLOC, "device allocation failed (workspaces)");
 
-  h->ws_vhs = h->ws && vhs_ws_usable(M, nc, h->L, h->Cf, h->A);
+  h->ws_vhs = !cplx && h->ws && vhs_ws_usable(M, nc, h->L, h->Cf, h->A);   // Im K is antisymmetric: dense route
+  if (cplx) {
+    h->e1i = dalloc(h, (size_t)mw * 2 * 2);
+    h->Xe_s = dalloc(h, (size_t)h->nf * mwg * 2);
+    bool ok = h->e1i && h->Xe_s;
+    for (int b = 0; b < h->nblk; ++b) {
+      const int G = h->ws ? exchange_ws_group_size(h->ns[b]) : exchange_group_size(h->ns[b]);
+      h->exgroups_c[b] = (h->nf + G - 1) / G;
+      for (int k = 0; k < 2; ++k) {
+        h->expart_c[k][b] = dalloc(h, (size_t)h->exgroups_c[b] * mwg * 2);
+        ok = ok && h->expart_c[k][b];
+      }
+    }
+    if (!ok) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex energy buffers)");
+  }
   if (h->ws_vhs) {
     std::vector<int> tl;
     h->vhs_ntile = vhs_ws_tile_list(M, &tl);
@@ -842,10 +1041,10 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   }
   if (G > 1 && !h->ws_vhs) return bail(AFQMC_ERR_UNSUPPORTED, "a distributed Hamiltonian needs the TMA V_HS kernel (16-byte aligned L)");
   h->e_shift = p->e_shift_auto ? h->e_trial : p->e_shift;
-  if (h->Lpk || h->Lb) {             // the dense tensor is not touched after this point
+  if (h->Lpk || h->Lb || h->cplx) {  // the caller's tensor is not touched after this point
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
       return bail(AFQMC_ERR_CUDA, "packing / splitting the Cholesky tensor failed");
-    h->L = nullptr;
+    h->L = h->cplx ? h->Ks : nullptr;
   }
   *out = h;
   return AFQMC_OK;
@@ -865,7 +1064,7 @@ int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double
   const double* x = aux_fields;
   if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
   if (hostWt) { to_device(h, h->stWt, weights, nw); wt = h->stWt; }
-  if (hostX) { to_device(h, h->stX, aux_fields, (size_t)nw * h->n_chol); x = h->stX; }
+  if (hostX) { to_device(h, h->stX, aux_fields, (size_t)nw * h->nf); x = h->stX; }
   {
     const int rc = step_device(h, W, wt, x, dt, nw);
     if (rc != AFQMC_OK) return rc;
@@ -959,7 +1158,7 @@ int32_t afqmc_run_block(afqmc_handle* h, void* walkers, double* weights, const d
   if (!(dt > 0.0) || !std::isfinite(dt)) return fail(h, AFQMC_ERR_INVALID, "dt must be positive");
   const int n_pop = pop_every > 0 ? n_steps / pop_every : 0;
   if (n_pop > 0 && !xi) return fail(h, AFQMC_ERR_INVALID, "xi is needed when pop_every > 0");
-  const int nc = h->n_chol;
+  const int nc = h->nf;
   const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
   const bool hostW = !is_device_ptr(walkers), hostWt = !is_device_ptr(weights), hostX = !is_device_ptr(aux_fields);
   const bool hostXi = n_pop > 0 && !is_device_ptr(xi);
@@ -1033,7 +1232,7 @@ int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out) {
   const long MM = (long)h->M * h->M;
   const int nw = h->last_nw;
   switch (which) {
-    case 0: src = h->X; n = (int64_t)2 * nw * h->n_chol; break;
+    case 0: src = h->X; n = (int64_t)2 * nw * h->nf; break;
     case 1: src = h->A; n = (int64_t)2 * nw * MM; break;
     case 2: src = h->E1; n = MM; break;
     case 3: src = h->hmod; n = MM; break;

@@ -198,6 +198,29 @@ int run_push_e2(double* dst, const double* E, int n, cudaStream_t st);
 int run_energy_finish(double* E_out, const double* e1, const double* const* slots, int G, int nblk, double sf,
                       int nw, cudaStream_t st);
 
+// cplx.cu: complex Cholesky vectors on the real kernels
+struct CShiftArgs {
+  const double* Xp; long sXp; int nsplit;     // [split][2 nw][nv] partial sums over the nv = 2 nf planes
+  const double* m;                            // [nf] (the first nf entries of the mean field of the planes)
+  const double* x;                            // [nw][nf]
+  double *X, *Cf, *cfb, *cmf;                 // X [nw][2][nf]; Cf [nw][2][nv]
+  int nf;
+  double spin_factor, sqrt_dt;
+};
+struct CEnergyArgs {
+  const double* Xr; const double* Xi;         // tr(T) of the Re / Im plane runs, [nf][nw] complex
+  const double* expart[3][2]; int ngroups[2]; // sums of tr(TT) of the runs r, i, r + i per spin block
+  const double* e1r; const double* e1i;       // [nw][nblk] complex: Re(h)rot . Theta, Im(h)rot . Theta
+  double* E_out;
+  int nf, nw, nblk;
+  double spin_factor;
+};
+int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStream_t st);
+int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st);
+int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st);
+int run_energy_cplx(const CEnergyArgs& a, cudaStream_t st);
+int run_e1(const OTArgs& a, int nw, cudaStream_t st);    // small.cu: one-body energy sum only
+
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);
 int run_sum_mL(const double* L, const double* m, double* out, int M, int n_chol, cudaStream_t st);

@@ -561,6 +561,11 @@ static int run_overlap_theta_gemm(const OTArgs& a, int nw, cudaStream_t st) {
   return launches;
 }
 
+int run_e1(const OTArgs& a, int nw, cudaStream_t st) {
+  e1_kernel<<<dim3(a.nblk, nw), 1024, 0, st>>>(a);
+  return 1;
+}
+
 int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st) {
   if (a.Obuf && a.Aop && a.trialT) {
     const int r = run_overlap_theta_gemm(a, nw, st);

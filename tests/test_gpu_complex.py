@@ -1,0 +1,125 @@
+"""GPU parity for complex Cholesky vectors: `complex_chol = 1` against
+oracle/complex_chol_oracle.py (pinned by tests/test_oracle_complex_pins.py), same tolerances as the real path."""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+from paper_2406_16238_b200 import inputs
+from tests.gpu_util import planar_to_complex, rel_fro, rel_max
+
+pytestmark = pytest.mark.gpu
+
+TOL_STEP = 1e-10
+TOL_RUN = 1e-8
+
+
+def _torch():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def _pair(M, na, nb, npairs, kind, nw, seed=0):
+    torch = _torch()
+    from oracle.complex_chol_oracle import ComplexCholOracle
+    from paper_2406_16238_b200 import afqmc
+    h, L, trial, walkers = inputs.make_complex_problem(M, na, nb, npairs, kind, seed, nw)
+    o = ComplexCholOracle(h, L, trial, na, nb, kind)
+    Ld = torch.from_numpy(L).cuda()
+    g = afqmc.AFQMC(h, Ld, trial, M=M, n_alpha=na, n_beta=nb, n_chol=L.shape[0], max_walkers=nw, walker_kind=kind,
+                    complex_chol=True)
+    Ld.fill_(float("nan"))                 # the caller's tensor is not referenced after afqmc_create
+    torch.cuda.synchronize()
+    return o, g, walkers
+
+
+def _step(g, W, wt, x, dt):
+    torch = _torch()
+    Wd = torch.from_numpy(np.ascontiguousarray(W)).cuda()
+    wd = torch.from_numpy(np.ascontiguousarray(wt)).cuda()
+    xd = torch.from_numpy(np.ascontiguousarray(x)).cuda()
+    ov = torch.empty(W.shape[0], dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    g.step(Wd, wd, xd, dt)
+    g.get_overlaps(ov)
+    g.sync()
+    return Wd.cpu().numpy(), wd.cpu().numpy(), ov.cpu().numpy()
+
+
+def _energy(g, W):
+    torch = _torch()
+    Wd = torch.from_numpy(np.ascontiguousarray(W)).cuda()
+    E = torch.empty((W.shape[0], 3), dtype=torch.complex128, device="cuda")
+    torch.cuda.synchronize()
+    g.local_energy(Wd, E)
+    g.sync()
+    return E.cpu().numpy()
+
+
+CASES = [(24, 5, 5, 12, 0, 8), (40, 9, 6, 10, 1, 5), (37, 7, 7, 9, 0, 3), (64, 16, 14, 20, 1, 6)]
+
+
+@pytest.mark.parametrize("M,na,nb,npairs,kind,nw", CASES)
+def test_setup_and_stages(M, na, nb, npairs, kind, nw):
+    o, g, walkers = _pair(M, na, nb, npairs, kind, nw)
+    c = g.constants()
+    assert abs(c["E_const"] - o.E_const) <= 1e-12 * abs(o.E_const)
+    assert abs(c["e_trial"] - o.e_shift) <= 1e-11 * abs(o.e_shift)
+    x = inputs.make_complex_fields(0, 0, nw, o.n_fields)
+    w0 = np.linspace(0.5, 1.5, nw)
+    new_o, info = o.propagate(walkers, x, 0.005)
+    Wg, wg, ovg = _step(g, walkers, w0, x, 0.005)
+    X = planar_to_complex(g.debug_read(0), (nw, o.n_fields))
+    assert rel_fro(X, info["X"]) < 1e-12
+    A = planar_to_complex(g.debug_read(1), (nw, M, M))
+    assert rel_fro(A, info["A"]) < 1e-11
+    assert rel_fro(Wg, new_o) < TOL_STEP
+    _, w_o, ov_o = o.step(walkers, w0, x, 0.005)
+    assert rel_max(ovg, ov_o) < TOL_STEP
+    assert rel_max(wg, w_o, scale=np.maximum(np.abs(w_o), 1e-3)) < TOL_STEP
+    g.close()
+
+
+@pytest.mark.parametrize("M,na,nb,npairs,kind,nw", CASES)
+def test_local_energy(M, na, nb, npairs, kind, nw):
+    o, g, walkers = _pair(M, na, nb, npairs, kind, nw)
+    Eo = o.local_energy(walkers)
+    Eg = _energy(g, walkers)
+    X = o.force_bias_X(o.theta(walkers))
+    ec = 0.5 * np.sum(X * X, axis=1)
+    sc = np.abs(Eo[:, 1]) + np.abs(ec) + np.abs(Eo[:, 2] - ec)
+    for k in range(3):
+        assert rel_max(Eg[:, k], Eo[:, k], scale=sc) < 1e-11
+    assert np.abs(Eo[:, 0].imag).max() > 1e-6          # genuinely complex energies: the cross term matters
+    g.close()
+
+
+def test_free_running():
+    o, g, walkers = _pair(40, 9, 6, 10, 1, 8)
+    Wo, wo = walkers, np.ones(8)
+    Wg, wg = walkers.copy(), np.ones(8)
+    for s in range(10):
+        x = inputs.make_complex_fields(0, s, 8, o.n_fields)
+        Wg, wg, ovg = _step(g, Wg, wg, x, 0.005)
+        Wo, wo, ovo = o.step(Wo, wo, x, 0.005)
+    assert rel_fro(Wg, Wo) < TOL_RUN
+    assert rel_max(wg, wo, scale=np.maximum(np.abs(wo), 1e-3)) < TOL_RUN
+    assert rel_max(ovg, ovo) < TOL_RUN
+    Eo, Eg = o.local_energy(Wo), _energy(g, Wg)
+    assert rel_max(Eg[:, 0], Eo[:, 0], scale=np.abs(Eo[:, 1]) + np.abs(Eo[:, 2])) < TOL_RUN
+    assert wo.min() > 0.05
+    g.close()
+
+
+def test_unsupported_combinations():
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc
+    h, L, trial, _ = inputs.make_complex_problem(24, 5, 5, 4, 0, 0, 2)
+    Ld = torch.from_numpy(L).cuda()
+    kw = dict(M=24, n_alpha=5, n_beta=5, n_chol=L.shape[0], max_walkers=2, walker_kind=0, complex_chol=True)
+    for extra in (dict(pack_chol=True), dict(mixed_precision=True), dict(group_size=2, group_rank=0)):
+        with pytest.raises(afqmc.AfqmcError) as e:
+            afqmc.AFQMC(h, Ld, trial, **kw, **extra)
+        assert e.value.code == -6
