@@ -40,11 +40,22 @@ NCU_TRAFFIC = {
 }
 
 
-def flops_model(cfg, nw):
-    """Algorithmic real FP64 flops per launch of each contraction stage."""
+def flops_model(cfg, nw, complex_fields=0):
+    """Algorithmic real FP64 flops per launch of each contraction stage.
+    complex_fields > 0: complex Cholesky vectors with that many Hermitian matrices (complex x complex products,
+    8 real flops per multiply-add; the exchange stage EXECUTES 1.5x this: three real-plane runs)."""
     M, ng, K = cfg.M, cfg.n_chol, cfg.taylor_order
     blocks = [cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta]
     Nt = sum(blocks)
+    if complex_fields:
+        nf = complex_fields
+        return {
+            "exchange": nw * sum(8.0 * nf * ns * ns * M + 8.0 * nf * ns * ns for ns in blocks),
+            "vhs": nw * 8.0 * nf * M * M,
+            "taylor": nw * 8.0 * K * M * M * Nt,
+            "force_bias": nw * 8.0 * nf * Nt * M,
+            "one_body": 2 * nw * 8.0 * M * M * Nt,
+        }
     return {
         "exchange": nw * sum(4.0 * ng * ns * ns * M + 8.0 * ng * ns * ns for ns in blocks),
         # symmetric half of A only (L_g = L_g^T; SURVEY 8a row a5 "packed-symmetric minimum")
@@ -298,6 +309,9 @@ def main():
     ap.add_argument("--mixed-precision", action="store_true",
                     help="V_HS build in emulated single precision on tcgen05 (afqmc_params.mixed_precision); "
                          "not the headline configuration (north_star: complex128 throughout)")
+    ap.add_argument("--complex-chol", action="store_true",
+                    help="complex Cholesky vectors (afqmc_params.complex_chol) on the workload's shapes: "
+                         "n_chol / 2 complex vectors = n_chol Hermitian matrices = n_chol fields (c1-c3)")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
     ap.add_argument("--group", type=int, default=0,
@@ -334,21 +348,39 @@ def main():
     h1 = inputs.make_h1(cfg, 0)
     trial = inputs.make_trial(cfg, h1, 0)
     want_cpu = (rank == 0 and world == 1 and not args.no_cpu_baseline)
-    Ld, _ = make_L(cfg, 0, False, True)
     stream = torch.cuda.Stream()
-    g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta,
-                    n_chol=cfg.n_chol, max_walkers=nw, walker_kind=cfg.walker_kind,
-                    taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every,
-                    stream=stream.cuda_stream, pack_chol=args.pack_chol,
-                    mixed_precision=args.mixed_precision)
-    if args.pack_chol or args.mixed_precision:
+    cx = None
+    if args.complex_chol:
+        if cfg.n_chol * cfg.M * cfg.M * 8 > (2 << 30):
+            raise SystemExit("--complex-chol: workloads c1-c3 only (host-generated tensor, host-built E1)")
+        hc, Lc, trial, walkers_c = inputs.make_complex_problem(cfg.M, cfg.n_alpha, cfg.n_beta, cfg.n_chol // 4,
+                                                               cfg.walker_kind, seed, nw)
+        cx = dict(h=hc, L=Lc, walkers=walkers_c, nf=2 * Lc.shape[0])
+        h1 = hc
+        Ld = torch.from_numpy(Lc).cuda()
+        g = afqmc.AFQMC(hc, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=Lc.shape[0],
+                        max_walkers=nw, walker_kind=cfg.walker_kind, taylor_order=cfg.taylor_order,
+                        ortho_every=cfg.ortho_every, stream=stream.cuda_stream, complex_chol=True)
+        args.no_block = True
+    else:
+        Ld, _ = make_L(cfg, 0, False, True)
+        g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta,
+                        n_chol=cfg.n_chol, max_walkers=nw, walker_kind=cfg.walker_kind,
+                        taylor_order=cfg.taylor_order, ortho_every=cfg.ortho_every,
+                        stream=stream.cuda_stream, pack_chol=args.pack_chol,
+                        mixed_precision=args.mixed_precision)
+    if args.pack_chol or args.mixed_precision or args.complex_chol:
         Ld = None
         torch.cuda.empty_cache()
     hbm_resident_gb = (torch.cuda.mem_get_info()[1] - torch.cuda.mem_get_info()[0]) / 1e9
     peak_dmma, peak_dfma, _ = afqmc.measure_fp64_peak(200.0)
 
-    walkers_h = inputs.make_walkers(cfg, trial, seed, nw)
-    xs_h = np.stack([inputs.make_aux_fields(cfg, seed, s, nw) for s in range(Wm + K)])
+    if cx:
+        walkers_h = cx["walkers"]
+        xs_h = np.stack([inputs.make_complex_fields(seed, s, nw, cx["nf"]) for s in range(Wm + K)])
+    else:
+        walkers_h = inputs.make_walkers(cfg, trial, seed, nw)
+        xs_h = np.stack([inputs.make_aux_fields(cfg, seed, s, nw) for s in range(Wm + K)])
     with torch.cuda.stream(stream):
         W = torch.from_numpy(walkers_h).cuda()
         wt = torch.ones(nw, dtype=torch.float64, device="cuda")
@@ -430,7 +462,7 @@ def main():
         return
 
     # ---- roofline of the dominant kernel -------------------------------------------------------
-    fl = flops_model(cfg, nw)
+    fl = flops_model(cfg, nw, cx["nf"] if cx else 0)
     per_stage = {k: {"ms_per_step": v[0] / K, "launches": v[1]} for k, v in stages.items() if v[1]}
     for k, f in fl.items():
         if k in per_stage and per_stage[k]["ms_per_step"] > 0:
@@ -487,7 +519,8 @@ def main():
                    "n_chol": cfg.n_chol, "n_walkers_per_gpu": nw, "dt": cfg.dt,
                    "taylor_order": cfg.taylor_order, "ortho_every": cfg.ortho_every,
                    "local_energy": "every step", "parallelism": f"replicas x{world}",
-                   "pack_chol": bool(args.pack_chol), "mixed_precision": bool(args.mixed_precision), "hbm_resident_gb": round(hbm_resident_gb, 1),
+                   "pack_chol": bool(args.pack_chol), "mixed_precision": bool(args.mixed_precision),
+                   "complex_chol": bool(args.complex_chol), "hbm_resident_gb": round(hbm_resident_gb, 1),
                    "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "stages": per_stage, "block": block,
@@ -496,11 +529,26 @@ def main():
                   "weights_max": float(wt_last.max())},
     }
 
-    if args.group > 1 and world == 1:
+    if args.group > 1 and world == 1 and not cx:
         if Ld is None:
             Ld, _ = make_L(cfg, 0, False, True)
         line["distributed_hamiltonian"] = time_sharded(cfg, h1, Ld, trial, args.group, K, Wm, seed)
 
+    if want_cpu and cx:
+        from oracle.complex_chol_oracle import ComplexCholOracle
+        g.close()
+        nw_s = 2
+        t0 = time.perf_counter()
+        o = ComplexCholOracle(cx["h"], cx["L"], trial, cfg.n_alpha, cfg.n_beta, cfg.walker_kind,
+                              taylor_order=cfg.taylor_order, check=False)
+        t1 = time.perf_counter()
+        Wn, wn, _ = o.step(cx["walkers"][:nw_s], np.ones(nw_s), xs_h[0][:nw_s], cfg.dt)
+        o.local_energy(Wn)
+        sec = time.perf_counter() - t1
+        line["cpu_baseline"] = {"value": nw_s / sec, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+                                "sample": f"{nw_s} of {nw} walkers x 1 step (step + local energy), {sec:.1f} s "
+                                          f"(+ {t1 - t0:.1f} s setup), oracle/complex_chol_oracle.py"}
+        want_cpu = False
     if want_cpu:
         g.close()
         if Ld is None:
