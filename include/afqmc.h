@@ -85,7 +85,8 @@ typedef struct {
                         /* symmetric tensor, h1 is EITHER complex128 [M][M] Hermitian, the trial stays real. */
                         /* The handle works with the 2 n_chol Hermitian matrices A_g = (L_g + L_g^+)/2,      */
                         /* B_g = (L_g - L_g^+)/(2i): aux_fields is [nw][2 n_chol] (fields of the A_g first), */
-                        /* L_chol is not referenced after afqmc_create.  Not combinable with pack_chol,      */
+                        /* L_chol is not referenced after afqmc_create; a set that does not factorise a      */
+                        /* symmetric tensor is rejected (AFQMC_ERR_INVALID).  Not combinable with pack_chol, */
                         /* mixed_precision or group_size > 1.                                                */
   int32_t reserved;     /* 0                                                                                   */
 } afqmc_params;

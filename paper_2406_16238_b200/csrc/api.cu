@@ -899,6 +899,43 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
         h->hm_host[MM + (size_t)r * M + c] = hi[(size_t)r * M + c] - 0.5 * (z - zt) + mli[(size_t)r * M + c];
       }
     dfree_one(h, part);
+    // The derivation needs sum_g (B_g x A_g - A_g x B_g) = 0 (a tensor with (ps|qr) = (qr|ps)).  Probe it with two
+    // random Hermitian matrices U, V:  sum_g [tr(B_g U) tr(A_g V) - tr(A_g U) tr(B_g V)] must vanish, where
+    // tr(K U) = sum Re K . Re U + sum Im K . Im U for Hermitian K, U.
+    {
+      const int n = p->n_chol;
+      std::vector<double> pr((size_t)2 * MM), tr_all((size_t)4 * nc);
+      double* probe = dalloc(h, 2 * MM);
+      double* tro = dalloc(h, (size_t)4 * nc);
+      if (!probe || !tro) return bail(AFQMC_ERR_ALLOC, "device allocation failed (symmetry probe)");
+      uint64_t lcg = 0x9E3779B97F4A7C15ull;
+      auto rnd = [&]() { lcg = lcg * 6364136223846793005ull + 1442695040888963407ull; return ((lcg >> 11) * (1.0 / 9007199254740992.0)) - 0.5; };
+      for (int t = 0; t < 2; ++t) {
+        for (int r = 0; r < M; ++r)
+          for (int c = r; c < M; ++c) {
+            const double a = rnd(), b = r == c ? 0.0 : rnd();
+            pr[(size_t)r * M + c] = pr[(size_t)c * M + r] = a;                      // Re U symmetric
+            pr[MM + (size_t)r * M + c] = b; pr[MM + (size_t)c * M + r] = -b;         // Im U antisymmetric
+          }
+        cudaMemcpyAsync(probe, pr.data(), 2 * MM * 8, cudaMemcpyHostToDevice, h->st);
+        h->launches += run_mean_field(h->Ks, probe, tro + (size_t)(2 * t) * nc, M, nc, h->st);          // . Re U
+        h->launches += run_mean_field(h->Ks, probe + MM, tro + (size_t)(2 * t + 1) * nc, M, nc, h->st); // . Im U
+        cudaStreamSynchronize(h->st);
+      }
+      cudaMemcpy(tr_all.data(), tro, tr_all.size() * 8, cudaMemcpyDeviceToHost);
+      // tr(K_g U) = (Re planes . Re U)[g] + (Im planes . Im U)[nf + g]
+      auto trK = [&](int t, int g) { return tr_all[(size_t)(2 * t) * nc + g] + tr_all[(size_t)(2 * t + 1) * nc + nf + g]; };
+      double f = 0.0, scale = 0.0;
+      for (int g = 0; g < n; ++g) {
+        const double aU = trK(0, g), bU = trK(0, n + g), aV = trK(1, g), bV = trK(1, n + g);
+        f += bU * aV - aU * bV;
+        scale += fabs(bU * aV) + fabs(aU * bV);
+      }
+      dfree_one(h, probe);
+      dfree_one(h, tro);
+      if (!(fabs(f) <= 1e-9 * scale + 1e-300))
+        return bail(AFQMC_ERR_INVALID, "complex_chol: the vectors do not factorise a (ps|qr) = (qr|ps) symmetric tensor");
+    }
   }
   dfree_one(h, dP);
   dfree_one(h, mL);

@@ -113,6 +113,18 @@ def test_free_running():
     g.close()
 
 
+def test_vectors_that_are_no_repulsion_integrals_are_rejected():
+    """Half of a {C, C^+} set: sum_g L_ps conj(L_rq) is not (ps|qr) = (qr|ps) symmetric; the oracle refuses it
+    (PC1) and so does the library."""
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc
+    h, L, trial, _ = inputs.make_complex_problem(24, 5, 5, 4, 0, 0, 2)
+    Ld = torch.from_numpy(np.ascontiguousarray(L[:4])).cuda()
+    with pytest.raises(afqmc.AfqmcError) as e:
+        afqmc.AFQMC(h, Ld, trial, M=24, n_alpha=5, n_beta=5, n_chol=4, max_walkers=2, walker_kind=0, complex_chol=True)
+    assert e.value.code == -1 and "symmetric tensor" in str(e.value)
+
+
 def test_unsupported_combinations():
     torch = _torch()
     from paper_2406_16238_b200 import afqmc
