@@ -135,3 +135,38 @@ def test_unsupported_combinations():
         with pytest.raises(afqmc.AfqmcError) as e:
             afqmc.AFQMC(h, Ld, trial, **kw, **extra)
         assert e.value.code == -6
+
+
+def test_block_with_population_control():
+    """afqmc_run_block in the complex mode: 10 steps, the comb every 5, energy and estimator sums, against the
+    plain composition of the complex oracle's step, the (pinned) comb and the estimator sums; then the CUDA-graph
+    replay of the same block gives the same bits."""
+    torch = _torch()
+    from oracle.block_oracle import run_block
+    nw, n_steps, pop_every = 12, 10, 5
+    o, g, walkers = _pair(40, 9, 6, 10, 1, nw)
+    x = np.stack([inputs.make_complex_fields(0, s, nw, o.n_fields) for s in range(n_steps)])
+    xi = inputs.make_pop_uniforms(0, n_steps // pop_every)
+    Wo, wo, ovo, Eo, est_o, maps = run_block(o, walkers, np.ones(nw), x, xi, 0.005, pop_every)
+    xd, xid = torch.from_numpy(x).cuda(), torch.from_numpy(xi).cuda()
+    E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
+    est = torch.empty(4, dtype=torch.float64, device="cuda")
+    outs = []
+    for rep in range(4):                   # eager, capture, two replays
+        W = torch.from_numpy(walkers).cuda() if rep == 0 else W.copy_(torch.from_numpy(walkers))
+        w = torch.ones(nw, dtype=torch.float64, device="cuda") if rep == 0 else w.fill_(1.0)
+        torch.cuda.synchronize()
+        g.run_block(W, w, xd, xid, 0.005, pop_every, E, est)
+        g.sync()
+        outs.append((W.cpu().numpy().copy(), w.cpu().numpy().copy(), E.cpu().numpy().copy(), est.cpu().numpy().copy()))
+    Wg, wg, Eg, estg = outs[0]
+    assert rel_fro(Wg, Wo) < TOL_RUN
+    assert rel_max(wg, wo) < TOL_RUN
+    sc = np.abs(Eo[:, 1]) + np.abs(Eo[:, 2])
+    assert rel_max(Eg[:, 0], Eo[:, 0], scale=sc) < TOL_RUN
+    assert abs(estg[0] / estg[1] - est_o[0] / est_o[1]) < TOL_RUN * np.mean(sc)
+    for other in outs[1:]:
+        for a, b in zip(outs[0], other):
+            assert np.array_equal(a, b)
+    assert g.set_block_graph(-1) >= 2
+    g.close()
