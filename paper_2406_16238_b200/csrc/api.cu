@@ -70,6 +70,7 @@ struct afqmc_handle {
   // complex Cholesky vectors (cplx.cu): n_chol counts the 4n real planes, nf = 2n fields
   bool cplx = false;
   int nf = 0;
+  double* A2 = nullptr;                         // complex: antisymmetric part of V_HS before the sign fix
   double *Ks = nullptr, *hrot_i = nullptr, *Lrot_sum = nullptr, *E1c = nullptr, *e1i = nullptr, *Xe_s = nullptr;
   double* expart_c[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [set i / set r+i][spin block]
   int exgroups_c[2] = {0, 0};
@@ -424,6 +425,17 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
     const int r = run_vhs_tc(h->Cf, h->Ab, h->Lb, Cb, 1, 2 * nw, h->tc_tiles, h->tc_ntile, M, nc, h->st);
     if (r < 0) return fail(h, AFQMC_ERR_CUDA, "vhs (mixed precision): tensor map encode failed");
     h->launches += r;
+  } else if (h->cplx && h->A2) {
+    StageTimer tm(h, AFQMC_STAGE_VHS);
+    const int nf = h->nf;
+    double* Cb1[1] = {h->A};
+    double* Cb2[1] = {h->A2};
+    const int r1 = run_vhs_ws_scatter(h->Cf, h->Ks, Cb1, 1, 2 * nw, h->vhs_tiles, h->vhs_ntile, M, nf, false, h->st, nc);
+    const int r2 = run_vhs_ws_scatter(h->Cf + nf, h->Ks + (size_t)nf * MM, Cb2, 1, 2 * nw, h->vhs_tiles, h->vhs_ntile, M, nf,
+                                      false, h->st, nc);
+    if (r1 < 0 || r2 < 0) return fail(h, AFQMC_ERR_CUDA, "vhs (complex): tensor map encode failed");
+    h->launches += r1 + r2;
+    h->launches += run_add_antisym(h->A, h->A2, 2 * nw, M, h->st);
   } else if (h->ws_vhs) {
     StageTimer tm(h, AFQMC_STAGE_VHS);
     const int r = run_vhs_ws(h->Cf, h->Lpk ? h->Lpk : h->L, h->A, h->vhs_tiles, h->vhs_ntile, M, nc, 2 * nw,
@@ -995,6 +1007,16 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     return bail(AFQMC_ERR_ALLOC, "device allocation failed (workspaces)");
 
   h->ws_vhs = !cplx && h->ws && vhs_ws_usable(M, nc, h->L, h->Cf, h->A);   // Im K is antisymmetric: dense route
+  if (cplx && h->ws && vhs_ws_usable(M, h->nf, h->L, h->Cf, h->A)) {
+    // V_HS as two symmetric-half runs: Re planes (symmetric sum) and Im planes (antisymmetric sum, sign fixed below)
+    std::vector<int> tl;
+    h->vhs_ntile = vhs_ws_tile_list(M, &tl);
+    h->vhs_tiles = (int*)dalloc(h, (tl.size() + 1) / 2 + 1);
+    h->A2 = dalloc(h, (size_t)mw * 2 * MM);
+    if (!h->vhs_tiles || !h->A2) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex V_HS)");
+    if (cudaMemcpy(h->vhs_tiles, tl.data(), tl.size() * sizeof(int), cudaMemcpyHostToDevice) != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "tile list upload failed");
+  }
   if (cplx) {
     h->e1i = dalloc(h, (size_t)mw * 2 * 2);
     h->Xe_s = dalloc(h, (size_t)h->nf * mwg * 2);

@@ -40,6 +40,15 @@ __global__ void axpy_kernel(double* dst, const double* a, const double* b, long 
   if (i < n) dst[i] = a[i] + b[i];
 }
 
+__global__ void add_antisym_kernel(double* A, const double* B, long MM, int M, long total) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= total) return;
+  const long e = i % MM;
+  const int p = (int)(e / M), q = (int)(e % M);
+  if (q > p) A[i] += B[i];
+  else if (q < p) A[i] -= B[i];
+}
+
 template <int NV>
 __device__ __forceinline__ void block_sum256(double (&v)[NV], double* scratch /* 8 * NV */) {
 #pragma unroll
@@ -151,6 +160,11 @@ int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStr
 }
 int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st) {
   axpy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(dst, a, b, n);
+  return 1;
+}
+int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st) {
+  const long MM = (long)M * M, total = MM * rows;
+  add_antisym_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(A, B, MM, M, total);
   return 1;
 }
 int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st) {

@@ -145,7 +145,8 @@ int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_de
 // to Cb[r / rows_per_member] + (r % rows_per_member) * M * M (distributed Hamiltonian: the partial
 // V_HS of a walker is stored straight into its owner's receive slot, possibly peer memory)
 int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int nmember, int rows_per_member,
-                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st);
+                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st,
+                       long ldcf = 0);
 // tile-packed upper triangle of L (the paper's pack_chol): [ntile_n][n_chol][8][16]
 size_t vhs_ws_packed_doubles(int ntile_n, int n_chol);
 int run_pack_tiles(const double* L, double* Lpk, const int* tiles_dev, int ntile_n, int M, int n_chol,
@@ -217,6 +218,9 @@ struct CEnergyArgs {
 };
 int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStream_t st);
 int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st);
+// A[r][p][q] += sign(q - p) * B[r][p][q] for `rows` matrices of M x M (B: an antisymmetric sum computed by the
+// symmetric-half V_HS kernel, i.e. correct above the diagonal and mirrored with the wrong sign below)
+int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st);
 int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st);
 int run_energy_cplx(const CEnergyArgs& a, cudaStream_t st);
 int run_e1(const OTArgs& a, int nw, cudaStream_t st);    // small.cu: one-body energy sum only

@@ -227,12 +227,14 @@ bool vhs_ws_usable(int M, int n_chol, const void* L, const void* Cf, const void*
 int run_vhs_ws(const double* Cf, const double* L, double* C, const int* tiles_dev, int ntile_n, int M,
                int n_chol, int rows, bool packed, cudaStream_t st) {
   double* Cb[1] = {C};
-  return run_vhs_ws_scatter(Cf, L, Cb, 1, rows, tiles_dev, ntile_n, M, n_chol, packed, st);
+  return run_vhs_ws_scatter(Cf, L, Cb, 1, rows, tiles_dev, ntile_n, M, n_chol, packed, st, 0);
 }
 
 int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int nmember, int rows_per_member,
-                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st) {
+                       const int* tiles_dev, int ntile_n, int M, int n_chol, bool packed, cudaStream_t st, long ldcf) {
   if (nmember < 1 || nmember > kMaxGroup || rows_per_member < 1) return -1;
+  if (ldcf <= 0) ldcf = n_chol;                  // row stride of Cf (a column block of a wider matrix otherwise)
+  if (ldcf & 1) return -1;
   const int rows = nmember * rows_per_member;
   static uint64_t attr = 0;
   if (first_use_on_device(&attr)) {
@@ -243,7 +245,7 @@ int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int
   TensorMap tmA, tmB;
   {
     const uint64_t dims[2] = {(uint64_t)n_chol, (uint64_t)rows};
-    const uint64_t str[1] = {(uint64_t)n_chol * 8};
+    const uint64_t str[1] = {(uint64_t)ldcf * 8};
     const uint32_t box[2] = {BKv, BMv};
     if (make_tensor_map_f64(&tmA, Cf, 2, dims, str, box) != 0) return -1;
   }
