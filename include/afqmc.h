@@ -181,7 +181,8 @@ int32_t afqmc_get_constants(afqmc_handle* h, double* out3);
  * the force-bias expectation <L_g> of the last step, spin summed), 1 = A = V_HS
  * [nw][2][M][M] (re plane, im plane), 2 = E1 [M][M], 3 = h_mod [M][M], 4 = m [n_chol],
  * 5 = Lrot [n_chol][Nt][M].  Returns the number of doubles written, or a negative code;
- * with out == NULL only returns the count. */
+ * with out == NULL only returns the count.  With complex_chol: 0 = X [nw][2][2 n_chol] (the Hermitian matrices'
+ * expectation values), 4 and 5 refer to the 4 n_chol real planes (Re K_1..Re K_2n, Im K_1..Im K_2n), 3 = Re h_mod. */
 int64_t afqmc_debug_read(afqmc_handle* h, int32_t which, double* out);
 
 /* Number of kernel launches issued by this handle since create (for bench.py). */
