@@ -170,3 +170,27 @@ def test_block_with_population_control():
             assert np.array_equal(a, b)
     assert g.set_block_graph(-1) >= 2
     g.close()
+
+
+def test_create_destroy_releases_device_memory():
+    """Handles of every flavour (double, pack_chol, mixed precision, complex, group member) give their device memory
+    back: free memory after 5 create/destroy rounds equals free memory after the first one."""
+    torch = _torch()
+    from paper_2406_16238_b200 import afqmc
+    cfg, h1, L, trial, _ = inputs.make_problem_host("c1", nw=4)
+    Ld = torch.from_numpy(L).cuda()
+    hc, Lc, tc, _ = inputs.make_complex_problem(24, 5, 5, 6, 0, 0, 4)
+    Lcd = torch.from_numpy(Lc).cuda()
+    kw = dict(M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, max_walkers=4, walker_kind=0)
+
+    def round_trip():
+        for extra in (dict(), dict(pack_chol=True), dict(mixed_precision=True), dict(group_size=2, group_rank=1)):
+            afqmc.AFQMC(h1, Ld, trial, n_chol=cfg.n_chol, **kw, **extra).close()
+        afqmc.AFQMC(hc, Lcd, tc, n_chol=Lc.shape[0], complex_chol=True, **kw).close()
+        torch.cuda.synchronize()
+        return torch.cuda.mem_get_info()[0]
+
+    first = round_trip()
+    for _ in range(4):
+        last = round_trip()
+    assert last == first
