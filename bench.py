@@ -352,7 +352,7 @@ def main():
     cx = None
     if args.complex_chol:
         if cfg.n_chol * cfg.M * cfg.M * 8 > (2 << 30):
-            raise SystemExit("--complex-chol: workloads c1-c3 only (host-generated tensor, host-built E1)")
+            raise SystemExit("--complex-chol: workloads c1-c3 only (the tensor is generated on the host)")
         hc, Lc, trial, walkers_c = inputs.make_complex_problem(cfg.M, cfg.n_alpha, cfg.n_beta, cfg.n_chol // 4,
                                                                cfg.walker_kind, seed, nw)
         cx = dict(h=hc, L=Lc, walkers=walkers_c, nf=2 * Lc.shape[0])

@@ -70,6 +70,7 @@ struct afqmc_handle {
   // complex Cholesky vectors (cplx.cu): n_chol counts the 4n real planes, nf = 2n fields
   bool cplx = false;
   int nf = 0;
+  double *hmod_c = nullptr, *cbuf = nullptr;    // complex: planar h_mod; scratch of the complex expm (8 M^2)
   double* A2 = nullptr;                         // complex: antisymmetric part of V_HS before the sign fix
   double *Ks = nullptr, *hrot_i = nullptr, *Lrot_sum = nullptr, *E1c = nullptr, *e1i = nullptr, *Xe_s = nullptr;
   double* expart_c[2][2] = {{nullptr, nullptr}, {nullptr, nullptr}};   // [set i / set r+i][spin block]
@@ -190,52 +191,40 @@ GemmArgs gemm_args() {
 
 // E1 = expm(-dt/2 h_mod) by scaling and squaring of a degree-16 Taylor polynomial (Horner),
 // every product on the DMMA GEMM.  (The oracle uses an eigendecomposition instead: reading S6.)
-// complex Hermitian h_mod (complex Cholesky vectors): E1 = expm(-dt/2 h_mod) on the HOST by scaling and squaring
-// of a degree-18 Taylor polynomial, plain O(M^3) complex products (cached per dt; the oracle uses eigh), then
-// uploaded as two planes.  Fine for the M of a few hundred this path is meant for.
-static void cmatmul(const std::vector<double>& A, const std::vector<double>& B, std::vector<double>& C, int M) {
-  const size_t MM = (size_t)M * M;
-  std::fill(C.begin(), C.end(), 0.0);
-  for (int i = 0; i < M; ++i)
-    for (int k = 0; k < M; ++k) {
-      const double ar = A[(size_t)i * M + k], ai = A[MM + (size_t)i * M + k];
-      if (ar == 0.0 && ai == 0.0) continue;
-      const double* br = &B[(size_t)k * M];
-      const double* bi = &B[MM + (size_t)k * M];
-      double* cr = &C[(size_t)i * M];
-      double* ci = &C[MM + (size_t)i * M];
-      for (int j = 0; j < M; ++j) {
-        cr[j] += ar * br[j] - ai * bi[j];
-        ci[j] += ar * bi[j] + ai * br[j];
-      }
-    }
-}
-
+// complex Hermitian h_mod (complex Cholesky vectors): E1 = expm(-dt/2 h_mod) by scaling and squaring of a
+// degree-18 Taylor polynomial (Horner) on the device, as the real case: every product is the planar-complex
+// DMMA GEMM (A planar, B and C interleaved), with a de-interleave between the squarings.  The oracle uses eigh.
 void build_E1_complex(afqmc_handle* h, double dt) {
+  StageTimer tm(h, AFQMC_STAGE_E1_BUILD);
   const int M = h->M;
-  const size_t MM = (size_t)M * M;
-  std::vector<double> X(2 * MM), P(2 * MM, 0.0), Q(2 * MM);
-  double n1 = 0.0;
-  for (int c = 0; c < M; ++c) {
-    double cs = 0.0;
-    for (int r = 0; r < M; ++r) cs += hypot(h->hm_host[(size_t)r * M + c], h->hm_host[MM + (size_t)r * M + c]);
-    if (cs > n1) n1 = cs;
-  }
-  double nrm = 0.5 * fabs(dt) * n1;
+  const long MM = (long)M * M;
+  double nrm = 0.5 * fabs(dt) * h->hmod_norm1;
   int s = 0;
   while (nrm > 0.25 && s < 40) { nrm *= 0.5; ++s; }
-  const double f = -0.5 * dt / std::ldexp(1.0, s);
-  for (size_t i = 0; i < 2 * MM; ++i) X[i] = f * h->hm_host[i];
-  for (int i = 0; i < M; ++i) P[(size_t)i * M + i] = 1.0;
-  for (int k = 18; k >= 1; --k) {               // Horner: P <- 1 + X P / k
-    cmatmul(X, P, Q, M);
-    for (size_t i = 0; i < 2 * MM; ++i) Q[i] /= k;
-    for (int i = 0; i < M; ++i) Q[(size_t)i * M + i] += 1.0;
-    P.swap(Q);
+  double* X = h->cbuf;              // planar scaled argument   [2][MM]
+  double* P = h->cbuf + 2 * MM;     // interleaved              [M][2M]
+  double* Q = h->cbuf + 4 * MM;     // interleaved
+  double* Pp = h->cbuf + 6 * MM;    // planar copy of P for the squarings
+  h->launches += run_scale_copy(X, h->hmod_c, -0.5 * dt / std::ldexp(1.0, s), 2 * MM, h->st);
+  h->launches += run_fill(P, 0.0, 2 * MM, h->st);
+  h->launches += run_caxpby_identity(P, 0.0, 1.0, M, h->st);
+  auto cgemm = [&](const double* Apl, const double* B, double* C, double alpha) {
+    GemmArgs g = gemm_args();
+    g.A = Apl; g.A2 = Apl + MM; g.lda = M; g.B = B; g.ldb = 2 * M; g.C = C; g.ldc = 2 * M;
+    g.M = M; g.N = 2 * M; g.K = M; g.alpha = alpha;
+    h->launches += run_gemm(GEMM_CPLX_KN, g, h->st);
+  };
+  for (int k = 18; k >= 1; --k) {                 // Horner: P <- 1 + X P / k
+    cgemm(X, P, Q, 1.0 / k);
+    h->launches += run_caxpby_identity(Q, 1.0, 1.0, M, h->st);
+    std::swap(P, Q);
   }
-  for (int i = 0; i < s; ++i) { cmatmul(P, P, Q, M); P.swap(Q); }
-  cudaMemcpyAsync(h->E1c, P.data(), 2 * MM * 8, cudaMemcpyHostToDevice, h->st);
-  cudaStreamSynchronize(h->st);                 // P is a local
+  for (int i = 0; i < s; ++i) {
+    h->launches += run_deinterleave(Pp, P, M, h->st);
+    cgemm(Pp, P, Q, 1.0);
+    std::swap(P, Q);
+  }
+  h->launches += run_deinterleave(h->E1c, P, M, h->st);
   h->dt_cached = dt;
 }
 
@@ -910,6 +899,19 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
         }
         h->hm_host[MM + (size_t)r * M + c] = hi[(size_t)r * M + c] - 0.5 * (z - zt) + mli[(size_t)r * M + c];
       }
+    h->hmod_c = dalloc(h, (size_t)2 * MM);
+    h->cbuf = dalloc(h, (size_t)8 * MM);
+    if (!h->hmod_c || !h->cbuf) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex expm)");
+    cudaMemcpy(h->hmod_c, h->hm_host.data(), (size_t)2 * MM * 8, cudaMemcpyHostToDevice);
+    {   // 1-norm of the complex h_mod for the scaling
+      double n1 = 0.0;
+      for (int c = 0; c < M; ++c) {
+        double cs = 0.0;
+        for (int r = 0; r < M; ++r) cs += hypot(h->hm_host[(size_t)r * M + c], h->hm_host[MM + (size_t)r * M + c]);
+        if (cs > n1) n1 = cs;
+      }
+      h->hmod_norm1 = n1;
+    }
     dfree_one(h, part);
     // The derivation needs sum_g (B_g x A_g - A_g x B_g) = 0 (a tensor with (ps|qr) = (qr|ps)).  Probe it with two
     // random Hermitian matrices U, V:  sum_g [tr(B_g U) tr(A_g V) - tr(A_g U) tr(B_g V)] must vanish, where

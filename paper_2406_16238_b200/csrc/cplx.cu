@@ -12,6 +12,8 @@
 //   energy_cplx_kernel        E_C = 1/2 sum X^2;  E_X = -1/2 sum tr(T T) with T = T_r + i T_i:
 //                             tr(T T) = tr(T_r T_r) - tr(T_i T_i) + i [tr((T_r + T_i)^2) - tr(T_r T_r) - tr(T_i T_i)]
 //                             (three runs of the exchange kernel: Lrot_r, Lrot_i and Lrot_r + Lrot_i)
+//   add_antisym_kernel        sign fix of the antisymmetric part of V_HS computed by the symmetric-half kernel
+//   deinterleave / caxpby_identity   helpers of the complex expm(-dt/2 h_mod) (api.cu: build_E1_complex)
 #include "internal.h"
 
 namespace afq {
@@ -47,6 +49,22 @@ __global__ void add_antisym_kernel(double* A, const double* B, long MM, int M, l
   const int p = (int)(e / M), q = (int)(e % M);
   if (q > p) A[i] += B[i];
   else if (q < p) A[i] -= B[i];
+}
+
+// planar [2][M][M] <- interleaved [M][2M]
+__global__ void deinterleave_kernel(double* planar, const double* inter, long MM) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= MM) return;
+  planar[i] = inter[2 * i];
+  planar[MM + i] = inter[2 * i + 1];
+}
+// interleaved complex M x M: P = a P + idval 1
+__global__ void caxpby_identity_kernel(double* P, double a, double idval, int M) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= (long)M * M) return;
+  const int r = (int)(i / M), c = (int)(i % M);
+  P[2 * i] = a * P[2 * i] + (r == c ? idval : 0.0);
+  P[2 * i + 1] = a * P[2 * i + 1];
 }
 
 template <int NV>
@@ -165,6 +183,16 @@ int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t 
 int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st) {
   const long MM = (long)M * M, total = MM * rows;
   add_antisym_kernel<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(A, B, MM, M, total);
+  return 1;
+}
+int run_deinterleave(double* planar, const double* inter, int M, cudaStream_t st) {
+  const long MM = (long)M * M;
+  deinterleave_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, st>>>(planar, inter, MM);
+  return 1;
+}
+int run_caxpby_identity(double* P, double a, double idval, int M, cudaStream_t st) {
+  const long MM = (long)M * M;
+  caxpby_identity_kernel<<<(unsigned)((MM + 255) / 256), 256, 0, st>>>(P, a, idval, M);
   return 1;
 }
 int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st) {

@@ -221,6 +221,8 @@ int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t 
 // A[r][p][q] += sign(q - p) * B[r][p][q] for `rows` matrices of M x M (B: an antisymmetric sum computed by the
 // symmetric-half V_HS kernel, i.e. correct above the diagonal and mirrored with the wrong sign below)
 int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st);
+int run_deinterleave(double* planar, const double* inter, int M, cudaStream_t st);       // [2][M][M] <- [M][2M]
+int run_caxpby_identity(double* P, double a, double idval, int M, cudaStream_t st);    // interleaved complex P
 int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st);
 int run_energy_cplx(const CEnergyArgs& a, cudaStream_t st);
 int run_e1(const OTArgs& a, int nw, cudaStream_t st);    // small.cu: one-body energy sum only
