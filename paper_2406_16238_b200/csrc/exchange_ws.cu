@@ -259,27 +259,33 @@ Plan make_plan(int ns) {
     p.eff = (double)(p.G * ns) * (p.Wn * 2 * ns) / ((double)TA * TB);
     const int RAp = (p.G * ns + 7) & ~7;
     const size_t fixed = 256 * 4 * 8 + 2 * 8 * 8 + 1024;   // comb + barriers + alignment slack
+    // The staging shape with the FEWEST epilogue passes first (Wp walkers of the tile at a time), then the deepest
+    // ring that still fits beside it.  Measured on B200: the operands come out of L2 and two stages already keep
+    // the DMMA pipe fed, while every extra epilogue pass costs three CTA-wide barriers (c2: 5 passes with 4 stages
+    // 4.26 ms, 2 passes with 2 stages 3.4 ms; c5 and c4 keep 3 stages and 2 passes).
     bool ok = false;
-    for (int S = 4; S >= 2 && !ok; --S) {
+    int best_passes = 1 << 30;
+    for (int S = 4; S >= 2; --S) {
       const size_t pipe = (size_t)S * (TA + TB) * 128;
       for (int Wp = p.Wn; Wp >= 1; --Wp) {
-        // items per pass must fit the comb table
         const int ldt = (Wp * 2 * ns) | 1;
         const size_t tot = pipe + (size_t)RAp * ldt * 8 + fixed;
-        if (tot <= (size_t)kSmemMax) {
-          p.stages = S; p.Wp = Wp; p.ldt = ldt; p.smem = tot; ok = true;
-          break;
+        if (tot > (size_t)kSmemMax) continue;
+        int split = 1, wp = Wp;
+        while (p.G * wp * split < ncw && split < 8) split *= 2;
+        while (p.G * wp * split > 256 && wp > 1) wp -= 1;      // items per pass must fit the comb table
+        if (p.G * wp * split > 256) continue;
+        const int passes = (p.Wn + wp - 1) / wp;
+        if (passes < best_passes) {             // strictly fewer: the deeper ring wins ties (S descends)
+          best_passes = passes;
+          p.stages = S; p.Wp = wp; p.ldt = (wp * 2 * ns) | 1; p.split = split;
+          p.smem = pipe + (size_t)RAp * p.ldt * 8 + fixed;
+          ok = true;
         }
+        break;                                  // smaller Wp only means more passes at this S
       }
     }
     if (!ok) continue;
-    // epilogue work items: at least one per consumer warp, at most the comb table
-    int split = 1;
-    while (p.G * p.Wp * split < ncw && split < 8) split *= 2;
-    while (p.G * p.Wp * split > 256 && p.Wp > 1) p.Wp -= 1;
-    if (p.G * p.Wp * split > 256) continue;
-    p.ldt = (p.Wp * 2 * ns) | 1;
-    p.split = split;
     if (p.eff > best.eff + 1e-9) best = p;
   }
   return best;
