@@ -394,8 +394,6 @@ def main():
         for s in range(Wm):
             one(s)
         g.sync()
-        g.set_profiling(True)
-        g.stage_times(reset=True)
         l0 = g.launch_count()
         barrier()
         torch.cuda.synchronize()
@@ -414,10 +412,25 @@ def main():
         clocks = clk.stop()
         ms = e0.elapsed_time(e1)
         launches = g.launch_count() - l0
-        stages = g.stage_times(reset=True)
-        g.set_profiling(False)
         E_last = E.cpu().numpy()
         wt_last = wt.cpu().numpy()
+        # the per-stage breakdown (roofline of the dominant kernel) comes from a SEPARATE pass over the same K
+        # steps with the library's event brackets on, so that `value` above carries no event-record overhead
+        Wb = torch.from_numpy(walkers_h).cuda()
+        wb = torch.ones(nw, dtype=torch.float64, device="cuda")
+        g.set_profiling(True)
+        g.stage_times(reset=True)
+        p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        p0.record(stream)
+        for s in range(Wm, Wm + K):
+            g.step(Wb, wb, xs[s], cfg.dt)
+            g.local_energy(Wb, E)
+        p1.record(stream)
+        torch.cuda.synchronize()
+        ms_prof = p0.elapsed_time(p1)
+        stages = g.stage_times(reset=True)
+        g.set_profiling(False)
+        del Wb, wb
 
     tmax = max_over_ranks(ms, dist, "cuda")
     value = job_value(world, nw, K, tmax)
@@ -496,7 +509,9 @@ def main():
             "achieved": per_stage[dom].get("tflops"), "frac": per_stage[dom].get("frac_of_dmma_peak"),
             "flops_per_launch": fl.get(dom, 0.0) / nl,
             "ms_per_launch": per_stage[dom]["ms_per_step"] / nl,
-            "share_of_step": per_stage[dom]["ms_per_step"] / (tmax / K),
+            "share_of_step": per_stage[dom]["ms_per_step"] / (ms_prof / K),
+            "timing": "CUDA events of the library's own stage brackets on the launch stream, in a separate pass "
+                      "over the same K steps (%.3f ms per step with the brackets on, %.3f without)" % (ms_prof / K, ms / K),
             "traffic": NCU_TRAFFIC.get((cfg.name, dom))}
     # the profiling guide's rule for a dtype without a measured peak: another dtype's measured peak x the
     # nominal ratio (bf16 burst figure of MEASURED_PEAKS.json x 40 / 2250 for FP64); a weaker denominator
@@ -541,12 +556,13 @@ def main():
         t0 = time.perf_counter()
         o = ComplexCholOracle(cx["h"], cx["L"], trial, cfg.n_alpha, cfg.n_beta, cfg.walker_kind,
                               taylor_order=cfg.taylor_order, check=False)
+        Wn, wn, _ = o.step(cx["walkers"][:nw_s], np.ones(nw_s), xs_h[0][:nw_s], cfg.dt)      # warm-up, untimed
         t1 = time.perf_counter()
-        Wn, wn, _ = o.step(cx["walkers"][:nw_s], np.ones(nw_s), xs_h[0][:nw_s], cfg.dt)
+        Wn, wn, _ = o.step(Wn, wn, xs_h[1 % len(xs_h)][:nw_s], cfg.dt)
         o.local_energy(Wn)
         sec = time.perf_counter() - t1
         line["cpu_baseline"] = {"value": nw_s / sec, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
-                                "sample": f"{nw_s} of {nw} walkers x 1 step (step + local energy), {sec:.1f} s "
+                                "sample": f"{nw_s} of {nw} walkers x 1 step after 1 warm-up step (step + local energy), {sec:.1f} s "
                                           f"(+ {t1 - t0:.1f} s setup), oracle/complex_chol_oracle.py"}
         want_cpu = False
     if want_cpu:
@@ -557,9 +573,11 @@ def main():
         del Ld
         torch.cuda.empty_cache()
         nw_s = sample_walkers(cfg)
-        v, sec, thr = oracle_sample(cfg, h1, Lh, trial, nw_s, 1, 0)
+        # one untimed warm-up step (first-touch page faults of the host tensor, BLAS thread start-up), two timed
+        v, sec, thr = oracle_sample(cfg, h1, Lh, trial, nw_s, 2, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
-                                "sample": f"{nw_s} of {nw} walkers x 1 step (step + local energy), {sec:.1f} s"}
+                                "sample": f"{nw_s} of {nw} walkers x 2 steps after 1 warm-up step (step + local "
+                                          f"energy), {sec:.1f} s per step"}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

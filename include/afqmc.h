@@ -29,8 +29,12 @@
  * L_chol; every entry point switches to that device for the duration of the call, so handles on
  * different devices can be driven from one host thread.  A walker whose overlap with the
  * trial is zero or non-finite is NOT an error: its weight becomes exactly 0 (Eq. 15,
- * reading S10).  One handle per host thread; no global mutable state besides the create
- * error string.
+ * reading S10).
+ *
+ * Threads: a handle may be driven by one host thread at a time; different handles may be driven from
+ * different host threads concurrently.  The only process-wide state is the per-device bookkeeping of
+ * one-off kernel attributes (mutex protected) and the message of a failed afqmc_create, which is kept per
+ * host thread (afqmc_last_error(NULL) returns the calling thread's).
  */
 #ifndef AFQMC_H_
 #define AFQMC_H_
@@ -88,7 +92,10 @@ typedef struct {
                         /* L_chol is not referenced after afqmc_create; a set that does not factorise a      */
                         /* symmetric tensor is rejected (AFQMC_ERR_INVALID).  Not combinable with pack_chol, */
                         /* mixed_precision or group_size > 1.                                                */
-  int32_t reserved;     /* 0                                                                                   */
+  int32_t kernel_path;  /* 0: the TMA warp-specialised kernels wherever the shapes allow (even M), the cp.async    */
+                        /* kernels otherwise.  1: force the cp.async kernels (what odd M runs; lets a test cover   */
+                        /* them at even M on the same inputs).  2: the one-kernel overlap / Theta route instead of */
+                        /* the batched DMMA GEMMs.  Results agree to rounding; ignored for group_size > 1.         */
 } afqmc_params;
 
 /* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;
@@ -103,7 +110,11 @@ typedef struct {
  *          0.51x the dense size at M = 1200) and every later call gives the same bits as with
  *          the dense tensor, so the caller may free L_chol afterwards.
  *   trial  EITHER [M][Nt] real, COPIED.
- *   out    receives the handle; NULL on failure. */
+ *   out    receives the handle; NULL on failure.
+ * Ordering: the handle runs on its own non-blocking stream (or params.stream).  afqmc_create synchronises the
+ * device once on entry, so h1, L_chol and trial may have been written on any stream before the call; for every
+ * LATER call the caller orders its own streams against the handle's (afqmc_sync, or events on params.stream).
+ * max_walkers is at most 65535. */
 int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial,
                      const afqmc_params* p, afqmc_handle** out);
 
@@ -133,7 +144,8 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
  * first j with c_j == W), and every new weight is s.  The overlaps kept in the handle are
  * permuted with the walkers.  If W is not finite or not > 0 nothing changes (identity map).
  *   walkers EITHER complex128 [nw][M][Nt], in/out.   weights EITHER double [nw], in/out.
- *   xi      EITHER one double in [0, 1), drawn by the caller (the library draws no random numbers).
+ *   xi      EITHER one double in [0, 1), drawn by the caller (the library draws no random numbers).  A host value
+ *           outside [0, 1) is rejected (AFQMC_ERR_INVALID); a device value is clamped into [0, 1) (NaN -> 0).
  *   map_out EITHER int32 [nw] or NULL: receives i_k (non-decreasing). */
 int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi,
                                  int32_t nw, int32_t* map_out);
@@ -259,6 +271,10 @@ void afqmc_destroy(afqmc_handle* h);
  * before that. */
 int32_t afqmc_shard_setup_partial(afqmc_handle* h, double* out);
 int32_t afqmc_shard_setup_finish(afqmc_handle* h, const double* sum);
+/* The member-order sum for callers that hold all partials in one place (one process driving G members, or after
+ * an all-gather): out[i] = parts[0][i] + parts[1][i] + ... + parts[n_members-1][i] in exactly that order.
+ *   parts HOST [n_members][n], out HOST [n], n = M*M + 2. */
+int32_t afqmc_shard_setup_reduce(const double* parts, int32_t n_members, int64_t n, double* out);
 
 /* The four exchange buffers of this member, as device addresses: out[0] Theta^T gather buffer
  * [G][nw][2][Nt][M], out[1] V_HS receive slots [G][nw][2][M][M], out[2] scalar slots
@@ -267,7 +283,8 @@ int32_t afqmc_shard_get_buffers(afqmc_handle* h, uint64_t* out4);
 /* CUDA IPC handle (64 bytes, HOST) of buffer `which` (0..3) for members in other processes, and
  * the matching open / close in the importing process (cudaIpcOpenMemHandle / Close). */
 int32_t afqmc_shard_ipc_export(afqmc_handle* h, int32_t which, void* handle64);
-int32_t afqmc_shard_ipc_open(const void* handle64, uint64_t* addr_out);
+/*   h: the importing member (the mapping is made on ITS device); NULL = the current device. */
+int32_t afqmc_shard_ipc_open(afqmc_handle* h, const void* handle64, uint64_t* addr_out);
 int32_t afqmc_shard_ipc_close(uint64_t addr);
 /* addrs HOST [G][4]: the buffers of every member as seen from THIS process (row group_rank
  * must be this handle's own).  The pointers are borrowed until afqmc_destroy. */

@@ -1,8 +1,8 @@
 """CPU oracle for the walker step and local energy with COMPLEX Cholesky vectors.
 
 TEST INFRASTRUCTURE ONLY (same rules as oracle/afqmc_oracle.py: only tests/ may import it; it shares no
-code with the CUDA library).  There is NO CUDA path for this case yet: this file and its pins
-(tests/test_oracle_complex_pins.py) are the groundwork the scope table asks for first.
+code with the CUDA library).  Pins: tests/test_oracle_complex_pins.py (PC1-PC5, CPU); the CUDA path
+(`complex_chol = 1`, csrc/cplx.cu) is compared with this file in tests/test_gpu_complex.py.
 
 Source: /root/reference/PAPER.md Sec. IV.B, PAPER.md:326-328 ("Support of complex Cholesky vectors ... the
 number of auxiliary fields is hence twice as many as the number of Cholesky vectors.  The implementation

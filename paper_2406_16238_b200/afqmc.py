@@ -22,7 +22,7 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_set_block_graph", "afqmc_shard_setup_partial", "afqmc_shard_setup_finish",
            "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
            "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
-           "afqmc_shard_energy", "afqmc_shard_energy_finish"]
+           "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce"]
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
           "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
@@ -36,7 +36,7 @@ class AfqmcParams(C.Structure):
                 ("ortho_every", C.c_int32), ("e_shift_auto", C.c_int32),
                 ("e_shift", C.c_double), ("stream", C.c_void_p), ("pack_chol", C.c_int32),
                 ("group_size", C.c_int32), ("group_rank", C.c_int32), ("mixed_precision", C.c_int32),
-                ("complex_chol", C.c_int32), ("reserved", C.c_int32)]
+                ("complex_chol", C.c_int32), ("kernel_path", C.c_int32)]
 
 
 def _load():
@@ -80,12 +80,14 @@ def _load():
     u64 = C.c_uint64
     for name, args in [("afqmc_shard_setup_partial", [vp, vp]), ("afqmc_shard_setup_finish", [vp, vp]),
                        ("afqmc_shard_get_buffers", [vp, vp]), ("afqmc_shard_ipc_export", [vp, i32, vp]),
-                       ("afqmc_shard_ipc_open", [vp, vp]), ("afqmc_shard_ipc_close", [u64]),
+                       ("afqmc_shard_ipc_open", [vp, vp, vp]), ("afqmc_shard_ipc_close", [u64]),
                        ("afqmc_shard_set_peers", [vp, vp]), ("afqmc_shard_theta", [vp, vp, i32, i32]),
                        ("afqmc_shard_vhs", [vp, vp, dbl, i32]), ("afqmc_shard_propagate", [vp, vp, vp, dbl, i32]),
                        ("afqmc_shard_energy", [vp, i32]), ("afqmc_shard_energy_finish", [vp, vp, i32])]:
         getattr(lib, name).argtypes = args
         getattr(lib, name).restype = i32
+    lib.afqmc_shard_setup_reduce.argtypes = [vp, i32, i64, vp]
+    lib.afqmc_shard_setup_reduce.restype = i32
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
     return lib
@@ -129,7 +131,7 @@ class AFQMC:
 
     def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
                  walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False,
-                 group_size=0, group_rank=0, mixed_precision=False, complex_chol=False):
+                 group_size=0, group_rank=0, mixed_precision=False, complex_chol=False, kernel_path=0):
         p = AfqmcParams()
         p.struct_size = C.sizeof(AfqmcParams)
         p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
@@ -142,6 +144,7 @@ class AFQMC:
         p.group_size, p.group_rank = int(group_size), int(group_rank)
         p.mixed_precision = 1 if mixed_precision else 0
         p.complex_chol = 1 if complex_chol else 0
+        p.kernel_path = int(kernel_path)
         # L_chol is borrowed by the library (only during create when pack_chol is set)
         self._keep = (h1, None if (pack_chol or mixed_precision or complex_chol) else L_chol, trial)
         self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers
@@ -211,6 +214,25 @@ class AFQMC:
         out = np.empty(self.M * self.M + 2)
         self._check(lib.afqmc_shard_setup_partial(self._h, out.ctypes.data))
         return out
+
+    @staticmethod
+    def shard_setup_reduce(parts):
+        """Member-order sum of the partials [G][M*M + 2] (done inside the library)."""
+        a = np.ascontiguousarray(parts, dtype=np.float64)
+        out = np.empty(a.shape[1])
+        rc = lib.afqmc_shard_setup_reduce(a.ctypes.data, a.shape[0], a.shape[1], out.ctypes.data)
+        if rc != 0:
+            raise AfqmcError(rc, "afqmc_shard_setup_reduce")
+        return out
+
+    def shard_ipc_open(self, handle_bytes):
+        """Map a peer's exported buffer on this member's device; returns the device address."""
+        out = np.zeros(1, dtype=np.uint64)
+        hb = np.frombuffer(handle_bytes, dtype=np.uint8).copy()
+        rc = lib.afqmc_shard_ipc_open(self._h, hb.ctypes.data, out.ctypes.data)
+        if rc != 0:
+            raise AfqmcError(rc, lib.afqmc_last_error(None).decode())
+        return int(out[0])
 
     def shard_setup_finish(self, total):
         self._check(lib.afqmc_shard_setup_finish(self._h, _ptr(total)))

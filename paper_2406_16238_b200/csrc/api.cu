@@ -94,7 +94,8 @@ struct afqmc_handle {
   int64_t stage_n[AFQMC_STAGE_COUNT] = {0};
 };
 
-static std::string g_create_err;
+// message of the last failed afqmc_create / handle-less call ON THIS HOST THREAD (afqmc_last_error(NULL))
+static thread_local std::string g_create_err;
 
 namespace {
 
@@ -694,6 +695,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->n_alpha > p->M || p->n_beta > p->M) return fail(nullptr, AFQMC_ERR_DIMS, "more occupied orbitals than basis functions");
   if (p->taylor_order > kMaxTaylor) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "taylor_order > 16");
   if (p->n_alpha > kMaxOcc || p->n_beta > kMaxOcc) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "occupied block > 64 columns");
+  // the per-walker kernels put the walker index in gridDim.y / gridDim.z (limit 65535)
+  if (p->max_walkers > 65535) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "max_walkers > 65535");
+  if (p->kernel_path < 0 || p->kernel_path > 2) return fail(nullptr, AFQMC_ERR_INVALID, "kernel_path must be 0, 1 or 2");
   const bool cplx = p->complex_chol == 1;
   const int nvec = cplx ? 4 * p->n_chol : p->n_chol;      // real planes the kernels run over
   if ((long)nvec * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
@@ -708,6 +712,11 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
 
   const int ldev = device_of(L_chol);
   DevGuard dg_(ldev >= 0 ? ldev : 0);
+  // The inputs may have been produced on ANY stream of the caller (torch fills the 55 GB tensor on its own
+  // stream); the handle's stream is non-blocking, so nothing orders it after them.  Setup is a one-off: drain
+  // the device once so that L_chol, h1 and trial are complete before the first kernel reads them.
+  if (cudaDeviceSynchronize() != cudaSuccess)
+    return fail(nullptr, AFQMC_ERR_CUDA, std::string("device not ready at afqmc_create: ") + cudaGetErrorString(cudaGetLastError()));
   afqmc_handle* h = new (std::nothrow) afqmc_handle();
   if (!h) return fail(nullptr, AFQMC_ERR_ALLOC, "host allocation failed");
   h->p = *p;
@@ -724,9 +733,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->off[1] = p->n_alpha; h->ns[1] = h->rhf ? 0 : p->n_beta;
   h->Nt = h->rhf ? p->n_alpha : p->n_alpha + p->n_beta;
   h->L = L_chol;
-  // TMA needs 16-byte global strides: even M.  AFQMC_LEGACY_KERNELS=1 forces the cp.async
-  // kernels (used by the tests to cover both paths on the same inputs).
-  h->ws = (p->M % 2 == 0) && (G > 1 || getenv("AFQMC_LEGACY_KERNELS") == nullptr);
+  // TMA needs 16-byte global strides: even M.  kernel_path = 1 forces the cp.async kernels that odd M
+  // takes anyway (tests cover both paths on the same inputs); a group always needs the TMA kernels.
+  h->ws = (p->M % 2 == 0) && (G > 1 || p->kernel_path != 1);
   if (p->stream) {
     h->st = (cudaStream_t)p->stream;
   } else {
@@ -982,7 +991,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->Xe = dalloc(h, (size_t)nc * mwg * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
   h->Obuf = dalloc(h, (size_t)mw * Nt * 2 * Nt); h->Aop = dalloc(h, (size_t)mw * 4 * Nt * Nt);
   if (!h->Obuf || !h->Aop) return bail(AFQMC_ERR_ALLOC, "device allocation failed (overlap operands)");
-  h->ot_gemm = h->ws && getenv("AFQMC_OT_KERNEL") == nullptr;   // AFQMC_OT_KERNEL=1: the one-kernel route (tests)
+  h->ot_gemm = h->ws && p->kernel_path != 2;   // kernel_path = 2: the one-kernel overlap / Theta route (tests)
   if (G > 1) {
     h->theta_buf = h->ThT;
     h->a_slots = dalloc(h, (size_t)G * mw * 2 * MM);
@@ -1370,6 +1379,16 @@ int32_t afqmc_shard_setup_partial(afqmc_handle* h, double* out) {
   return check_cuda(h, "afqmc_shard_setup_partial");
 }
 
+int32_t afqmc_shard_setup_reduce(const double* parts, int32_t n_members, int64_t n, double* out) {
+  if (!parts || !out || n_members < 1 || n_members > kMaxGroup || n < 1) return AFQMC_ERR_INVALID;
+  for (int64_t i = 0; i < n; ++i) {
+    double s = parts[i];
+    for (int r = 1; r < n_members; ++r) s += parts[(size_t)r * n + i];     // member order 0 .. G-1
+    out[i] = s;
+  }
+  return AFQMC_OK;
+}
+
 int32_t afqmc_shard_setup_finish(afqmc_handle* h, const double* sum) {
   SHARD_CHECK(h, false);
   if (!sum) return fail(h, AFQMC_ERR_INVALID, "null argument");
@@ -1415,8 +1434,11 @@ int32_t afqmc_shard_ipc_export(afqmc_handle* h, int32_t which, void* handle64) {
   return AFQMC_OK;
 }
 
-int32_t afqmc_shard_ipc_open(const void* handle64, uint64_t* addr_out) {
+int32_t afqmc_shard_ipc_open(afqmc_handle* h, const void* handle64, uint64_t* addr_out) {
   if (!handle64 || !addr_out) return AFQMC_ERR_INVALID;
+  int cur = 0;
+  cudaGetDevice(&cur);
+  DevGuard dg_(h ? h->dev : cur);          // the import is mapped on the importing member's device
   cudaIpcMemHandle_t mh;
   memcpy(&mh, handle64, 64);
   void* p = nullptr;

@@ -43,7 +43,11 @@ __global__ void __launch_bounds__(256) comb_kernel(double* weights, const double
     for (int k = threadIdx.x; k < nw; k += blockDim.x) map[k] = k;
     return;
   }
-  const double xi = *xi_p, spacing = s_spacing;
+  // xi is the caller's uniform in [0, 1); a device-resident value cannot be rejected by the host-side check,
+  // so it is clamped here (NaN -> 0): a tooth can then never leave its own interval of the comb
+  double xi = *xi_p;
+  xi = xi >= 0.0 ? (xi < 1.0 ? xi : 0x1.fffffffffffffp-1) : 0.0;
+  const double spacing = s_spacing;
   const int last = s_last;
   for (int k = threadIdx.x; k < nw; k += blockDim.x) {
     const double tooth = __dmul_rn(__dadd_rn((double)k, xi), spacing);

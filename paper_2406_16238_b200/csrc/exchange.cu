@@ -167,7 +167,7 @@ int launch_ex(const ExArgs& a, cudaStream_t st) {
   using Cfg = ExCfg<NP8, GW, SPLIT>;
   auto kern = exchange_kernel<NP8, GW, SPLIT>;
   static uint64_t done = 0;
-  if (first_use_on_device(&done)) {
+  if (auto once_ = first_use_on_device(&done)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
   }
   dim3 grid(a.nw, (a.n_chol + Cfg::G - 1) / Cfg::G);

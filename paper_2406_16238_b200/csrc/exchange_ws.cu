@@ -296,7 +296,7 @@ int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
   using Cfg = XwsCfg<WM, WN, MI, NI>;
   auto kern = exchange_ws_kernel<WM, WN, MI, NI>;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   }
   const int nsm = sm_count_current();

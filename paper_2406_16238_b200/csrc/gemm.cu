@@ -8,7 +8,7 @@ static int launch_cfg(const GemmArgs& a, cudaStream_t st) {
   using Cfg = GemmCfg<BM, BN, WM, WN, A_KM, B_NK, CPLX, STAGES>;
   auto kern = gemm_dmma_kernel<BM, BN, WM, WN, A_KM, B_NK, CPLX, STAGES>;
   static uint64_t attr_done = 0;
-  if (first_use_on_device(&attr_done)) {
+  if (auto once_ = first_use_on_device(&attr_done)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)Cfg::SMEM);
   }
   dim3 grid((a.N + BN - 1) / BN, (a.M + BM - 1) / BM, a.batch * a.splitK);

@@ -189,7 +189,7 @@ int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, cudaStream_t
   using Cfg = KnCfg<MI, NI, CPLX>;
   auto kern = gemm_ws_kn_kernel<MI, NI, CPLX>;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemCap);
   }
   int S = (kSmemCap - 1024 - 256) / Cfg::STAGE_BYTES;
@@ -405,7 +405,7 @@ int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double*
                    int M, int N, int K, int split, cudaStream_t st) {
   if (!(even(lda) && even(ldb) && al16(A) && al16(B))) return -1;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(gemm_ws_nk_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemCap);
   }
   TensorMap tmA, tmB;

@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -16,32 +18,66 @@ constexpr int kMaxTaylor = 16;
 constexpr int kMaxGroup = 8;    // members of a distributed-Hamiltonian group
 
 // Per-device one-off work (cudaFuncSetAttribute is per device; handles may live on different devices of one
-// process): true the first time it is called with this mask on the current device.
-inline bool first_use_on_device(uint64_t* mask) {
-  int dev = 0;
-  cudaGetDevice(&dev);
-  const uint64_t b = 1ull << (dev & 63);
-  if (*mask & b) return false;
-  *mask |= b;
-  return true;
+// process, and may be driven from different host threads).  Usage:
+//     if (auto once = first_use_on_device(&mask)) { cudaFuncSetAttribute(...); }
+// The guard holds a process-wide mutex for the whole if statement and marks the device as done only when it is
+// destroyed, so a second thread can never launch the kernel between "bit set" and "attribute set".
+inline std::mutex& device_once_mutex() {
+  static std::mutex m;
+  return m;
 }
-// largest dynamic shared-memory size requested so far on the current device; true if `bytes` exceeds it
-inline bool grow_on_device(size_t* cur /* [64] */, size_t bytes) {
+struct OnceGuard {
+  std::unique_lock<std::mutex> lk;
+  uint64_t* mask = nullptr;
+  uint64_t bit = 0;
+  bool first = false;
+  OnceGuard() = default;
+  OnceGuard(OnceGuard&& o) noexcept : lk(std::move(o.lk)), mask(o.mask), bit(o.bit), first(o.first) { o.mask = nullptr; }
+  explicit operator bool() const { return first; }
+  ~OnceGuard() { if (first && mask) *mask |= bit; }
+};
+inline OnceGuard first_use_on_device(uint64_t* mask) {
   int dev = 0;
   cudaGetDevice(&dev);
-  if (bytes <= cur[dev & 63]) return false;
-  cur[dev & 63] = bytes;
-  return true;
+  OnceGuard g;
+  g.lk = std::unique_lock<std::mutex>(device_once_mutex());
+  g.mask = mask;
+  g.bit = 1ull << (dev & 63);
+  g.first = (*mask & g.bit) == 0;
+  return g;
+}
+// largest dynamic shared-memory size requested so far on the current device; the guard is true if `bytes`
+// exceeds it (same locking as above; the new size is recorded when the guard is destroyed)
+struct GrowGuard {
+  std::unique_lock<std::mutex> lk;
+  size_t* slot = nullptr;
+  size_t bytes = 0;
+  bool grow = false;
+  GrowGuard() = default;
+  GrowGuard(GrowGuard&& o) noexcept : lk(std::move(o.lk)), slot(o.slot), bytes(o.bytes), grow(o.grow) { o.slot = nullptr; }
+  explicit operator bool() const { return grow; }
+  ~GrowGuard() { if (grow && slot) *slot = bytes; }
+};
+inline GrowGuard grow_on_device(size_t* cur /* [64] */, size_t bytes) {
+  int dev = 0;
+  cudaGetDevice(&dev);
+  GrowGuard g;
+  g.lk = std::unique_lock<std::mutex>(device_once_mutex());
+  g.slot = &cur[dev & 63];
+  g.bytes = bytes;
+  g.grow = bytes > *g.slot;
+  return g;
 }
 // SM count of the current device (cached per device)
 inline int sm_count_current() {
-  static int n[64] = {0};
+  static std::atomic<int> n[64];
   int dev = 0;
   cudaGetDevice(&dev);
-  int& v = n[dev & 63];
+  int v = n[dev & 63].load(std::memory_order_relaxed);
   if (!v) {
     cudaDeviceGetAttribute(&v, cudaDevAttrMultiProcessorCount, dev);
     if (v <= 0) v = 148;
+    n[dev & 63].store(v, std::memory_order_relaxed);
   }
   return v;
 }

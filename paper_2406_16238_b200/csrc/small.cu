@@ -542,7 +542,7 @@ static int run_overlap_theta_gemm(const OTArgs& a, int nw, cudaStream_t st) {
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = (size_t)nsmax * 2 * nsmax * 16 + (size_t)nsmax * 16 + 64;
   static size_t cur[64] = {0};
-  if (grow_on_device(cur, sm)) cudaFuncSetAttribute(gj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+  if (auto grow_ = grow_on_device(cur, sm)) cudaFuncSetAttribute(gj_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
   gj_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);
   ++launches;
   if (!a.want_theta) return launches;
@@ -575,7 +575,7 @@ int run_overlap_theta(const OTArgs& a, int nw, cudaStream_t st) {
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = ot_smem(nsmax);
   static size_t cur[64] = {0};
-  if (grow_on_device(cur, sm)) {
+  if (auto grow_ = grow_on_device(cur, sm)) {
     cudaFuncSetAttribute(overlap_theta_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
   }
   overlap_theta_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);
@@ -597,7 +597,7 @@ int run_cholqr_pass(const QRArgs& a, int nw, cudaStream_t st) {
   if (a.nblk > 1 && a.ns[1] > nsmax) nsmax = a.ns[1];
   const size_t sm = (size_t)2 * nsmax * nsmax * 16 + (size_t)kRows * (nsmax | 1) * 16 + 64;
   static size_t cur[64] = {0};
-  if (grow_on_device(cur, sm)) {
+  if (auto grow_ = grow_on_device(cur, sm)) {
     cudaFuncSetAttribute(cholqr_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
   }
   cholqr_kernel<<<dim3(a.nblk, nw), 256, sm, st>>>(a);

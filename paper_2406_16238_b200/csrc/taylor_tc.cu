@@ -282,7 +282,7 @@ int taylor_tc_prepare_E1(const double* E1, void* E1b, int M, cudaStream_t st) {
 // Tb <- T [nw][M][N2] (walker layout): [T^T | (J T)^T] rows
 int taylor_tc_prepare_T(const double* T, void* Tb, int nw, int M, int N2, cudaStream_t st) {
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr))
+  if (auto once_ = first_use_on_device(&attr))
     cudaFuncSetAttribute(split_T_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 32 * 257 * 8);
   const int Kp = round_up(M, TY_BK);
   split_T_kernel<<<dim3(Kp / 32, nw), 256, (size_t)32 * (N2 + 1) * 8, st>>>(T, (__nv_bfloat16*)Tb, M, N2,
@@ -305,7 +305,7 @@ int taylor_tc_apply(const void* Aplanes, bool real_shared, const void* Tb, void*
   if (S < 2) return -1;
   const size_t smem = (size_t)S * stage + 1024 + 256;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr))
+  if (auto once_ = first_use_on_device(&attr))
     cudaFuncSetAttribute(taylor_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, TY_SMEM_CAP);
   const int nsm = sm_count_current();
   TensorMap tmA, tmB;

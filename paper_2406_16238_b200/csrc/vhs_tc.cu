@@ -367,7 +367,7 @@ int run_vhs_tc(const double* Cf, void* Ab, const void* Lb, double* const* Cb, in
   const int rows = nmember * rows_per_member;
   const int Gp = vhs_tc_gamma_padded(n_chol), Rp = vhs_tc_rows_padded(rows);
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(vhs_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
     cudaFuncSetAttribute(vhs_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
   }
@@ -431,7 +431,7 @@ int run_fb_tc(const double* ThT, void* Tbuf, const void* Lrb, double* Xp, long l
               int K, int split, cudaStream_t st) {
   const int Kp = vhs_tc_gamma_padded(K), Rp = vhs_tc_rows_padded(rows), Np = fb_tc_rows_padded(n_chol);
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(vhs_tc_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
     cudaFuncSetAttribute(vhs_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)TC_SMEM);
   }

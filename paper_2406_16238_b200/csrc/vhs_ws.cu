@@ -237,7 +237,7 @@ int run_vhs_ws_scatter(const double* Cf, const double* L, double* const* Cb, int
   if (ldcf & 1) return -1;
   const int rows = nmember * rows_per_member;
   static uint64_t attr = 0;
-  if (first_use_on_device(&attr)) {
+  if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(vhs_ws_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
     cudaFuncSetAttribute(vhs_ws_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEMv);
   }

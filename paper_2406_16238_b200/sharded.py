@@ -75,11 +75,8 @@ class LocalGroup:
                         ortho_every=ortho_every, e_shift=e_shift, pack_chol=pack_chol,
                         group_size=self.G, group_rank=r)
             for r, Ls in enumerate(L_slices)]
-        # setup sums in member order 0..G-1, the same on every member
-        total = None
-        for m in self.members:
-            part = m.shard_setup_partial()
-            total = part if total is None else total + part
+        # setup sums in member order 0..G-1 (added up inside the library), the same on every member
+        total = afqmc.AFQMC.shard_setup_reduce(np.stack([m.shard_setup_partial() for m in self.members]))
         addrs = np.stack([m.shard_get_buffers() for m in self.members])
         for m in self.members:
             m.shard_setup_finish(total)
@@ -163,13 +160,8 @@ class DistGroup:
                 if r == self.rank:
                     addrs[r, k] = own[k]
                 else:
-                    out = np.zeros(1, dtype=np.uint64)
-                    hb = np.frombuffer(everyone[r][k], dtype=np.uint8).copy()
-                    rc = afqmc.lib.afqmc_shard_ipc_open(hb.ctypes.data, out.ctypes.data)
-                    if rc != 0:
-                        raise afqmc.AfqmcError(rc, afqmc.lib.afqmc_last_error(None).decode())
-                    addrs[r, k] = out[0]
-                    self._opened.append(int(out[0]))
+                    addrs[r, k] = self.member.shard_ipc_open(everyone[r][k])
+                    self._opened.append(int(addrs[r, k]))
         self.member.shard_set_peers(addrs)
         self._flag = torch.zeros(1, device="cuda") if self.nccl else None
         self.barrier()

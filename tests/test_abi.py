@@ -32,17 +32,23 @@ def test_library_exports_every_declared_symbol():
 
 
 def test_params_struct_layout_matches_c(tmp_path):
+    """sizeof and the offset of EVERY field of afqmc_params, as gcc lays the header's struct out, against the
+    ctypes mirror (same names, same order)."""
     from paper_2406_16238_b200 import afqmc
+    P = afqmc.AfqmcParams
+    names = [f[0] for f in P._fields_]
+    hdr = re.sub(r"/\*.*?\*/", "", open(HEADER).read(), flags=re.S)
+    body = hdr[hdr.index("typedef struct {"):hdr.index("} afqmc_params;")]
+    assert re.findall(r"\b(\w+);", body) == names
     src = tmp_path / "sz.c"
+    offs = ", ".join(f"offsetof(afqmc_params, {n})" for n in names)
     src.write_text('#include <stdio.h>\n#include <stddef.h>\n#include "afqmc.h"\n'
-                   'int main(){printf("%zu %zu %zu %zu\\n", sizeof(afqmc_params), '
-                   'offsetof(afqmc_params, e_shift), offsetof(afqmc_params, stream), '
-                   'offsetof(afqmc_params, e_shift_auto));return 0;}\n')
+                   'int main(){size_t v[] = {sizeof(afqmc_params), ' + offs + '};\n'
+                   'for (unsigned i = 0; i < sizeof(v) / sizeof(v[0]); ++i) printf("%zu ", v[i]);return 0;}\n')
     exe = tmp_path / "sz"
     subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
     out = subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.split()
-    P = afqmc.AfqmcParams
-    assert [int(v) for v in out] == [C.sizeof(P), P.e_shift.offset, P.stream.offset, P.e_shift_auto.offset]
+    assert [int(v) for v in out] == [C.sizeof(P)] + [getattr(P, n).offset for n in names]
 
 
 def test_header_is_plain_c():
@@ -76,3 +82,23 @@ def test_no_cpu_fallback_in_the_product_path():
         for f in fs:
             if f.endswith((".py", ".cu", ".cuh", ".h")):
                 assert not pat.search(open(os.path.join(d, f)).read()), f
+
+
+def test_library_reads_no_environment_variables():
+    """The kernel path is chosen by afqmc_params.kernel_path only: a user's environment cannot change it."""
+    pk = os.path.join(ROOT, "paper_2406_16238_b200", "csrc")
+    for f in os.listdir(pk):
+        assert "getenv" not in open(os.path.join(pk, f)).read(), f
+
+
+def test_shard_setup_reduce_adds_in_member_order():
+    """afqmc_shard_setup_reduce is a plain host loop (no device): left-to-right sum over the members."""
+    from paper_2406_16238_b200 import afqmc
+    r = np.random.default_rng(3)
+    parts = r.standard_normal((5, 11)) * 10.0 ** r.integers(-8, 8, size=(5, 11))
+    out = afqmc.AFQMC.shard_setup_reduce(parts)
+    ref = parts[0].copy()
+    for k in range(1, 5):
+        ref = ref + parts[k]
+    assert np.array_equal(out, ref)
+    assert afqmc.lib.afqmc_shard_setup_reduce(None, 2, 3, None) == -1

@@ -168,6 +168,34 @@ def test_free_running_parity(name, nw):
     pr.close()
 
 
+# --------------------------------------------------------------------------- the other kernel paths at even M
+@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 24, {}),
+                                          ("c1", 3, dict(M=90, n_alpha=42, n_beta=42, n_chol=38))])
+def test_kernel_paths_at_even_M(name, nw, over, path):
+    """afqmc_params.kernel_path: 1 = the cp.async kernels (what odd M runs), 2 = the one-kernel overlap / Theta
+    route, both at EVEN M where the default is the TMA path: a step with QR and the local energy against the
+    oracle, and against the default path to rounding."""
+    _torch()
+    pr = Pair(name, nw=nw, ortho_every=1, kernel_path=path, **over)
+    ref = Pair(name, nw=nw, ortho_every=1, oracle=False, **over)
+    cfg = pr.cfg
+    x = pr.fields(0)
+    w0 = np.linspace(0.5, 1.5, nw)
+    Wg, wg, ovg = gpu_step(pr, pr.walkers0, w0, x, cfg.dt)
+    Wr, wr, ovr = gpu_step(ref, pr.walkers0, w0, x, cfg.dt)
+    Wo, wo, ovo = pr.oracle.step(pr.walkers0, w0, x, cfg.dt)
+    assert rel_fro(Wg, Wo) < TOL_STEP and rel_max(wg, wo) < TOL_STEP and rel_max(ovg, ovo) < TOL_STEP
+    assert rel_fro(Wg, Wr) < 1e-12 and rel_max(wg, wr) < 1e-12
+    E_o = pr.oracle.local_energy(Wo)
+    sc = energy_scale(pr.oracle, Wo, E_o)
+    E_g = gpu_energy(pr, Wo)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10
+    pr.close()
+    ref.close()
+
+
 # --------------------------------------------------------------------------- random shapes
 def _random_cases(n, seed):
     rng = np.random.default_rng(seed)
@@ -209,7 +237,7 @@ def test_random_shapes(name, nw, over):
 
 
 # --------------------------------------------------------------------------- full sizes
-@pytest.mark.parametrize("name,idx,device_L", [("c3", (0, 129, 255), False),
+@pytest.mark.parametrize("name,idx,device_L", [("c3", (0, 1, 2, 3, 64, 65, 127, 128, 129, 130, 191, 200, 252, 253, 254, 255), False),
                                                ("c4", (0, 77, 127), True),
                                                ("c5", (0, 37, 63), True)])
 def test_full_size_sampled_walkers(name, idx, device_L):
@@ -357,22 +385,78 @@ def test_walker_equals_trial():
 
 
 def test_dead_walkers_get_zero_weight():
-    """Reading S10: zero overlap or cos(theta) <= 0 gives weight exactly 0, no error."""
+    """Reading S10: zero overlap or cos(theta) <= 0 gives weight exactly 0, no error.  Every walker's weight is
+    compared with the oracle's.  Walker 1 has an overlap that is pure rounding noise (1e-17): its ratio
+    ovlp'/ovlp is defined by that noise, so only finiteness is comparable there; walker 4 has an EXACT zero overlap
+    (a zero column: the pivot search finds an exactly zero column on both sides) and must give exactly 0 on both;
+    walker 5 has a small but representable overlap (1e-6) and must agree to cond * eps."""
     _torch()
-    pr = Pair("c1", nw=4)
+    pr = Pair("c1", nw=6)
     cfg = pr.cfg
     W = pr.walkers0.copy()
-    # walker 1: first column replaced by an unoccupied eigenvector of h1 -> overlap exactly ~0
+    # walker 1: first column replaced by an unoccupied eigenvector of h1 -> overlap ~ rounding noise
     lam, v = np.linalg.eigh(pr.h1)
     W[1] = pr.trial.astype(np.complex128)
     W[1][:, 0] = v[:, cfg.M - 1]
     W[2] = np.nan
-    Wg, wg, ovg = gpu_step(pr, W, np.ones(4), pr.fields(0), cfg.dt)
-    _, wo, _ = pr.oracle.step(W, np.ones(4), pr.fields(0), cfg.dt)
+    W[4][:, 2] = 0.0
+    W[5] = pr.trial.astype(np.complex128)
+    W[5][:, 0] = v[:, cfg.M - 1] + 1e-6 * pr.trial[:, 0]
+    x = pr.fields(0, nw=6)
+    Wg, wg, ovg = gpu_step(pr, W, np.ones(6), x, cfg.dt)
+    _, wo, ovo = pr.oracle.step(W, np.ones(6), x, cfg.dt)
     assert wg[2] == 0.0 and wo[2] == 0.0
+    assert wg[4] == 0.0 and wo[4] == 0.0
     assert wg[0] > 0 and wg[3] > 0
     assert rel_max(wg[[0, 3]], wo[[0, 3]]) < TOL_STEP
-    assert np.isfinite(wg[1]) and wg[1] >= 0.0
+    assert np.isfinite(wg[1]) and wg[1] >= 0.0 and np.isfinite(wo[1]) and wo[1] >= 0.0
+    # overlap 1e-6 of O(1) columns: relative error of the old overlap ~ 1e-16 / 1e-6
+    assert wo[5] > 0 and abs(wg[5] - wo[5]) < 1e-8 * wo[5]
+    assert abs(ovg[5] - ovo[5]) < 1e-10 * abs(ovo[5])
+    pr.close()
+
+
+# --------------------------------------------------------------------------- literal amplitudes (stress case)
+def test_c1_literal_amplitudes():
+    """SURVEY 8(d) R1 / BASELINE.md 5: c1 with BASELINE.json's LITERAL N(0,1) exp(-g/24) amplitudes (no global
+    rescale).  ||A||_2 = 2..9, |xbar| up to 50, Taylor-6 is no exponential there and every weight is exactly 0
+    by step 7 - but one step is still a deterministic map, so per-step parity (GPU re-seeded from the oracle
+    each step) must hold to 1e-10 on walkers and overlaps, and the weights must agree INCLUDING the exact
+    zeros of the phaseless cut: oracle zero => GPU zero unless |cos theta| < 1e-9 (SURVEY 8c "Parity metric")."""
+    _torch()
+    pr = Pair("c1", literal=True)
+    o, cfg, nw = pr.oracle, pr.cfg, pr.nw
+    Wo, wo = pr.walkers0.copy(), np.ones(nw)
+    zeros_seen = 0
+    borderline = []
+    for s in range(cfg.steps):
+        x = pr.fields(s)
+        _, info = o.propagate(Wo, x, cfg.dt)
+        nA = max(np.linalg.norm(info["A"][w], 2) for w in range(nw))
+        if s == 0:
+            assert nA > 1.5                                   # this IS the stress regime
+        cos = info["S"].real / np.abs(info["S"])
+        w_in = wo.copy() if s > 0 else np.ones(nw)
+        w_in = np.where(w_in > 0, w_in, 1.0)                  # keep every walker's weight rule exercised
+        Wg, wg, ovg = gpu_step(pr, Wo, w_in, x, cfg.dt)
+        o.n_steps_done = 0
+        Wn, wn, ovn = o.step(Wo, w_in, x, cfg.dt)
+        assert rel_fro(Wg, Wn) < TOL_STEP, (s, rel_fro(Wg, Wn))
+        assert rel_max(ovg, ovn) < TOL_STEP, s
+        for k in range(nw):
+            if abs(cos[k]) < 1e-9:
+                borderline.append((s, k))
+                continue
+            if wn[k] == 0.0:
+                assert wg[k] == 0.0, (s, k, wg[k], cos[k])
+                zeros_seen += 1
+            else:
+                assert abs(wg[k] - wn[k]) < TOL_STEP * wn[k], (s, k, wg[k], wn[k])
+        _, wo, _ = Wn, wo * (wn / w_in), ovn
+        Wo = Wn
+    assert zeros_seen >= 10, zeros_seen                       # the phaseless cut really fired
+    assert np.all(wo == 0.0)                                  # R1: all 16 walkers are dead by the last step
+    assert not borderline, borderline
     pr.close()
 
 

@@ -1,4 +1,4 @@
-"""Pins P1-P13: the oracle against what the paper and the mathematics fix.
+"""Pins P1-P16 (P14-P16 added in DESIGN.md §4): the oracle against what the paper and the mathematics fix.
 
 None of these retype the oracle's formulas: they use explicit many-body matrices
 (tests/fock.py), brute-force four-index sums, closed forms, scipy's matrix exponential,
@@ -274,10 +274,9 @@ def test_P10_taylor_vs_expm():
             assert err <= 1.05 * tol_fn(nA) * scale + 1e-14
             if K == 6:
                 assert err > 1e-3 * tol_fn(nA) * scale             # the bound is not vacuous
-            # A = -i sqrt(dt) sum xs_g L_g, complex symmetric
+            # A is complex symmetric (its value is pinned by P6's quadrature and P16's many-body propagator,
+            # not by retyping the formula here)
             assert np.abs(A - A.T).max() < 1e-15
-            ref = -1j * np.sqrt(dt) * np.einsum("g,gpq->pq", info["xs"][w], L)
-            assert np.abs(A - ref).max() < 1e-14
 
 
 # --------------------------------------------------------------------------- P11
@@ -440,3 +439,63 @@ def test_P15_estimator_and_block_loop():
     o3 = AFQMCOracle(h, L, trial, 3, 3, 0, ortho_every=2)
     _, w3, _, _, _, maps3 = run_block(o3, walkers, np.ones(6), x, [], 0.01, 0)
     assert maps3 == [] and not np.allclose(w3, w3[0])
+
+
+# --------------------------------------------------------------------------- P16 weight rule, L != 0
+@pytest.mark.parametrize("kind,na,nb,seed", [(1, 2, 1, 21), (0, 2, 2, 22)])
+def test_P16_weight_rule_many_body(kind, na, nb, seed):
+    """Eqs. (13), (15)-(18) with L != 0, from explicit many-body matrices only.
+
+    In the 256-dimensional Fock space the one-sample propagator is built WITHOUT any of the oracle's one-body
+    formulas: with m_g = <Psi_T|L_g|Psi_T>, E_c = -1/2 sum m_g^2 and V0 = H - E_c - 1/2 sum_g (L_g - m_g)^2
+    (the operator the Trotter split of Eq. 7 calls v0 after the mean-field shift),
+        B(x - xbar) = e^{-dt E_c} e^{-dt/2 V0} e^{-i sqrt(dt) sum_g (x - xbar)_g (L_g - m_g)} e^{-dt/2 V0},
+    xbar_g = i sqrt(dt) (<L_g>_mixed - m_g).  Then S = <Psi_T|B|phi>/<Psi_T|phi> e^{+dt E_c} (Eq. 17; real
+    positive factors do not enter theta), I = <Psi_T|B|phi>/<Psi_T|phi> e^{x.xbar - xbar.xbar/2} e^{dt E_shift}
+    (Eq. 16 with the energy shift of reading S7) and w' = w |I| max(0, Re S/|S|) (Eqs. 13, 15, 18).  The oracle's
+    `step` (Taylor order 24, i.e. the exact exponential to 1e-15) must give the same weights and overlaps."""
+    M, ng, dt = 4, 3, 0.04
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, seed, lscale=0.45, noise=0.35, nw=6)
+    o = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24)
+    F = Fock(M)
+    dim = 2 ** F.n
+    Id = np.eye(dim)
+    H = F.hamiltonian(h, L)
+    ta, tb = spin_blocks(o, trial)
+    psiT = F.det_state(ta.astype(complex), tb.astype(complex))
+    bra = psiT.conj()
+    assert abs(bra @ psiT - 1.0) < 1e-12
+    Lop = [F.one_body(L[g]) for g in range(ng)]
+    m = np.array([(bra @ Lop[g] @ psiT).real for g in range(ng)])
+    E_c = -0.5 * float(m @ m)
+    e_shift = float((bra @ H @ psiT).real)
+    V0 = H - E_c * Id
+    for g in range(ng):
+        d = Lop[g] - m[g] * Id
+        V0 = V0 - 0.5 * d @ d
+    half = sla.expm(-0.5 * dt * V0)
+    x = np.random.default_rng(seed).standard_normal((walkers.shape[0], ng))
+    w0 = np.linspace(0.5, 2.0, walkers.shape[0])
+    expect_w, expect_ov, phases = [], [], []
+    for k in range(walkers.shape[0]):
+        wa, wb = spin_blocks(o, walkers[k])
+        ket = F.det_state(wa, wb)
+        ov = bra @ ket
+        X = np.array([(bra @ Lop[g] @ ket) / ov for g in range(ng)])
+        xbar = 1j * np.sqrt(dt) * (X - m)
+        xs = x[k] - xbar
+        two = sla.expm(-1j * np.sqrt(dt) * sum(xs[g] * (Lop[g] - m[g] * Id) for g in range(ng)))
+        Bket = np.exp(-dt * E_c) * (half @ (two @ (half @ ket)))
+        ratio = (bra @ Bket) / ov
+        S = ratio * np.exp(dt * E_c)
+        I = ratio * np.exp(np.sum(x[k] * xbar) - 0.5 * np.sum(xbar * xbar)) * np.exp(dt * e_shift)
+        expect_w.append(w0[k] * abs(I) * max(0.0, S.real / abs(S)))
+        expect_ov.append(bra @ Bket * np.exp(dt * E_c) / np.exp(1j * np.sqrt(dt) * (xs @ m)))
+        phases.append(np.angle(S))
+    new, w, ov_new = o.step(walkers, w0, x, dt)
+    assert abs(o.e_shift - e_shift) < 1e-12 and abs(o.E_const - E_c) < 1e-12
+    assert np.max(np.abs(w - np.array(expect_w))) < 1e-10 * max(expect_w)
+    # the propagated determinant itself: <Psi_T|phi'> = <Psi_T|B|phi> without the scalars B carries
+    assert np.max(np.abs(ov_new - np.array(expect_ov)) / np.abs(expect_ov)) < 1e-10
+    assert np.max(np.abs(phases)) > 1e-2          # theta is not trivially zero: the cos factor is exercised
+    assert np.all(np.array(expect_w) > 0)
