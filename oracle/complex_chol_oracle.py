@@ -21,8 +21,14 @@ follows is derived from the paper's own equations:
     symmetric L: 2n auxiliary fields, v_g' = i K_g', m_g' = tr(K_g' P) (real), h' = h - 1/2 sum K K,
     h_mod = h' + sum m K (Hermitian), E1 = expm(-dt/2 h_mod), A = -i sqrt(dt) sum xs K, Lrot = psi^T K,
     X = tr(Lrot Theta), E_C = 1/2 sum X^2, E_X = -1/2 sum tr(T T), T = Lrot Theta.
-  * Readings: real trial (S12 kept); h1 complex Hermitian; a vector set whose antisymmetric sum does not vanish
-    (not a set of ERIs) is rejected at construction.
+  * Readings: h1 complex Hermitian; a vector set whose antisymmetric sum does not vanish (not a set of ERIs) is
+    rejected at construction.
+  * Complex trial (PAPER.md:219 Code Snippet 6 gives the trial no dtype; magnetic fields,
+    spin-orbit coupling and Bloch orbitals make the wavefunctions complex; SURVEY S12 "formulas keep psi^+"):
+    <Psi_T| = prod_i (sum_p conj(psi_pi) a_p), so every psi^T of the real-trial formulas is psi^+:
+        O = psi^+ phi,  Theta = phi O^-1,  G_pq = <a+_p a_q> = [Theta psi^+]_qp,  P = psi psi^+ (Hermitian),
+        m_g' = tr(K_g' P) (still real: K and P Hermitian),  Lrot = psi^+ K,  hrot = psi^+ h.
+    A real trial is the special case; nothing else changes (the propagator does not see the trial).
 
 Plain NumPy complex128; library primitives as single steps (matmul, det, solve, eigh, qr).
 """
@@ -43,7 +49,8 @@ def hermitian_parts(L):
 class ComplexCholOracle:
     def __init__(self, h1, L, trial, n_alpha, n_beta, walker_kind, taylor_order=6, e_shift=None, check=True):
         h1 = np.asarray(h1, dtype=np.complex128)
-        trial = np.asarray(trial, dtype=np.float64)
+        trial = np.asarray(trial)
+        trial = trial.astype(np.complex128 if np.iscomplexobj(trial) else np.float64)
         self.M = M = h1.shape[0]
         self.n_alpha, self.n_beta, self.walker_kind = int(n_alpha), int(n_beta), int(walker_kind)
         self.K_order = int(taylor_order) if taylor_order else 6
@@ -61,13 +68,13 @@ class ComplexCholOracle:
             anti = np.einsum("gps,gqr->psqr", K[n:], K[:n]) - np.einsum("gps,gqr->psqr", K[:n], K[n:])
             if np.abs(anti).max() > 1e-10 * max(1.0, np.abs(K).max() ** 2):
                 raise ValueError("the vectors do not factorise a (ps|qr) = (qr|ps) symmetric tensor")
-        P_tot = sum(p @ p.T for p in self.psi) * self.spin_factor
-        self.m = np.einsum("gpq,pq->g", K, P_tot).real                    # tr(K P), real for Hermitian K
+        P_tot = sum(p @ p.conj().T for p in self.psi) * self.spin_factor      # P = psi psi^+
+        self.m = np.einsum("gpq,qp->g", K, P_tot).real                    # tr(K P), real for Hermitian K, P
         hprime = h1 - 0.5 * np.einsum("gpq,gqr->pr", K, K)
         self.h_mod = hprime + np.einsum("g,gpq->pq", self.m, K)
         self.E_const = -0.5 * float(self.m @ self.m)
-        self.Lrot = [np.einsum("pi,gpq->giq", p, K) for p in self.psi]   # psi^T K_g  [2n, Ns, M]
-        self.hrot = [p.T @ h1 for p in self.psi]
+        self.Lrot = [np.einsum("pi,gpq->giq", p.conj(), K) for p in self.psi]   # psi^+ K_g  [2n, Ns, M]
+        self.hrot = [p.conj().T @ h1 for p in self.psi]
         if e_shift is None:
             w0 = np.concatenate(self.psi, axis=1).astype(np.complex128)[None]
             self.e_shift = float(self.local_energy(w0)[0, 0].real)
@@ -82,7 +89,7 @@ class ComplexCholOracle:
         ov = np.ones(walkers.shape[0], dtype=np.complex128)
         for (a, b), p in zip(self.blocks, self.psi):
             for w in range(walkers.shape[0]):
-                d = np.linalg.det(p.T @ walkers[w, :, a:b])
+                d = np.linalg.det(p.conj().T @ walkers[w, :, a:b])
                 ov[w] *= d * d if self.walker_kind == 0 else d
         return ov
 
@@ -91,7 +98,7 @@ class ComplexCholOracle:
         for (a, b), p in zip(self.blocks, self.psi):
             for w in range(walkers.shape[0]):
                 phi = walkers[w, :, a:b]
-                th[w, :, a:b] = np.linalg.solve((p.T @ phi).T, phi.T).T
+                th[w, :, a:b] = np.linalg.solve((p.conj().T @ phi).T, phi.T).T
         return th
 
     def force_bias_X(self, th):
