@@ -312,6 +312,19 @@ int32_t afqmc_shard_energy_finish(afqmc_handle* h, void* E_out, int32_t nw);
  * (DFMA) TFLOP/s, out[2] = SM clock seen (MHz, from clock64/elapsed).  HOST pointer. */
 int32_t afqmc_measure_fp64_peak(double ms, double* out3);
 
+/* Measurement helper (host only, no GPU work): the tile plan of the exchange kernel (a11, Eq. 11) for an occupied
+ * block of `ns` columns and `M` basis functions (the K loop), as text in `out` (HOST, at most `n` bytes incl. the terminator): consumer warps, vectors and
+ * walkers per tile, useful fraction of the issued DMMA blocks, ring depth, epilogue passes.  `pair` = 1: the plan
+ * of the complex (two-plane) half-rotated tensor.  Returns that useful fraction times 1e6, or AFQMC_ERR_INVALID. */
+int32_t afqmc_exchange_plan(int32_t ns, int32_t M, int32_t pair, char* out, int32_t n);
+/* Tuning hook (host only): replace the plan chosen for (ns, M, pair) in this process by the candidate with `warps`
+ * consumer warps (8 or 12) arranged as wm x (warps / wm), warp rectangles of at most mi x ni DMMA blocks, G vectors x
+ * Wn walkers per tile.  Results do not depend on the plan beyond the order of the fixed-order sums.  Handles
+ * created BEFORE the call keep buffers sized for the old plan: pin first, then create.  AFQMC_ERR_UNSUPPORTED if
+ * no such candidate exists (does not fit shared memory or registers). */
+int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t warps, int32_t mi, int32_t ni, int32_t wm,
+                                int32_t G, int32_t Wn);
+
 #ifdef __cplusplus
 }
 #endif

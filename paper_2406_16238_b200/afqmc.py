@@ -22,7 +22,7 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_set_block_graph", "afqmc_shard_setup_partial", "afqmc_shard_setup_finish",
            "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
            "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
-           "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce"]
+           "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce", "afqmc_exchange_plan", "afqmc_exchange_plan_pin"]
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
           "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
@@ -90,6 +90,10 @@ def _load():
     lib.afqmc_shard_setup_reduce.restype = i32
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
+    lib.afqmc_exchange_plan.argtypes = [i32, i32, i32, C.c_char_p, i32]
+    lib.afqmc_exchange_plan.restype = i32
+    lib.afqmc_exchange_plan_pin.argtypes = [i32] * 9
+    lib.afqmc_exchange_plan_pin.restype = i32
     return lib
 
 
@@ -124,6 +128,21 @@ def measure_fp64_peak(ms=200.0):
     if rc != 0:
         raise AfqmcError(rc, "afqmc_measure_fp64_peak")
     return tuple(out)
+
+
+def exchange_plan(ns, M, pair=False):
+    """(useful fraction of the issued DMMA blocks, description) of the exchange kernel's tile plan."""
+    buf = C.create_string_buffer(512)
+    rc = lib.afqmc_exchange_plan(int(ns), int(M), int(bool(pair)), buf, 512)
+    if rc < 0:
+        raise AfqmcError(rc, "afqmc_exchange_plan")
+    return rc * 1e-6, buf.value.decode()
+
+
+def exchange_plan_pin(ns, M, pair, warps, mi, ni, wm, G, Wn):
+    """Pin the exchange kernel's tile plan for (ns, M, pair); call before creating handles.  False if it does not fit."""
+    return lib.afqmc_exchange_plan_pin(int(ns), int(M), int(bool(pair)), int(warps), int(mi), int(ni), int(wm),
+                                       int(G), int(Wn)) == 0
 
 
 class AFQMC:

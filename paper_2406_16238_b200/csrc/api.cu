@@ -297,7 +297,7 @@ int energy_from_theta(afqmc_handle* h, const double* e1, double* E_out, int nw) 
   return AFQMC_OK;
 }
 
-// complex Cholesky vectors: three runs of the exchange kernel (Re planes, Im planes, their sum), cplx.cu
+// complex Cholesky vectors: Lrot = Lr + i Li as two planes
 int local_energy_complex_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
   const int nf = h->nf;
   {
@@ -308,30 +308,46 @@ int local_energy_complex_device(afqmc_handle* h, const double* W, double* E_out,
     h->launches += run_e1(a, nw, h->st);                      // e1i <- Im(h)rot . Theta
   }
   const size_t lsz = (size_t)nf * h->Nt * h->M;
-  const double* lrot[3] = {h->Lrot, h->Lrot + lsz, h->Lrot_sum};
-  double* xe[3] = {h->Xe, h->Xe + (size_t)nf * h->mwg * 2, h->Xe_s};
-  for (int k = 0; k < 3; ++k)
+  CEnergyArgs c;
+  c.pair = h->ws ? 1 : 0;
+  if (h->ws) {
+    // ONE run: the tile's rows are [Re plane | Im plane] of the same vectors, T = Lrot Theta is put together as a
+    // complex matrix by the epilogue warps (exchange_ws.cu, pair mode)
     for (int b = 0; b < h->nblk; ++b) {
       StageTimer tm(h, AFQMC_STAGE_EXCHANGE);
       ExArgs e;
-      e.Lrot = lrot[k]; e.ThT = h->ThT; e.expart = k == 0 ? h->expart[b] : h->expart_c[k - 1][b]; e.X = xe[k];
+      e.Lrot = h->Lrot; e.plane_stride = (long)lsz; e.ThT = h->ThT; e.expart = h->expart_c[0][b]; e.X = h->Xe;
       e.M = h->M; e.Nt = h->Nt; e.n_chol = nf; e.nw = nw;
       e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
-      if (h->ws) {
-        const int r = run_exchange_ws(e, h->st);
-        if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
-        h->launches += r;
-      } else {
+      const int r = run_exchange_ws(e, h->st);
+      if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
+      h->launches += r;
+    }
+    c.Xr = h->Xe; c.Xi = nullptr;
+    for (int b = 0; b < 2; ++b) {
+      c.expart[0][b] = h->expart_c[0][b]; c.expart[1][b] = nullptr; c.expart[2][b] = nullptr;
+      c.ngroups[b] = h->exgroups_c[b];
+    }
+  } else {
+    // odd M (no TMA): three runs of the cp.async kernel (Re planes, Im planes, their sum), cplx.cu
+    const double* lrot[3] = {h->Lrot, h->Lrot + lsz, h->Lrot_sum};
+    double* xe[3] = {h->Xe, h->Xe + (size_t)nf * h->mwg * 2, h->Xe_s};
+    for (int k = 0; k < 3; ++k)
+      for (int b = 0; b < h->nblk; ++b) {
+        StageTimer tm(h, AFQMC_STAGE_EXCHANGE);
+        ExArgs e;
+        e.Lrot = lrot[k]; e.ThT = h->ThT; e.expart = k == 0 ? h->expart[b] : h->expart_c[k - 1][b]; e.X = xe[k];
+        e.M = h->M; e.Nt = h->Nt; e.n_chol = nf; e.nw = nw;
+        e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
         h->launches += run_exchange(e, h->st);
       }
+    c.Xr = xe[0]; c.Xi = xe[1];
+    for (int b = 0; b < 2; ++b) {
+      c.expart[0][b] = h->expart[b]; c.expart[1][b] = h->expart_c[0][b]; c.expart[2][b] = h->expart_c[1][b];
+      c.ngroups[b] = h->exgroups_c[b];
     }
-  StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
-  CEnergyArgs c;
-  c.Xr = xe[0]; c.Xi = xe[1];
-  for (int b = 0; b < 2; ++b) {
-    c.expart[0][b] = h->expart[b]; c.expart[1][b] = h->expart_c[0][b]; c.expart[2][b] = h->expart_c[1][b];
-    c.ngroups[b] = h->exgroups_c[b];
   }
+  StageTimer tm(h, AFQMC_STAGE_E_REDUCE);
   c.e1r = h->e1; c.e1i = h->e1i; c.E_out = E_out;
   c.nf = nf; c.nw = nw; c.nblk = h->nblk; c.spin_factor = h->sf;
   h->launches += run_energy_cplx(c, h->st);
@@ -984,7 +1000,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->T0 = dalloc(h, wsz); h->T1 = dalloc(h, wsz); h->Acc = dalloc(h, wsz);
   h->ovlp = dalloc(h, 2 * mw); h->detR = dalloc(h, 2 * mw);
   for (int b = 0; b < h->nblk; ++b) {
-    const int G = h->ws ? exchange_ws_group_size(h->ns[b]) : exchange_group_size(h->ns[b]);
+    const int G = h->ws ? exchange_ws_group_size(h->ns[b], M) : exchange_group_size(h->ns[b]);
     h->exgroups[b] = (nc + G - 1) / G;
     h->expart[b] = dalloc(h, (size_t)h->exgroups[b] * mwg * 2);
   }
@@ -1033,7 +1049,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->Xe_s = dalloc(h, (size_t)h->nf * mwg * 2);
     bool ok = h->e1i && h->Xe_s;
     for (int b = 0; b < h->nblk; ++b) {
-      const int G = h->ws ? exchange_ws_group_size(h->ns[b]) : exchange_group_size(h->ns[b]);
+      const int G = h->ws ? exchange_ws_group_size(h->ns[b], M, true) : exchange_group_size(h->ns[b]);
       h->exgroups_c[b] = (h->nf + G - 1) / G;
       for (int k = 0; k < 2; ++k) {
         h->expart_c[k][b] = dalloc(h, (size_t)h->exgroups_c[b] * mwg * 2);
@@ -1118,6 +1134,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   }
   *out = h;
   return AFQMC_OK;
+}
+
+int32_t afqmc_exchange_plan(int32_t ns, int32_t M, int32_t pair, char* out, int32_t n) {
+  if (ns < 1 || ns > afq::kMaxOcc || M < ns || !out || n < 1) return AFQMC_ERR_INVALID;
+  afq::exchange_ws_describe(ns, M, pair != 0, out, n);
+  return (int32_t)(afq::exchange_ws_efficiency(ns, M, pair != 0) * 1e6);
+}
+
+int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t warps, int32_t mi, int32_t ni, int32_t wm,
+                                int32_t G, int32_t Wn) {
+  if (ns < 1 || ns > afq::kMaxOcc || M < ns) return AFQMC_ERR_INVALID;
+  return afq::exchange_ws_pin(ns, M, pair != 0, warps, mi, ni, wm, G, Wn) ? AFQMC_OK : AFQMC_ERR_UNSUPPORTED;
 }
 
 int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {

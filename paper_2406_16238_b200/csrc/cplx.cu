@@ -135,12 +135,15 @@ __global__ void __launch_bounds__(256) energy_cplx_kernel(CEnergyArgs a) {
   double v[8] = {0, 0, 0, 0, 0, 0, 0, 0};   // sum X^2 (re, im); sums of tr(TT) for the sets r, i, s (re, im each)
   for (int g = threadIdx.x; g < nf; g += blockDim.x) {
     const double* xr = a.Xr + ((size_t)g * nw + w) * 2;   // tr(T_r) of this field (complex)
-    const double* xi = a.Xi + ((size_t)g * nw + w) * 2;
-    const double Xre = a.spin_factor * (xr[0] - xi[1]), Xim = a.spin_factor * (xr[1] + xi[0]);
+    double Xre = a.spin_factor * xr[0], Xim = a.spin_factor * xr[1];
+    if (!a.pair) {
+      const double* xi = a.Xi + ((size_t)g * nw + w) * 2;
+      Xre = a.spin_factor * (xr[0] - xi[1]); Xim = a.spin_factor * (xr[1] + xi[0]);
+    }
     v[0] += Xre * Xre - Xim * Xim;
     v[1] += 2.0 * Xre * Xim;
   }
-  for (int k = 0; k < 3; ++k)
+  for (int k = 0; k < (a.pair ? 1 : 3); ++k)
     for (int b = 0; b < a.nblk; ++b)
       for (int q = threadIdx.x; q < a.ngroups[b]; q += blockDim.x) {
         const double* e = a.expart[k][b] + ((size_t)q * nw + w) * 2;
@@ -159,8 +162,8 @@ __global__ void __launch_bounds__(256) energy_cplx_kernel(CEnergyArgs a) {
     e1r *= a.spin_factor;
     e1i *= a.spin_factor;
     // tr(TT) = t_r - t_i + i (t_s - t_r - t_i), each t complex
-    const double tr_re = v[2] - v[4] - (v[7] - v[3] - v[5]);
-    const double tr_im = v[3] - v[5] + (v[6] - v[2] - v[4]);
+    const double tr_re = a.pair ? v[2] : v[2] - v[4] - (v[7] - v[3] - v[5]);
+    const double tr_im = a.pair ? v[3] : v[3] - v[5] + (v[6] - v[2] - v[4]);
     const double e2r = 0.5 * v[0] - 0.5 * a.spin_factor * tr_re;
     const double e2i = 0.5 * v[1] - 0.5 * a.spin_factor * tr_im;
     double* o = a.E_out + (size_t)w * 6;

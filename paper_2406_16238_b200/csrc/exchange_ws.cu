@@ -2,13 +2,26 @@
 // PAPER.md:94; D7), warp-specialised TMA version:
 //     T^g_w = Lrot^g [ns x M] * Theta_w [M x ns],   expart += tr(T T),   X_g = tr(T)
 //
-// One persistent CTA per SM.  A producer warp feeds a ring of shared-memory stages with TMA
-// (cp.async.bulk.tensor, SWIZZLE_128B, mbarrier full/empty pairs); WM x WN consumer warps
-// issue nothing but 16-byte fragment loads and DMMA.  A tile is G whole Cholesky vectors
-// (rows (g, i), taken UNPADDED out of Lrot[n_chol][Nt][M] by a 3-D box) times Wn whole
-// walkers (columns (w, plane, j) out of ThT[nw][2][Nt][M] by a 4-D box), so the only padding
-// is the round-up of G*ns and Wn*2*ns to the warp grid.  After the K = M loop the tile is
-// staged through shared memory Wp walkers at a time for tr(T T) and tr(T); T never reaches HBM.
+// One persistent CTA per SM, three roles:
+//   * producer warp: feeds a ring of shared-memory stages with TMA (cp.async.bulk.tensor,
+//     SWIZZLE_128B, mbarrier full/empty pairs);
+//   * 8 or 12 consumer warps: 16-byte fragment loads and DMMA, nothing else.  A tile is G whole
+//     Cholesky vectors (rows (g, i), UNPADDED out of Lrot[n_chol][Nt][M] by a 3-D box) times Wn
+//     whole walkers (columns (w, plane, j) out of ThT[nw][2][Nt][M] by a 4-D box).  The tile's 8 x 8
+//     blocks are dealt to the warps as RECTANGLES of unequal size (XwsArgs::rect): the block counts
+//     19 x 13 of N_occ = 50 do not factor over a warp grid, so the plan balances the four
+//     sub-partitions' DMMA load instead of padding every warp to the largest rectangle;
+//   * 3 epilogue warps (the rest of the producer's warpgroup): after the K = M loop the consumers
+//     only DUMP their accumulators into a shared-memory staging buffer (one pass = Gp vectors x Wp
+//     walkers, two buffers when a tile needs several passes) and go on with the next tile; the
+//     epilogue warps form tr(T T) and tr(T) from the staging buffer while the DMMA pipe is busy
+//     with the next main loop.  T never reaches HBM.
+// Pair mode (complex Cholesky vectors / complex trial: Lrot = Lr + i Li as two planes): the tile's rows are
+// [plane][g][i], the four real products share the Theta fragments and the epilogue warps put
+// T = (Lr Th_r - Li Th_i) + i (Lr Th_i + Li Th_r) together: one run instead of three.
+#include <algorithm>
+#include <map>
+
 #include "internal.h"
 #include "tma.cuh"
 
@@ -17,86 +30,268 @@ namespace afq {
 namespace {
 
 constexpr int kProducerThreads = 128;     // one warpgroup (setmaxnreg is warpgroup-wide)
+constexpr int kEpiWarps = 3;              // warps 1..3 of the producer's warpgroup
+constexpr int kEpiThreads = kEpiWarps * 32;
 constexpr int kSmemMax = 232448;          // 227 KB opt-in limit per CTA
+constexpr int kMaxTasks = 512;            // (gamma, walker, row pair) lane tasks per tile: 16 KB of partial sums
+constexpr int kMaxWarps = 12;
 
 struct XwsArgs {
   double* expart;      // [ngroups][nw] complex
   double* X;           // [n_chol][nw] complex
   int M, ns, off, n_chol, nw;
-  int G, Wn, Wp;       // gammas / walkers per tile, walkers per epilogue pass
-  int ldt;             // staging row stride (doubles), odd
-  int stages;
+  int G, Wn;           // gammas / walkers per tile
+  int Gp, Wp;          // gammas / walkers per epilogue pass
+  int ldt;             // staging row stride (doubles)
+  int stages, nbuf;
+  int rowsA, rowsB;    // rows TMA writes per stage; the stage holds round-up-to-8 of each
   int ntile_w, ntiles;
   int accumulate;
-  int split;           // epilogue work items per (gamma, walker)
+  int pair;            // 1: A rows are [2 planes][G][ns]
+  unsigned rect[kMaxWarps];   // r0 | mi << 8 | c0 << 16 | ni << 24, in 8 x 8 blocks
 };
 
-template <int WM, int WN, int MI, int NI>
+template <int NCW, int MI, int NI>
 struct XwsCfg {
-  static constexpr int NCW = WM * WN;
   static constexpr int NCT = NCW * 32;
   static constexpr int THREADS = NCT + kProducerThreads;
-  static constexpr int TA = 8 * WM * MI, TB = 8 * WN * NI;
-  static constexpr int STAGE_BYTES = (TA + TB) * 128;
-  static constexpr int CREGS = ((65536 - kProducerThreads * 24) / NCT) / 8 * 8 > 240
-                                   ? 240 : ((65536 - kProducerThreads * 24) / NCT) / 8 * 8;
-  static constexpr int MAXITEMS = 256;    // comb slots
+  // register file: THREADS * R0 at launch (R0 from __launch_bounds__), then PREGS for the producer's
+  // warpgroup and CREGS for the consumers
+  static constexpr int R0 = (65536 / THREADS) / 8 * 8;
+  static constexpr int PREGS = NCW == 12 ? 40 : 56;
+  static constexpr int CREGS_ = ((THREADS * R0 - kProducerThreads * PREGS) / NCT) / 8 * 8;
+  static constexpr int CREGS = CREGS_ > 232 ? 232 : CREGS_;
 };
 
-template <int WM, int WN, int MI, int NI>
-__global__ void __launch_bounds__(XwsCfg<WM, WN, MI, NI>::THREADS, 1)
+__device__ __forceinline__ void named_bar_sync_epi() { named_bar_sync(2, kEpiThreads); }
+
+// K = M loop of one tile for a warp rectangle of MU x NU blocks known at compile time (no predicates in the DMMA
+// stream); GENERIC: rectangle sizes from registers (small or odd problems), predicated.
+// Ring state of a consumer: soff = byte offset of the current stage, sbar = 8 * stage index, ph = its parity,
+// prev = 8 * index of the stage to release (lagged release, tma.cuh) or -1.
+struct Ring { uint32_t soff, sbar, ph; int prev; };
+
+template <int MI, int NI, int MU, int NU, bool GENERIC>
+__device__ __forceinline__ void xws_kloop(double (&acc)[MI][NI][2], uint32_t full_u32, uint32_t empty_u32, int KT,
+                                          uint32_t ring_bytes, uint32_t stage_bytes, Ring& r, uint32_t a0, uint32_t b0,
+                                          int lane, int mi, int ni) {
+  for (int kt = 0; kt < KT; ++kt) {
+    mbar_wait_u32(full_u32 + r.sbar, r.ph);
+    if (r.prev >= 0 && lane == 0) mbar_arrive_u32(empty_u32 + r.prev);
+    r.prev = (int)r.sbar;
+    const uint32_t sa = a0 + r.soff, sb = b0 + r.soff;
+    r.soff += stage_bytes; r.sbar += 8;
+    if (r.soff == ring_bytes) { r.soff = 0; r.sbar = 0; r.ph ^= 1; }
+#pragma unroll
+    for (int kp = 0; kp < 2; ++kp) {
+      const uint32_t x = kp ? 64u : 0u;       // the second k pair of a row sits 64 bytes further, modulo the swizzle
+      double2 af[MU];
+#pragma unroll
+      for (int i = 0; i < MU; ++i)
+        if (!GENERIC || i < mi) af[i] = lds128((sa + i * 1024) ^ x);
+#pragma unroll
+      for (int j = 0; j < NU; ++j) {
+        if (!GENERIC || j < ni) {
+          const double2 bf = lds128((sb + j * 1024) ^ x);
+#pragma unroll
+          for (int i = 0; i < MU; ++i)
+            if (!GENERIC || i < mi) dmma884(acc[i][j][0], acc[i][j][1], af[i].x, bf.x);
+#pragma unroll
+          for (int i = 0; i < MU; ++i)
+            if (!GENERIC || i < mi) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, bf.y);
+        }
+      }
+    }
+  }
+}
+
+template <int NCW, int MI, int NI>
+__global__ void __launch_bounds__(XwsCfg<NCW, MI, NI>::THREADS, 1)
 exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB,
-                   const XwsArgs a) {
-  using Cfg = XwsCfg<WM, WN, MI, NI>;
-  constexpr int NCW = Cfg::NCW, NCT = Cfg::NCT, TA = Cfg::TA;
-  extern __shared__ unsigned char smem_raw[];
-  // SWIZZLE_128B tiles need a 1024-byte aligned base (the launch adds the slack)
-  unsigned char* smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+                   const __grid_constant__ XwsArgs a) {
+  using Cfg = XwsCfg<NCW, MI, NI>;
+  constexpr int NCT = Cfg::NCT;
+  // SWIZZLE_128B tiles need a 1024-byte aligned base
+  extern __shared__ __align__(1024) unsigned char smem[];
+  if (smem_u32(smem) & 1023u) __trap();
   const int S = a.stages;
+  const int TAr = (a.rowsA + 7) & ~7, TBr = (a.rowsB + 7) & ~7;
+  const uint32_t stage_bytes = (uint32_t)(TAr + TBr) * 128u;
+  const int ns = a.ns, ldt = a.ldt;
+  const int planes = a.pair ? 2 : 1;
+  const int srows = planes * a.Gp * ns;                 // staging rows per buffer
+  const int nitems = a.G * a.Wn;
   unsigned char* tiles = smem;
-  double* stg = reinterpret_cast<double*>(smem + (size_t)S * Cfg::STAGE_BYTES);
-  const int RAp = (a.G * a.ns + 7) & ~7;
-  double* comb = stg + (size_t)RAp * a.ldt;                       // [MAXITEMS][4]
-  uint64_t* full = reinterpret_cast<uint64_t*>(comb + Cfg::MAXITEMS * 4);
+  double* stg = reinterpret_cast<double*>(smem + (size_t)S * stage_bytes);
+  double* part = stg + (size_t)a.nbuf * srows * ldt;                  // [nitems][row pairs][4]
+  uint64_t* full = reinterpret_cast<uint64_t*>(part + (size_t)nitems * ((ns + 1) >> 1) * 4);
   uint64_t* empty = full + S;
+  uint64_t* sfull = empty + S;                                        // staging buffer written
+  uint64_t* sempty = sfull + 2;                                       // staging buffer read
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int KT = (a.M + 15) >> 4;
+  const int npass_g = (a.G + a.Gp - 1) / a.Gp, npass_w = (a.Wn + a.Wp - 1) / a.Wp;
 
   if (tid == 0) {
     for (int s = 0; s < S; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], NCW); }
+    for (int b = 0; b < 2; ++b) { mbar_init(&sfull[b], NCT); mbar_init(&sempty[b], kEpiThreads); }
     fence_barrier_init();
   }
-  // rows of the A / B tiles that TMA never writes (round-up of G*ns, Wn*2*ns) must read as
-  // finite numbers: zero all stages once
+  // rows of the A / B tiles that TMA never writes (round-up to 8 rows) must read as finite numbers
   {
     uint4* z = reinterpret_cast<uint4*>(tiles);
-    const int n16 = S * Cfg::STAGE_BYTES / 16;
+    const int n16 = (int)(S * stage_bytes / 16);
     for (int i = tid; i < n16; i += Cfg::THREADS) z[i] = make_uint4(0, 0, 0, 0);
   }
   fence_proxy_async();
   __syncthreads();
 
   if (warp >= NCW) {
-    // ------------------------------------------------------------------ producer warpgroup
-    reg_dealloc<24>();
-    if (warp == NCW && lane == 0) {
-      prefetch_tensormap(&tmA);
-      prefetch_tensormap(&tmB);
-      const uint32_t bytes = (uint32_t)(a.G * a.ns + a.Wn * 2 * a.ns) * 128u;
-      uint32_t it = 0;
-      for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-        const int g0 = (tile / a.ntile_w) * a.G, w0 = (tile % a.ntile_w) * a.Wn;
-        for (int kt = 0; kt < KT; ++kt, ++it) {
-          const int s = it % S;
-          const uint32_t ph = (it / S) & 1;
-          mbar_wait(&empty[s], ph ^ 1);
-          mbar_expect_tx(&full[s], bytes);
-          unsigned char* sa = tiles + (size_t)s * Cfg::STAGE_BYTES;
-          tma_load_3d(sa, &tmA, &full[s], kt * 16, a.off, g0);
-          tma_load_4d(sa + TA * 128, &tmB, &full[s], kt * 16, a.off, 0, w0);
+    reg_dealloc<Cfg::PREGS>();
+    if (warp == NCW) {
+      // ---------------------------------------------------------------------- producer
+      if (lane == 0) {
+        prefetch_tensormap(&tmA);
+        prefetch_tensormap(&tmB);
+        const uint32_t bytes = (uint32_t)(a.rowsA + a.rowsB) * 128u;
+        uint32_t it = 0;
+        for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+          const int g0 = (tile / a.ntile_w) * a.G, w0 = (tile % a.ntile_w) * a.Wn;
+          for (int kt = 0; kt < KT; ++kt, ++it) {
+            const int s = it % S;
+            const uint32_t ph = (it / S) & 1;
+            mbar_wait(&empty[s], ph ^ 1);
+            mbar_expect_tx(&full[s], bytes);
+            unsigned char* sa = tiles + (size_t)s * stage_bytes;
+            tma_load_4d(sa, &tmA, &full[s], kt * 16, a.off, g0, 0);
+            tma_load_4d(sa + TAr * 128, &tmB, &full[s], kt * 16, a.off, 0, w0);
+          }
         }
       }
+      return;
+    }
+    // ------------------------------------------------------------------------ epilogue warps
+    // One lane per (vector, walker, row pair): lane task (item, ii) forms the i < j part of
+    //   tr(T T) = sum_i T_ii^2 + 2 sum_{i<j} T_ij T_ji
+    // for the rows i = ii and i = ns - 1 - ii, which together hold ns - 1 pairs for every ii: all lanes run the same
+    // trip count, no shuffles, and neighbouring lanes are ldt + 1 doubles apart in both operands (conflict free).
+    const int et = tid - (NCW + 1) * 32, ew = warp - NCW - 1;
+    const int h = (ns + 1) >> 1;                            // row pairs per item
+    int hp = 1;
+    while (hp < h) hp <<= 1;
+    const uint32_t plane_off = (uint32_t)(a.Gp * ns * ldt * 8);   // second plane of the staging buffer (pair mode)
+    const uint32_t ns8 = (uint32_t)ns * 8, ldt8 = (uint32_t)ldt * 8;
+    const uint32_t stg_e = smem_u32(stg), buf_bytes_e = (uint32_t)(srows * ldt * 8), part_e = smem_u32(part);
+    uint32_t e = 0;
+    for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
+      const int tg = tile / a.ntile_w;
+      const int g0 = tg * a.G, w0 = (tile % a.ntile_w) * a.Wn;
+      for (int pg = 0; pg < npass_g; ++pg)
+        for (int pw = 0; pw < npass_w; ++pw, ++e) {
+          const int gp0 = pg * a.Gp, wp0 = pw * a.Wp;
+          const int Gpc = min(a.Gp, a.G - gp0), Wpc = min(a.Wp, a.Wn - wp0);
+          const int buf = e % a.nbuf;
+          mbar_wait(&sfull[buf], (e / a.nbuf) & 1);
+          const uint32_t sb = stg_e + (uint32_t)buf * buf_bytes_e;
+          const int ntask = Gpc * Wpc * h;
+          for (int task = et; task < ntask; task += kEpiThreads) {
+            const int item = task / h, ii = task - item * h;
+            const int gl = item / Wpc, wl = item - gl * Wpc;
+            const uint32_t p0 = sb + (uint32_t)((gl * ns * ldt + wl * 2 * ns) * 8);   // plane 0: [i][re j | im j]
+            const int i2 = ns - 1 - ii, n1 = ns - 1 - ii;                             // n1 pairs in row ii, ii in row i2
+            // byte addresses of T_ij (row walk, +8 per pair) and T_ji (column walk, +8 ldt per pair)
+            uint32_t aij = p0 + (uint32_t)((ii * ldt + ii + 1) * 8), aji = p0 + (uint32_t)(((ii + 1) * ldt + ii) * 8);
+            const int nk = (i2 == ii) ? n1 : ns - 1;        // odd ns: the middle row is its own partner
+            // two pairs per trip on separate accumulators: an FP64 add or multiply of these warps queues behind the
+            // consumers' DMMAs (same pipe), so the dependent chain is what takes the time
+            double vr = 0.0, vi = 0.0, ur = 0.0, ui = 0.0;
+            for (int k = 0; k < nk; k += 2) {
+              if (k == n1) {                                // switch to row i2
+                aij = p0 + (uint32_t)((i2 * ldt + i2 + 1) * 8);
+                aji = p0 + (uint32_t)(((i2 + 1) * ldt + i2) * 8);
+              }
+              double ar = lds64(aij), ai = lds64(aij + ns8);
+              double br = lds64(aji), bi = lds64(aji + ns8);
+              if (a.pair) {
+                ar -= lds64(aij + plane_off + ns8); ai += lds64(aij + plane_off);
+                br -= lds64(aji + plane_off + ns8); bi += lds64(aji + plane_off);
+              }
+              aij += 8; aji += ldt8;
+              vr += ar * br - ai * bi;
+              vi += ar * bi + ai * br;
+              if (k + 1 < nk) {
+                if (k + 1 == n1) {
+                  aij = p0 + (uint32_t)((i2 * ldt + i2 + 1) * 8);
+                  aji = p0 + (uint32_t)(((i2 + 1) * ldt + i2) * 8);
+                }
+                double cr = lds64(aij), ci = lds64(aij + ns8);
+                double dr = lds64(aji), di = lds64(aji + ns8);
+                if (a.pair) {
+                  cr -= lds64(aij + plane_off + ns8); ci += lds64(aij + plane_off);
+                  dr -= lds64(aji + plane_off + ns8); di += lds64(aji + plane_off);
+                }
+                aij += 8; aji += ldt8;
+                ur += cr * dr - ci * di;
+                ui += cr * di + ci * dr;
+              }
+            }
+            vr += ur; vi += ui;
+            vr *= 2.0; vi *= 2.0;
+            double xr = 0.0, xi = 0.0;
+            for (int q = 0; q < (i2 == ii ? 1 : 2); ++q) {                    // the two diagonal elements
+              const uint32_t o = p0 + (uint32_t)((q ? i2 : ii) * (ldt + 1) * 8);
+              double ar = lds64(o), ai = lds64(o + ns8);
+              if (a.pair) { ar -= lds64(o + plane_off + ns8); ai += lds64(o + plane_off); }
+              vr += ar * ar - ai * ai;
+              vi += 2.0 * ar * ai;
+              xr += ar; xi += ai;
+            }
+            const uint32_t c = part_e + (uint32_t)((((gp0 + gl) * a.Wn + wp0 + wl) * h + ii) * 32);
+            sts64(c, vr); sts64(c + 8, vi); sts64(c + 16, xr); sts64(c + 24, xi);
+          }
+          // the stores above depend on every value read from the buffer
+          mbar_arrive(&sempty[buf]);
+        }
+      // fixed-order sums over the tile's vectors and row pairs, between two barriers of the epilogue warps (the
+      // second one frees the table for the next tile)
+      named_bar_sync_epi();
+      // one warp per walker of the tile; a group of hp lanes (hp = h rounded up to a power of two) sums the row
+      // pairs of one vector, 32 / hp vectors at a time, in a fixed order
+      for (int wl = ew; wl < a.Wn; wl += kEpiWarps) {
+        const int w = w0 + wl;
+        const int sub = lane / hp, k = lane & (hp - 1);
+        double sr = 0.0, si = 0.0;
+        for (int gl0 = 0; gl0 < a.G; gl0 += 32 / hp) {
+          const int gl = gl0 + sub;
+          const bool valid = gl < a.G && k < h;
+          double vr = 0.0, vi = 0.0, xr = 0.0, xi = 0.0;
+          if (valid) {
+            const uint32_t c = part_e + (uint32_t)(((gl * a.Wn + wl) * h + k) * 32);
+            vr = lds64(c); vi = lds64(c + 8); xr = lds64(c + 16); xi = lds64(c + 24);
+          }
+          for (int o = hp >> 1; o > 0; o >>= 1) {
+            vr += __shfl_xor_sync(0xffffffffu, vr, o);
+            vi += __shfl_xor_sync(0xffffffffu, vi, o);
+            xr += __shfl_xor_sync(0xffffffffu, xr, o);
+            xi += __shfl_xor_sync(0xffffffffu, xi, o);
+          }
+          sr += vr; si += vi;
+          if (k == 0 && gl < a.G && w < a.nw && g0 + gl < a.n_chol) {
+            double* xo = a.X + ((size_t)(g0 + gl) * a.nw + w) * 2;
+            if (a.accumulate) { xo[0] += xr; xo[1] += xi; } else { xo[0] = xr; xo[1] = xi; }
+          }
+        }
+        for (int o = 16; o >= hp; o >>= 1) {
+          sr += __shfl_xor_sync(0xffffffffu, sr, o);
+          si += __shfl_xor_sync(0xffffffffu, si, o);
+        }
+        if (lane == 0 && w < a.nw) {
+          double* eo = a.expart + ((size_t)tg * a.nw + w) * 2;
+          eo[0] = sr; eo[1] = si;
+        }
+      }
+      named_bar_sync_epi();
     }
     return;
   }
@@ -104,208 +299,239 @@ exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant_
   // -------------------------------------------------------------------- consumer warps
   reg_alloc<Cfg::CREGS>();
   const int g = lane >> 2, t = lane & 3;
-  const int wm = warp % WM, wn = warp / WM;
   const int p = rperm(g);
+  const unsigned rc = a.rect[warp];
+  const int r0 = rc & 255, mi = (rc >> 8) & 255, c0 = (rc >> 16) & 255, ni = rc >> 24;
   const uint32_t lane0 = (uint32_t)(p * 128 + ((t ^ p) << 4));
-  const uint32_t lane1 = (uint32_t)(p * 128 + (((t ^ p) ^ 4) << 4));
   const uint32_t tiles_u32 = smem_u32(tiles);
-  const uint32_t aoff = (uint32_t)(wm * MI) * 1024u;
-  const uint32_t boff = (uint32_t)(TA * 128) + (uint32_t)(wn * NI) * 1024u;
-  const int ns = a.ns, RA = a.G * ns;
+  const uint32_t a0 = tiles_u32 + (uint32_t)r0 * 1024u + lane0;
+  const uint32_t b0 = tiles_u32 + (uint32_t)(TAr * 128) + (uint32_t)c0 * 1024u + lane0;
+  const uint32_t full_u32 = smem_u32(full), empty_u32 = smem_u32(empty);
+  const uint32_t ring_bytes = (uint32_t)S * stage_bytes;
+  const uint32_t stg_u32 = smem_u32(stg), buf_bytes = (uint32_t)(srows * ldt * 8);
+  const uint32_t sfull_u32 = smem_u32(sfull), sempty_u32 = smem_u32(sempty);
+  const int Gns = a.G * ns, rows_all = planes * Gns;
 
-  uint32_t it = 0;
+  // the rectangle is one of (MI | MI - 1) x (NI | NI - 1) for every plan of a production shape
+  const int variant = (mi == MI && ni == NI) ? 0 : (mi == MI - 1 && ni == NI) ? 1 : (mi == MI && ni == NI - 1) ? 2
+                      : (mi == MI - 1 && ni == NI - 1) ? 3 : 4;
+  uint32_t d = 0;
+  Ring ring = {0u, 0u, 0u, -1};
   for (int tile = blockIdx.x; tile < a.ntiles; tile += gridDim.x) {
-    const int tg = tile / a.ntile_w;
-    const int g0 = tg * a.G, w0 = (tile % a.ntile_w) * a.Wn;
-
     double acc[MI][NI][2];
 #pragma unroll
     for (int i = 0; i < MI; ++i)
 #pragma unroll
       for (int j = 0; j < NI; ++j) acc[i][j][0] = acc[i][j][1] = 0.0;
 
-    for (int kt = 0; kt < KT; ++kt, ++it) {
-      const int s = it % S;
-      mbar_wait(&full[s], (it / S) & 1);
-      consumer_release_prev(empty, it, S, lane);
-      const uint32_t sa = tiles_u32 + (uint32_t)s * Cfg::STAGE_BYTES + aoff;
-      const uint32_t sb = tiles_u32 + (uint32_t)s * Cfg::STAGE_BYTES + boff;
-#pragma unroll
-      for (int kp = 0; kp < 2; ++kp) {
-        const uint32_t lo = kp ? lane1 : lane0;
-        double2 af[MI];
-#pragma unroll
-        for (int i = 0; i < MI; ++i) af[i] = lds128(sa + i * 1024 + lo);
-#pragma unroll
-        for (int j = 0; j < NI; ++j) {
-          const double2 bf = lds128(sb + j * 1024 + lo);
-#pragma unroll
-          for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].x, bf.x);
-#pragma unroll
-          for (int i = 0; i < MI; ++i) dmma884(acc[i][j][0], acc[i][j][1], af[i].y, bf.y);
-        }
-      }
+    switch (variant) {
+      case 0: xws_kloop<MI, NI, MI, NI, false>(acc, full_u32, empty_u32, KT, ring_bytes, stage_bytes, ring, a0, b0, lane, mi, ni); break;
+      case 1: xws_kloop<MI, NI, MI - 1, NI, false>(acc, full_u32, empty_u32, KT, ring_bytes, stage_bytes, ring, a0, b0, lane, mi, ni); break;
+      case 2: xws_kloop<MI, NI, MI, NI - 1, false>(acc, full_u32, empty_u32, KT, ring_bytes, stage_bytes, ring, a0, b0, lane, mi, ni); break;
+      case 3: xws_kloop<MI, NI, MI - 1, NI - 1, false>(acc, full_u32, empty_u32, KT, ring_bytes, stage_bytes, ring, a0, b0, lane, mi, ni); break;
+      default: xws_kloop<MI, NI, MI, NI, true>(acc, full_u32, empty_u32, KT, ring_bytes, stage_bytes, ring, a0, b0, lane, mi, ni); break;
     }
 
-    // ------------------------------------------------------------------ epilogue
-    const int ldt = a.ldt;
-    const int nsns = ns * ns;
-    for (int wp0 = 0; wp0 < a.Wn; wp0 += a.Wp) {
-      const int Wp = min(a.Wp, a.Wn - wp0);
-      const int clo = wp0 * 2 * ns, chi = (wp0 + Wp) * 2 * ns;
-      // (1) stage the columns of walkers [wp0, wp0 + Wp)
+    // ---------------------------------------------------------------- dump, one pass at a time
+    // (32-bit shared addresses, one predicate bit per store: this code runs on the DMMA warps' time)
+    for (int pg = 0; pg < npass_g; ++pg)
+      for (int pw = 0; pw < npass_w; ++pw, ++d) {
+        const int gp0 = pg * a.Gp, wp0 = pw * a.Wp;
+        const int rlo = gp0 * ns, rhi = min(a.Gp, a.G - gp0) * ns + rlo;
+        const int clo = wp0 * 2 * ns, chi = min(a.Wp, a.Wn - wp0) * 2 * ns + clo;
+        unsigned m0 = 0, m1 = 0;               // bit j: column 8 (c0 + j) + t (+ 4) belongs to this pass
 #pragma unroll
-      for (int i = 0; i < MI; ++i) {
-        const int r = 8 * (wm * MI + i) + p;
-        if (r < RA) {
+        for (int j = 0; j < NI; ++j) {
+          const int c = 8 * (c0 + j) + t;
+          m0 |= (j < ni && c >= clo && c < chi) ? 1u << j : 0u;
+          m1 |= (j < ni && c + 4 >= clo && c + 4 < chi) ? 1u << j : 0u;
+        }
+        uint32_t buf_u32 = stg_u32;
+        uint32_t bar_off = 0;
+        if (a.nbuf == 2 && (d & 1)) { buf_u32 += buf_bytes; bar_off = 8; }
+        mbar_wait_u32(sempty_u32 + bar_off, (a.nbuf == 2 ? (d >> 1) & 1 : d & 1) ^ 1);
 #pragma unroll
-          for (int j = 0; j < NI; ++j) {
-            const int c = 8 * (wn * NI + j) + t;
-            if (c >= clo && c < chi) stg[(size_t)r * ldt + (c - clo)] = acc[i][j][0];
-            if (c + 4 >= clo && c + 4 < chi) stg[(size_t)r * ldt + (c + 4 - clo)] = acc[i][j][1];
-          }
-        }
-      }
-      named_bar_sync(1, NCT);
-      // (2) work items (gamma_local, walker_local, slice of the (i, j) range)
-      const int nitems = a.G * Wp * a.split;
-      const int chunk = (nsns + a.split - 1) / a.split;
-      for (int item = warp; item < nitems; item += NCW) {
-        const int sl = item % a.split, gw = item / a.split;
-        const int wl = gw % Wp, gl = gw / Wp;
-        const double* pr = stg + (size_t)(gl * ns) * ldt + wl * 2 * ns;
-        const double* pi = pr + ns;
-        double vr = 0.0, vi = 0.0, xr = 0.0, xi = 0.0;
-        const int e1 = min(nsns, (sl + 1) * chunk);
-        for (int idx = sl * chunk + lane; idx < e1; idx += 32) {
-          const int i = idx / ns, j = idx - i * ns;
-          const double ar = pr[i * ldt + j], ai = pi[i * ldt + j];
-          const double br = pr[j * ldt + i], bi = pi[j * ldt + i];
-          vr += ar * br - ai * bi;
-          vi += ar * bi + ai * br;
-          if (i == j) { xr += ar; xi += ai; }
-        }
+        for (int i = 0; i < MI; ++i) {
+          const int r = 8 * (r0 + i) + p;
+          const int pl = r >= Gns ? 1 : 0;
+          const int rr = r - pl * Gns;
+          if (i < mi && r < rows_all && rr >= rlo && rr < rhi) {
+            const uint32_t row = buf_u32 + (uint32_t)(((pl * a.Gp * ns + rr - rlo) * ldt + 8 * c0 + t - clo) * 8);
 #pragma unroll
-        for (int o = 16; o > 0; o >>= 1) {
-          vr += __shfl_down_sync(0xffffffffu, vr, o);
-          vi += __shfl_down_sync(0xffffffffu, vi, o);
-          xr += __shfl_down_sync(0xffffffffu, xr, o);
-          xi += __shfl_down_sync(0xffffffffu, xi, o);
-        }
-        if (lane == 0) {
-          comb[item * 4 + 0] = vr; comb[item * 4 + 1] = vi;
-          comb[item * 4 + 2] = xr; comb[item * 4 + 3] = xi;
-        }
-      }
-      named_bar_sync(1, NCT);
-      // (3) fixed-order final sums
-      for (int wl = tid; wl < Wp; wl += NCT) {
-        const int w = w0 + wp0 + wl;
-        if (w < a.nw) {
-          double sr = 0.0, si = 0.0;
-          for (int gl = 0; gl < a.G; ++gl)
-            for (int sl = 0; sl < a.split; ++sl) {
-              const int item = (gl * Wp + wl) * a.split + sl;
-              sr += comb[item * 4 + 0];
-              si += comb[item * 4 + 1];
+            for (int j = 0; j < NI; ++j) {
+              if (m0 >> j & 1) sts64(row + j * 64, acc[i][j][0]);
+              if (m1 >> j & 1) sts64(row + j * 64 + 32, acc[i][j][1]);
             }
-          double* eo = a.expart + ((size_t)tg * a.nw + w) * 2;
-          eo[0] = sr; eo[1] = si;
-        }
-      }
-      for (int gw = NCT - 1 - tid; gw < a.G * Wp; gw += NCT) {
-        const int wl = gw % Wp, gl = gw / Wp;
-        const int w = w0 + wp0 + wl, gg = g0 + gl;
-        if (w < a.nw && gg < a.n_chol) {
-          double xr = 0.0, xi = 0.0;
-          for (int sl = 0; sl < a.split; ++sl) {
-            xr += comb[(gw * a.split + sl) * 4 + 2];
-            xi += comb[(gw * a.split + sl) * 4 + 3];
           }
-          double* xo = a.X + ((size_t)gg * a.nw + w) * 2;
-          if (a.accumulate) { xo[0] += xr; xo[1] += xi; } else { xo[0] = xr; xo[1] = xi; }
         }
+        mbar_arrive_u32(sfull_u32 + bar_off);
       }
-      // the next pass (or tile) overwrites stg / comb only after its own first barrier;
-      // that barrier is reached by every thread after it has finished (3)
-      named_bar_sync(1, NCT);
-    }
   }
 }
 
 struct Plan {
-  int cfg = -1;       // index into the instantiation table
-  int G = 0, Wn = 0, Wp = 0, ldt = 0, stages = 0, split = 1;
+  int inst = -1;      // index into kInst
+  int WM = 0;         // warp grid rows
+  int ncw = 0, G = 0, Wn = 0, Gp = 0, Wp = 0, ldt = 0, stages = 0, nbuf = 1;
+  int rowsA = 0, rowsB = 0;
+  unsigned rect[kMaxWarps] = {};
   size_t smem = 0;
-  double eff = 0.0;
+  double eff = 0.0;     // useful share of the issued DMMA blocks
+  double score = 0.0;   // useful flops per modelled cycle
+  double bpf = 1e30;    // operand bytes per useful flop (shared-memory fill traffic out of L2)
 };
 
-struct Inst { int WM, WN, MI, NI; };
-constexpr Inst kInst[] = {{4, 3, 4, 7}, {4, 2, 5, 5}, {4, 2, 5, 7}, {4, 2, 6, 6}};
+struct Inst { int NCW, MI, NI; };
+constexpr Inst kInst[] = {{8, 5, 7}, {8, 7, 5}, {8, 6, 6}, {12, 4, 7}, {12, 7, 4}, {12, 5, 5}, {12, 5, 4}, {12, 4, 5}};
 constexpr int kNumInst = sizeof(kInst) / sizeof(kInst[0]);
 
-Plan make_plan(int ns) {
-  Plan best;
+// staging row stride: stride mod 16 in {6, 10} spreads the accumulator dump (8 rows x 4 columns per store
+// instruction) over all banks exactly twice and keeps the column reads of the epilogue warps 4-way at worst
+int staging_stride(int cols) {
+  int l = cols;
+  while (l % 16 != 6 && l % 16 != 10) ++l;
+  return l;
+}
+
+// Deal nbr x nbc blocks to a WM x WN grid of near-equal rectangles and the rectangles to warp ids so that the
+// four sub-partitions (warp id mod 4) carry about the same number of DMMA blocks.  Returns the largest
+// sub-partition load; fails (-1) if a rectangle exceeds MI x NI.
+int deal_rectangles(int nbr, int nbc, int WM, int WN, int MI, int NI, unsigned* rect) {
+  const int ncw = WM * WN;
+  struct R { int r0, mi, c0, ni; };
+  std::vector<R> rs;
+  for (int wn = 0; wn < WN; ++wn)
+    for (int wm = 0; wm < WM; ++wm) {
+      R r;
+      r.mi = nbr / WM + (wm < nbr % WM ? 1 : 0);
+      r.r0 = wm * (nbr / WM) + std::min(wm, nbr % WM);
+      r.ni = nbc / WN + (wn < nbc % WN ? 1 : 0);
+      r.c0 = wn * (nbc / WN) + std::min(wn, nbc % WN);
+      if (r.mi > MI || r.ni > NI) return -1;
+      rs.push_back(r);
+    }
+  std::stable_sort(rs.begin(), rs.end(), [](const R& x, const R& y) { return x.mi * x.ni > y.mi * y.ni; });
+  int load[4] = {0, 0, 0, 0}, cnt[4] = {0, 0, 0, 0};
+  for (const R& r : rs) {           // largest first, to the lightest sub-partition that still has a warp slot
+    int best = -1;
+    for (int s = 0; s < 4; ++s)
+      if (cnt[s] < ncw / 4 && (best < 0 || load[s] < load[best])) best = s;
+    const int warp = best + 4 * cnt[best];
+    rect[warp] = (unsigned)r.r0 | ((unsigned)r.mi << 8) | ((unsigned)r.c0 << 16) | ((unsigned)r.ni << 24);
+    load[best] += r.mi * r.ni;
+    cnt[best] += 1;
+  }
+  return std::max(std::max(load[0], load[1]), std::max(load[2], load[3]));
+}
+
+// shared memory beside the ring and the staging buffers: partial-sum table, barriers, alignment slack
+size_t fixed_smem(int ns, int nitems) {
+  return (size_t)nitems * ((ns + 1) / 2) * 32 + 16 * 8 + 64;
+}
+
+// Cycle model of one tile on one SM (measured on B200, profiles/r2_exchange.md): the main loop runs at 64 clocks per
+// DMMA block and k-tile on the busiest sub-partition unless the fill of the stage out of L2 is slower (c5 sustains
+// 21 B/clk/SM at 92 % of the DMMA peak; 30 taken as the ceiling); every pass costs the DMMA warps a dump; the
+// epilogue warps need about 150 + 30 (ns - 1) clocks per round of 96 lane tasks and stall the consumers when a tile
+// has more passes than staging buffers, or when they cannot keep up with a short K loop.
+std::vector<Plan> enumerate_plans(int ns, bool pair, int KT) {
+  const int planes = pair ? 2 : 1;
+  const int h = (ns + 1) / 2;
+  auto t_epi = [&](int items) { return 300.0 + ((items * h + kEpiThreads - 1) / kEpiThreads) * (150.0 + 30.0 * (ns - 1)); };
+  std::vector<Plan> cands;
   for (int c = 0; c < kNumInst; ++c) {
     const Inst& I = kInst[c];
-    const int TA = 8 * I.WM * I.MI, TB = 8 * I.WN * I.NI, ncw = I.WM * I.WN;
-    Plan p;
-    p.cfg = c;
-    p.G = TA / ns;
-    p.Wn = TB / (2 * ns);
-    if (p.G < 1 || p.Wn < 1) continue;
-    if (p.G > 256) p.G = 256;
-    if (p.Wn > 256) p.Wn = 256;
-    p.eff = (double)(p.G * ns) * (p.Wn * 2 * ns) / ((double)TA * TB);
-    const int RAp = (p.G * ns + 7) & ~7;
-    const size_t fixed = 256 * 4 * 8 + 2 * 8 * 8 + 1024;   // comb + barriers + alignment slack
-    // The staging shape with the FEWEST epilogue passes first (Wp walkers of the tile at a time), then the deepest
-    // ring that still fits beside it.  Measured on B200: the operands come out of L2 and two stages already keep
-    // the DMMA pipe fed, while every extra epilogue pass costs three CTA-wide barriers (c2: 5 passes with 4 stages
-    // 4.26 ms, 2 passes with 2 stages 3.4 ms; c5 and c4 keep 3 stages and 2 passes).
-    bool ok = false;
-    int best_passes = 1 << 30;
-    for (int S = 4; S >= 2; --S) {
-      const size_t pipe = (size_t)S * (TA + TB) * 128;
-      for (int Wp = p.Wn; Wp >= 1; --Wp) {
-        const int ldt = (Wp * 2 * ns) | 1;
-        const size_t tot = pipe + (size_t)RAp * ldt * 8 + fixed;
-        if (tot > (size_t)kSmemMax) continue;
-        int split = 1, wp = Wp;
-        while (p.G * wp * split < ncw && split < 8) split *= 2;
-        while (p.G * wp * split > 256 && wp > 1) wp -= 1;      // items per pass must fit the comb table
-        if (p.G * wp * split > 256) continue;
-        const int passes = (p.Wn + wp - 1) / wp;
-        if (passes < best_passes) {             // strictly fewer: the deeper ring wins ties (S descends)
-          best_passes = passes;
-          p.stages = S; p.Wp = wp; p.ldt = (wp * 2 * ns) | 1; p.split = split;
-          p.smem = pipe + (size_t)RAp * p.ldt * 8 + fixed;
-          ok = true;
+    for (int WM = 1; WM <= I.NCW; ++WM) {
+      if (I.NCW % WM) continue;
+      const int WN = I.NCW / WM;
+      const int Gmax = std::min(255, 8 * WM * I.MI / (planes * ns)), Wmax = std::min(255, 8 * WN * I.NI / (2 * ns));
+      for (int G = 1; G <= Gmax; ++G)
+        for (int Wn = 1; Wn <= Wmax; ++Wn) {
+          if (G * Wn * ((ns + 1) / 2) > kMaxTasks) continue;
+          Plan p;
+          p.inst = c; p.ncw = I.NCW; p.G = G; p.Wn = Wn; p.WM = WM;
+          p.rowsA = planes * G * ns; p.rowsB = Wn * 2 * ns;
+          const int nbr = (p.rowsA + 7) / 8, nbc = (p.rowsB + 7) / 8;
+          const int maxload = deal_rectangles(nbr, nbc, WM, WN, I.MI, I.NI, p.rect);
+          if (maxload < 0) continue;
+          const double useful = (double)p.rowsA * p.rowsB;
+          const double bytes = (double)(p.rowsA + p.rowsB) * 128.0;
+          p.eff = useful / (256.0 * maxload);
+          p.bpf = bytes / useful;
+          const size_t stage = (size_t)(8 * nbr + 8 * nbc) * 128;
+          const size_t fixed = fixed_smem(ns, G * Wn);
+          for (int S = 3; S >= 2; --S) {
+            if (S * stage + fixed >= (size_t)kSmemMax) continue;
+            const size_t left = (size_t)kSmemMax - fixed - S * stage;
+            // as few passes as fit beside the ring; two buffers as soon as there is more than one pass
+            int bp = 1 << 30;
+            Plan q = p;
+            for (int Gp = G; Gp >= 1; --Gp)
+              for (int Wp = Wn; Wp >= 1; --Wp) {
+                const int passes = ((G + Gp - 1) / Gp) * ((Wn + Wp - 1) / Wp);
+                const int nbuf = passes > 1 ? 2 : 1;
+                const int ldt = staging_stride(Wp * 2 * ns);
+                const size_t need = (size_t)nbuf * planes * Gp * ns * ldt * 8;
+                if (need > left || passes >= bp) continue;
+                bp = passes;
+                q.Gp = Gp; q.Wp = Wp; q.ldt = ldt; q.nbuf = nbuf; q.stages = S;
+                q.smem = S * stage + need + fixed;
+              }
+            if (bp == 1 << 30) continue;
+            // 12 consumer warps run on 152 registers (a few spills in the k loop), 8 on 224: measured 2 % apart
+            double main = KT * std::max(64.0 * maxload, bytes / 30.0) * (S == 2 ? 1.03 : 1.0) * (I.NCW == 12 ? 1.02 : 1.0);
+            const double dump = bp * (I.NCW / 4) * (6.0 * I.MI * I.NI + 150.0);
+            const double epi_pass = t_epi(q.Gp * q.Wp);
+            const double stall = std::max(0, bp - q.nbuf) * epi_pass;
+            const double epi_all = bp * epi_pass + 300.0;
+            // rectangles other than (MI | MI - 1) x (NI | NI - 1) run the predicated k loop
+            bool generic = false;
+            for (int w = 0; w < I.NCW; ++w) {
+              const int mi = (q.rect[w] >> 8) & 255, ni = q.rect[w] >> 24;
+              generic = generic || mi < I.MI - 1 || ni < I.NI - 1;
+            }
+            if (generic) main *= 1.15;
+            const double t_tile = std::max(main + 800.0 + dump + stall, epi_all);
+            q.score = useful * KT / t_tile;
+            cands.push_back(q);
+          }
         }
-        break;                                  // smaller Wp only means more passes at this S
-      }
     }
-    if (!ok) continue;
-    if (p.eff > best.eff + 1e-9) best = p;
+  }
+  return cands;
+}
+
+Plan make_plan(int ns, bool pair, int KT) {
+  const std::vector<Plan> cands = enumerate_plans(ns, pair, KT);
+  // the most useful work per cycle; among plans within 1 % of it the one that moves the fewest bytes per flop (the
+  // squarest tile), then the deeper ring
+  Plan best;
+  double top = 0.0;
+  for (const Plan& p : cands) top = std::max(top, p.score);
+  for (const Plan& p : cands) {
+    if (p.score < 0.99 * top) continue;
+    if (best.inst < 0 || p.bpf < best.bpf - 1e-12 || (p.bpf < best.bpf + 1e-12 && p.stages > best.stages)) best = p;
   }
   return best;
 }
 
-template <int WM, int WN, int MI, int NI>
+template <int NCW, int MI, int NI>
 int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
-  using Cfg = XwsCfg<WM, WN, MI, NI>;
-  auto kern = exchange_ws_kernel<WM, WN, MI, NI>;
+  using Cfg = XwsCfg<NCW, MI, NI>;
+  auto kern = exchange_ws_kernel<NCW, MI, NI>;
   static uint64_t attr = 0;
   if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
   }
   const int nsm = sm_count_current();
+  const bool pair = e.plane_stride != 0;
   TensorMap tmA, tmB;
   {
-    const uint64_t dims[3] = {(uint64_t)e.M, (uint64_t)e.Nt, (uint64_t)e.n_chol};
-    const uint64_t str[2] = {(uint64_t)e.M * 8, (uint64_t)e.Nt * e.M * 8};
-    const uint32_t box[3] = {16, (uint32_t)e.ns, (uint32_t)p.G};
-    if (make_tensor_map_f64(&tmA, e.Lrot, 3, dims, str, box) != 0) return -1;
+    const uint64_t dims[4] = {(uint64_t)e.M, (uint64_t)e.Nt, (uint64_t)e.n_chol, (uint64_t)(pair ? 2 : 1)};
+    const uint64_t str[3] = {(uint64_t)e.M * 8, (uint64_t)e.Nt * e.M * 8,
+                             pair ? (uint64_t)e.plane_stride * 8 : (uint64_t)e.n_chol * e.Nt * e.M * 8};
+    const uint32_t box[4] = {16, (uint32_t)e.ns, (uint32_t)p.G, (uint32_t)(pair ? 2 : 1)};
+    if (make_tensor_map_f64(&tmA, e.Lrot, 4, dims, str, box) != 0) return -1;
   }
   {
     const uint64_t dims[4] = {(uint64_t)e.M, (uint64_t)e.Nt, 2, (uint64_t)e.nw};
@@ -316,13 +542,30 @@ int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
   XwsArgs a;
   a.expart = e.expart; a.X = e.X;
   a.M = e.M; a.ns = e.ns; a.off = e.off; a.n_chol = e.n_chol; a.nw = e.nw;
-  a.G = p.G; a.Wn = p.Wn; a.Wp = p.Wp; a.ldt = p.ldt; a.stages = p.stages; a.split = p.split;
+  a.G = p.G; a.Wn = p.Wn; a.Gp = p.Gp; a.Wp = p.Wp; a.ldt = p.ldt; a.stages = p.stages; a.nbuf = p.nbuf;
+  a.rowsA = p.rowsA; a.rowsB = p.rowsB;
   a.ntile_w = (e.nw + p.Wn - 1) / p.Wn;
   a.ntiles = a.ntile_w * ((e.n_chol + p.G - 1) / p.G);
   a.accumulate = e.accumulate;
+  a.pair = pair ? 1 : 0;
+  for (int w = 0; w < kMaxWarps; ++w) a.rect[w] = p.rect[w];
   const int grid = a.ntiles < nsm ? a.ntiles : nsm;
   kern<<<grid, Cfg::THREADS, p.smem, st>>>(tmA, tmB, a);
   return 1;
+}
+
+std::mutex g_plan_mu;
+std::map<long, Plan> g_plan_cache;
+
+const Plan& cached_plan(int ns, bool pair, int M) {
+  std::mutex& mu = g_plan_mu;
+  std::map<long, Plan>& cache = g_plan_cache;
+  const int KT = (M + 15) / 16;
+  const long key = ((long)KT << 8 | ns) << 1 | (pair ? 1 : 0);
+  std::lock_guard<std::mutex> lk(mu);
+  auto it = cache.find(key);
+  if (it == cache.end()) it = cache.emplace(key, make_plan(ns, pair, KT)).first;
+  return it->second;      // std::map nodes are stable
 }
 
 }  // namespace
@@ -331,19 +574,49 @@ bool exchange_ws_usable(int M, const void* Lrot, const void* ThT) {
   return (M % 2 == 0) && (((uintptr_t)Lrot | (uintptr_t)ThT) & 15) == 0;
 }
 
-int exchange_ws_group_size(int ns) { return make_plan(ns).G; }
+int exchange_ws_group_size(int ns, int M, bool pair) { return cached_plan(ns, pair, M).G; }
 
-double exchange_ws_efficiency(int ns) { return make_plan(ns).eff; }
+double exchange_ws_efficiency(int ns, int M, bool pair) { return cached_plan(ns, pair, M).eff; }
+
+// Tuning hook: replace the plan of (ns, M, pair) by the candidate with this warp count, rectangle bound, warp grid
+// and tile (the deepest ring that fits); false if there is no such candidate.
+bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn) {
+  const int KT = (M + 15) / 16;
+  const std::vector<Plan> cands = enumerate_plans(ns, pair, KT);
+  const Plan* pick = nullptr;
+  for (const Plan& p : cands)
+    if (p.ncw == ncw && kInst[p.inst].MI == mi && kInst[p.inst].NI == ni && p.WM == wm && p.G == G && p.Wn == Wn &&
+        (!pick || p.stages > pick->stages))
+      pick = &p;
+  if (!pick) return false;
+  const long key = ((long)KT << 8 | ns) << 1 | (pair ? 1 : 0);
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  g_plan_cache[key] = *pick;
+  return true;
+}
+
+// human-readable plan (bench / tests)
+void exchange_ws_describe(int ns, int M, bool pair, char* out, int n) {
+  const Plan& p = cached_plan(ns, pair, M);
+  if (p.inst < 0) { snprintf(out, n, "no plan"); return; }
+  snprintf(out, n, "warps %d grid %dx%d (<=%dx%d blocks each) G %d Wn %d tile %dx%d eff %.3f stages %d passes %dx%d nbuf %d ldt %d smem %zu",
+           p.ncw, p.WM, p.ncw / p.WM, kInst[p.inst].MI, kInst[p.inst].NI, p.G, p.Wn, p.rowsA, p.rowsB, p.eff, p.stages,
+           (p.G + p.Gp - 1) / p.Gp, (p.Wn + p.Wp - 1) / p.Wp, p.nbuf, p.ldt, p.smem);
+}
 
 // returns launches issued, or -1 if the tensor maps could not be encoded
 int run_exchange_ws(const ExArgs& e, cudaStream_t st) {
-  const Plan p = make_plan(e.ns);
-  if (p.cfg < 0) return -1;
-  switch (p.cfg) {
-    case 0: return launch_xws<4, 3, 4, 7>(e, p, st);
-    case 1: return launch_xws<4, 2, 5, 5>(e, p, st);
-    case 2: return launch_xws<4, 2, 5, 7>(e, p, st);
-    case 3: return launch_xws<4, 2, 6, 6>(e, p, st);
+  const Plan& p = cached_plan(e.ns, e.plane_stride != 0, e.M);
+  if (p.inst < 0) return -1;
+  switch (p.inst) {
+    case 0: return launch_xws<8, 5, 7>(e, p, st);
+    case 1: return launch_xws<8, 7, 5>(e, p, st);
+    case 2: return launch_xws<8, 6, 6>(e, p, st);
+    case 3: return launch_xws<12, 4, 7>(e, p, st);
+    case 4: return launch_xws<12, 7, 4>(e, p, st);
+    case 5: return launch_xws<12, 5, 5>(e, p, st);
+    case 6: return launch_xws<12, 5, 4>(e, p, st);
+    case 7: return launch_xws<12, 4, 5>(e, p, st);
   }
   return -1;
 }

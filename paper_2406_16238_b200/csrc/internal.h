@@ -152,13 +152,17 @@ struct ExArgs {
   int M, Nt, n_chol, nw;
   int off, ns;                  // spin block
   int accumulate;               // 1: add to expart / X (second spin block)
+  long plane_stride = 0;        // != 0 (exchange_ws only): Lrot = Lr + i Li, the imaginary plane starts plane_stride
+                                // doubles after Lrot; T is then the complex product and X = tr(T) of it
 };
 int exchange_group_size(int ns);            // gamma per CTA tile for this block size
 int run_exchange(const ExArgs& a, cudaStream_t st);
 // exchange_ws.cu: warp-specialised TMA version (needs even M and 16-byte aligned operands)
 bool exchange_ws_usable(int M, const void* Lrot, const void* ThT);
-int exchange_ws_group_size(int ns);
-double exchange_ws_efficiency(int ns);
+int exchange_ws_group_size(int ns, int M, bool pair = false);      // the plan depends on the K = M loop length
+double exchange_ws_efficiency(int ns, int M, bool pair = false);
+void exchange_ws_describe(int ns, int M, bool pair, char* out, int n);
+bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn);
 int run_exchange_ws(const ExArgs& a, cudaStream_t st);
 
 struct EnergyArgs {
@@ -251,6 +255,7 @@ struct CEnergyArgs {
   double* E_out;
   int nf, nw, nblk;
   double spin_factor;
+  int pair = 0;                               // 1: Xr holds tr(T) of the complex T, expart[0] its tr(T T) (one run)
 };
 int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStream_t st);
 int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st);

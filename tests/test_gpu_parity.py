@@ -447,8 +447,19 @@ def test_c1_literal_amplitudes():
         Wg, wg, ovg = gpu_step(pr, Wo, w_in, x, cfg.dt)
         o.n_steps_done = 0
         Wn, wn, ovn = o.step(Wo, w_in, x, cfg.dt)
-        assert rel_fro(Wg, Wn) < TOL_STEP, (s, rel_fro(Wg, Wn))
-        assert rel_max(ovg, ovn) < TOL_STEP, s
+        # Conditioning of the stress regime (values from the oracle): the blown-up walkers have nearly dependent
+        # columns, cond(O) = cond(psi^T phi) grows from 1 to 3e6 over the ten steps.  Theta = phi O^-1 (hence xbar, A
+        # and the propagated walker) amplifies FP64 rounding by cond(O_old), a determinant by cond of its matrix.
+        # With 1e-14 (a hundred ulps) as the agreement of two FP64 evaluations in different summation orders the
+        # bars are 1e-10 max(1, 1e-4 cond): the plain 1e-10 up to cond = 1e4.
+        blk = slice(0, cfg.n_alpha)
+        c_old = np.array([np.linalg.cond(pr.trial[:, blk].T @ Wo[k][:, blk]) for k in range(nw)])
+        c_new = np.array([np.linalg.cond(pr.trial[:, blk].T @ Wn[k][:, blk]) for k in range(nw)])
+        a_old = np.maximum(1.0, 1e-4 * c_old)
+        a_new = np.maximum(1.0, 1e-4 * (c_old + c_new))
+        dW = np.linalg.norm((Wg - Wn).reshape(nw, -1), axis=1) / np.linalg.norm(Wn.reshape(nw, -1), axis=1)
+        assert np.all(dW < TOL_STEP * a_old), (s, dW.max(), c_old.max())
+        assert np.all(np.abs(ovg - ovn) < TOL_STEP * a_new * np.abs(ovn)), (s, c_new.max())
         for k in range(nw):
             if abs(cos[k]) < 1e-9:
                 borderline.append((s, k))
@@ -457,7 +468,7 @@ def test_c1_literal_amplitudes():
                 assert wg[k] == 0.0, (s, k, wg[k], cos[k])
                 zeros_seen += 1
             else:
-                amp = max(1.0, abs(info["c_fb"][k]) + abs(info["c_mf"][k]))
+                amp = max(1.0, abs(info["c_fb"][k]) + abs(info["c_mf"][k])) * a_new[k]
                 assert abs(wg[k] - wn[k]) < TOL_STEP * amp * wn[k], (s, k, wg[k], wn[k], amp)
         _, wo, _ = Wn, wo * (wn / w_in), ovn
         Wo = Wn
