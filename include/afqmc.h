@@ -86,7 +86,7 @@ typedef struct {
                         /* M and n_chol.  Results agree with the double path to ~1e-6 relative.      */
   int32_t complex_chol; /* 1: complex Cholesky vectors.  L_chol is DEVICE complex128     */
                         /* [n_chol][M][M] with (ps|qr) = sum_g L^g_ps conj(L^g_rq) a (ps|qr) = (qr|ps)      */
-                        /* symmetric tensor, h1 is EITHER complex128 [M][M] Hermitian, the trial stays real. */
+                        /* symmetric tensor, h1 is EITHER complex128 [M][M] Hermitian; trial: see complex_trial. */
                         /* The handle works with the 2 n_chol Hermitian matrices A_g = (L_g + L_g^+)/2,      */
                         /* B_g = (L_g - L_g^+)/(2i): aux_fields is [nw][2 n_chol] (fields of the A_g first), */
                         /* L_chol is not referenced after afqmc_create; a set that does not factorise a      */
@@ -96,6 +96,18 @@ typedef struct {
                         /* kernels otherwise.  1: force the cp.async kernels (what odd M runs; lets a test cover   */
                         /* them at even M on the same inputs).  2: the one-kernel overlap / Theta route instead of */
                         /* the batched DMMA GEMMs.  Results agree to rounding; ignored for group_size > 1.         */
+  int32_t complex_trial; /* 1: `trial` is complex128 [M][Nt] (PAPER.md:219 gives the trial no dtype; PAPER.md:328:   */
+                        /* magnetic fields, spin-orbit coupling, Bloch orbitals).  <Psi_T| carries conj(psi):       */
+                        /* O = psi^+ phi, Lrot = psi^+ K, hrot = psi^+ h, P = psi psi^+, m_g = tr(K_g P) (real).    */
+                        /* Needs complex_chol = 1 (a real tensor is passed as complex vectors with zero imaginary  */
+                        /* part; half of the 2 n_chol fields then multiply zero matrices).                          */
+  int32_t reserved0;    /* must be 0 (keeps the doubles below 8-byte aligned)                                       */
+  double xbar_bound;    /* > 0: every component of the force-bias shift is capped in modulus, xbar_g <- xbar_g      */
+                        /* min(1, bound / |xbar_g|), BEFORE xs, c_fb and c_mf are formed (Eqs. 12, 16 hold for any  */
+                        /* xbar, so the estimator stays exact).  0: no bound (default).  SURVEY 8f NEXT-1, S8.      */
+  double ehyb_bound;    /* > 0: the modulus of the importance function is bounded, |I| <- exp(-dt clip(D, -b, b))   */
+                        /* with D = -log|I| / dt (the real part of the hybrid energy relative to E_shift); the      */
+                        /* phase factor max(0, cos theta) is untouched.  0: no bound (default).                     */
 } afqmc_params;
 
 /* Setup (Eqs. 4-6; mean-field shift PAPER.md:108;

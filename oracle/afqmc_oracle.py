@@ -59,7 +59,7 @@ class AFQMCOracle:
 
     # ------------------------------------------------------------------ O0 create
     def __init__(self, h1, L, trial, n_alpha, n_beta, walker_kind,
-                 taylor_order=6, ortho_every=0, e_shift=None, n_chol=None):
+                 taylor_order=6, ortho_every=0, e_shift=None, n_chol=None, xbar_bound=0.0, ehyb_bound=0.0):
         h1 = np.asarray(h1, dtype=np.float64)
         trial = np.asarray(trial, dtype=np.float64)
         self.M = M = h1.shape[0]
@@ -69,6 +69,8 @@ class AFQMCOracle:
         self.ortho_every = int(ortho_every)
         self.n_steps_done = 0
         self.L = L
+        # optional bounds (reading S8b in DESIGN.md); 0 = off, the paper's own algorithm
+        self.xbar_bound, self.ehyb_bound = float(xbar_bound), float(ehyb_bound)
         if self.walker_kind == 0:
             if n_alpha != n_beta:
                 raise ValueError("RHF walkers need n_alpha == n_beta")
@@ -207,6 +209,12 @@ class AFQMCOracle:
         xbar = 1j * sq * (X - self.m[None, :])
         if xbar_override is not None:
             xbar = np.broadcast_to(np.asarray(xbar_override, dtype=np.complex128), X.shape)
+        elif self.xbar_bound > 0.0:
+            # S8b: cap the modulus of every component, keep its phase.  Eqs. (12), (16) hold for ANY xbar, and
+            # xs, c_fb, c_mf below are formed from the xbar actually used.
+            mag = np.abs(xbar)
+            with np.errstate(all="ignore"):
+                xbar = xbar * np.where(mag > self.xbar_bound, self.xbar_bound / mag, 1.0)
         xs = x - xbar                                        # O4, Eq. (12)
         # Eq. (16) exponent; bilinear sums, no conjugation (reading S14)
         c_fb = np.sum(x * xbar, axis=1) - 0.5 * np.sum(xbar * xbar, axis=1)
@@ -247,7 +255,13 @@ class AFQMCOracle:
                 w[k] = 0.0                                   # reading S10
                 continue
             cos_theta = S[k].real / abs(S[k])                # Eq. (18) without a branch cut
-            w[k] = w[k] * abs(I[k]) * max(0.0, cos_theta)    # Eqs. (13), (15)
+            absI = abs(I[k])
+            if self.ehyb_bound > 0.0 and absI > 0.0:
+                # S8b: D = -log|I| / dt is the real part of the hybrid energy relative to E_shift; clip it
+                D = -np.log(absI) / dt
+                if abs(D) > self.ehyb_bound:
+                    absI = np.exp(-dt * np.copysign(self.ehyb_bound, D))
+            w[k] = w[k] * absI * max(0.0, cos_theta)         # Eqs. (13), (15)
         self.n_steps_done += 1
         if self.ortho_every > 0 and self.n_steps_done % self.ortho_every == 0:
             new, detR = self.reorthonormalise(new)

@@ -47,7 +47,9 @@ def hermitian_parts(L):
 
 
 class ComplexCholOracle:
-    def __init__(self, h1, L, trial, n_alpha, n_beta, walker_kind, taylor_order=6, e_shift=None, check=True):
+    def __init__(self, h1, L, trial, n_alpha, n_beta, walker_kind, taylor_order=6, e_shift=None, check=True,
+                 xbar_bound=0.0, ehyb_bound=0.0):
+        self.xbar_bound, self.ehyb_bound = float(xbar_bound), float(ehyb_bound)      # as in afqmc_oracle.py (S8b)
         h1 = np.asarray(h1, dtype=np.complex128)
         trial = np.asarray(trial)
         trial = trial.astype(np.complex128 if np.iscomplexobj(trial) else np.float64)
@@ -119,6 +121,10 @@ class ComplexCholOracle:
         xbar = 1j * sq * (X - self.m[None, :])
         if xbar_override is not None:
             xbar = np.broadcast_to(np.asarray(xbar_override, dtype=np.complex128), X.shape)
+        elif self.xbar_bound > 0.0:
+            mag = np.abs(xbar)
+            with np.errstate(all="ignore"):
+                xbar = xbar * np.where(mag > self.xbar_bound, self.xbar_bound / mag, 1.0)
         xs = x - xbar
         c_fb = np.sum(x * xbar, axis=1) - 0.5 * np.sum(xbar * xbar, axis=1)
         c_mf = 1j * sq * (xs @ self.m)
@@ -145,7 +151,12 @@ class ComplexCholOracle:
             if not (np.isfinite(S[k]) and np.isfinite(I[k]) and abs(S[k]) > 0.0):
                 w[k] = 0.0
                 continue
-            w[k] = w[k] * abs(I[k]) * max(0.0, S[k].real / abs(S[k]))
+            absI = abs(I[k])
+            if self.ehyb_bound > 0.0 and absI > 0.0:
+                D = -np.log(absI) / dt
+                if abs(D) > self.ehyb_bound:
+                    absI = np.exp(-dt * np.copysign(self.ehyb_bound, D))
+            w[k] = w[k] * absI * max(0.0, S[k].real / abs(S[k]))
         return new, w, info["ovlp_new"].copy()
 
     def local_energy(self, walkers):

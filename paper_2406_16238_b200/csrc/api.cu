@@ -25,6 +25,7 @@ struct afqmc_handle {
   std::vector<void*> allocs;
   // constants
   double *h1 = nullptr, *trial = nullptr, *trialT = nullptr, *Lrot = nullptr, *hrot = nullptr;
+  double* trial_im = nullptr;   // complex trial: Im psi [M][Nt]; trialT is then [2][Nt][M] = (Re psi^T, -Im psi^T)
   double *m = nullptr, *hmod = nullptr, *E1 = nullptr, *Xs = nullptr, *Pa = nullptr, *Pb = nullptr;
   double E_const = 0.0, e_shift = 0.0, e_trial = NAN, hmod_norm1 = 0.0, dt_cached = NAN;
   // per-step workspaces
@@ -264,7 +265,7 @@ void build_E1(afqmc_handle* h, double dt) {
 OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, int want_e1,
                double* ThT = nullptr) {
   OTArgs a;
-  a.W = W; a.trial = h->trial; a.hrot = h->hrot; a.det = det; a.ThT = ThT ? ThT : h->ThT; a.e1 = h->e1;
+  a.W = W; a.trial = h->trial; a.trial_im = h->trial_im; a.hrot = h->hrot; a.det = det; a.ThT = ThT ? ThT : h->ThT; a.e1 = h->e1;
   a.M = h->M; a.Nt = h->Nt; a.nblk = h->nblk;
   for (int b = 0; b < 2; ++b) { a.off[b] = h->off[b]; a.ns[b] = h->ns[b]; }
   a.want_theta = want_theta; a.want_e1 = want_e1;
@@ -394,14 +395,14 @@ int force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw)
     CShiftArgs c;
     c.Xp = h->Xp; c.sXp = (long)2 * h->mwg * nc; c.nsplit = nsplit; c.m = h->m; c.x = x;
     c.X = h->X; c.Cf = h->Cf; c.cfb = h->cfb; c.cmf = h->cmf; c.nf = h->nf;
-    c.spin_factor = h->sf; c.sqrt_dt = sqrt(dt);
+    c.spin_factor = h->sf; c.sqrt_dt = sqrt(dt); c.xbar_bound = h->p.xbar_bound;
     h->launches += run_field_shift_cplx(c, nw, h->st);
   } else {
     StageTimer tm(h, AFQMC_STAGE_FIELD_SHIFT);
     ShiftArgs s;
     s.Xp = h->Xp; s.sXp = (long)2 * h->mwg * nc; s.nsplit = nsplit; s.m = h->m; s.x = x;
     s.X = h->X; s.Cf = h->Cf; s.cfb = h->cfb; s.cmf = h->cmf; s.n_chol = nc;
-    s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt);
+    s.spin_factor = h->sf; s.sqrt_dt = sqrt(dt); s.xbar_bound = h->p.xbar_bound;
     h->launches += run_field_shift(s, nw, h->st);
   }
   return AFQMC_OK;
@@ -472,6 +473,7 @@ int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb
     a.det_old = h->det_old; a.det_new = h->det_new; a.cfb = cfb; a.cmf = cmf;
     a.weights = wt; a.ovlp = h->ovlp; a.nblk = h->nblk; a.rhf = h->rhf;
     a.expo = -dt * (h->E_const - h->e_shift);
+    a.dt = dt; a.ehyb_bound = h->p.ehyb_bound;
     h->launches += run_weight_update(a, nw, h->st);
   }
   // a10: re-orthonormalisation
@@ -704,7 +706,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (!h1 || !L_chol || !trial || !p || !out) return fail(nullptr, AFQMC_ERR_INVALID, "null argument");
   if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
   if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
-      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->complex_chol != 0 && p->complex_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1))
+      p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->complex_chol != 0 && p->complex_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1) ||
+      (p->complex_trial != 0 && p->complex_trial != 1) || p->reserved0 != 0 || !(p->xbar_bound >= 0.0) || !(p->ehyb_bound >= 0.0))
     return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
   if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
   if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
@@ -715,6 +718,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->max_walkers > 65535) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "max_walkers > 65535");
   if (p->kernel_path < 0 || p->kernel_path > 2) return fail(nullptr, AFQMC_ERR_INVALID, "kernel_path must be 0, 1 or 2");
   const bool cplx = p->complex_chol == 1;
+  const bool ctrial = p->complex_trial == 1;
+  if (ctrial && !cplx) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "complex_trial needs complex_chol = 1");
   const int nvec = cplx ? 4 * p->n_chol : p->n_chol;      // real planes the kernels run over
   if ((long)nvec * p->M >= (1L << 31)) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "n_chol * M >= 2^31");
   if (cplx && (p->pack_chol || p->mixed_precision || p->group_size > 1))
@@ -770,9 +775,16 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   };
 
   // ---- host copies of the small inputs, checks, P_tot ------------------------------------
-  std::vector<double> th((size_t)M * Nt), hh((size_t)MM), hi;
-  if (cudaMemcpy(th.data(), trial, th.size() * 8, cudaMemcpyDefault) != cudaSuccess)
+  std::vector<double> th((size_t)M * Nt), hh((size_t)MM), hi, ti;     // ti: Im psi (complex trial)
+  if (ctrial) {
+    std::vector<double> tc((size_t)2 * M * Nt);
+    if (cudaMemcpy(tc.data(), trial, tc.size() * 8, cudaMemcpyDefault) != cudaSuccess)
+      return bail(AFQMC_ERR_CUDA, "copy of the trial failed");
+    ti.resize(th.size());
+    for (size_t i = 0; i < th.size(); ++i) { th[i] = tc[2 * i]; ti[i] = tc[2 * i + 1]; }
+  } else if (cudaMemcpy(th.data(), trial, th.size() * 8, cudaMemcpyDefault) != cudaSuccess) {
     return bail(AFQMC_ERR_CUDA, "copy of the trial failed");
+  }
   if (cplx) {                                  // complex Hermitian h1: planes
     std::vector<double> hc((size_t)2 * MM);
     if (cudaMemcpy(hc.data(), h1, hc.size() * 8, cudaMemcpyDefault) != cudaSuccess)
@@ -790,22 +802,44 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   for (int b = 0; b < h->nblk; ++b)
     for (int i = 0; i < h->ns[b]; ++i)
       for (int j = i; j < h->ns[b]; ++j) {
-        double s = 0.0;
-        for (int q = 0; q < M; ++q) s += th[(size_t)q * Nt + h->off[b] + i] * th[(size_t)q * Nt + h->off[b] + j];
-        if (!(fabs(s - (i == j ? 1.0 : 0.0)) <= 1e-10)) return bail(AFQMC_ERR_TRIAL, "trial columns are not orthonormal to 1e-10");
+        double s = 0.0, si = 0.0;        // (psi^+ psi)_ij = sum_q conj(psi_qi) psi_qj
+        for (int q = 0; q < M; ++q) {
+          const size_t qi = (size_t)q * Nt + h->off[b] + i, qj = (size_t)q * Nt + h->off[b] + j;
+          s += th[qi] * th[qj];
+          if (ctrial) { s += ti[qi] * ti[qj]; si += th[qi] * ti[qj] - ti[qi] * th[qj]; }
+        }
+        if (!(fabs(s - (i == j ? 1.0 : 0.0)) <= 1e-10) || !(fabs(si) <= 1e-10))
+          return bail(AFQMC_ERR_TRIAL, "trial columns are not orthonormal to 1e-10");
       }
-  std::vector<double> P((size_t)MM, 0.0), tT((size_t)Nt * M);
+  // P = psi psi^+ = Pr + i Pi (times the spin factor); Pi = 0 for a real trial.  tT: planes (Re psi^T, -Im psi^T)
+  std::vector<double> P((size_t)MM, 0.0), Pi, tT((size_t)(ctrial ? 2 : 1) * Nt * M);
   for (int q = 0; q < M; ++q)
-    for (int i = 0; i < Nt; ++i) tT[(size_t)i * M + q] = th[(size_t)q * Nt + i];
+    for (int i = 0; i < Nt; ++i) {
+      tT[(size_t)i * M + q] = th[(size_t)q * Nt + i];
+      if (ctrial) tT[(size_t)Nt * M + (size_t)i * M + q] = -ti[(size_t)q * Nt + i];
+    }
   for (int i = 0; i < Nt; ++i)
     for (int a = 0; a < M; ++a) {
       const double f = h->sf * tT[(size_t)i * M + a];
       if (f == 0.0) continue;
       for (int c = 0; c < M; ++c) P[(size_t)a * M + c] += f * tT[(size_t)i * M + c];
     }
+  if (ctrial) {
+    Pi.assign((size_t)MM, 0.0);
+    const double* nI = tT.data() + (size_t)Nt * M;           // -Im psi^T
+    for (int i = 0; i < Nt; ++i)
+      for (int a = 0; a < M; ++a) {
+        const double ra = tT[(size_t)i * M + a], ia = -nI[(size_t)i * M + a];
+        for (int c = 0; c < M; ++c) {
+          const double rc = tT[(size_t)i * M + c], ic = -nI[(size_t)i * M + c];
+          P[(size_t)a * M + c] += h->sf * ia * ic;             // Re (psi_a conj(psi_c)) = ra rc + ia ic
+          Pi[(size_t)a * M + c] += h->sf * (ia * rc - ra * ic); // Im (psi_a conj(psi_c))
+        }
+      }
+  }
 
   // ---- device constants ---------------------------------------------------------------
-  h->h1 = dalloc(h, MM); h->trial = dalloc(h, (size_t)M * Nt); h->trialT = dalloc(h, (size_t)Nt * M);
+  h->h1 = dalloc(h, MM); h->trial = dalloc(h, (size_t)M * Nt); h->trialT = dalloc(h, tT.size());
   h->Lrot = dalloc(h, (size_t)nc * Nt * M); h->hrot = dalloc(h, (size_t)Nt * M); h->m = dalloc(h, nc);
   h->hmod = dalloc(h, MM); h->E1 = dalloc(h, MM); h->Xs = dalloc(h, MM); h->Pa = dalloc(h, MM); h->Pb = dalloc(h, MM);
   double* dP = dalloc(h, MM);
@@ -820,6 +854,19 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
 
   // m_g = tr(L_g P_tot); mL = sum_g m_g L_g
   h->launches += run_mean_field(h->L, dP, h->m, M, nc, h->st);
+  if (ctrial) {
+    // tr(K P) = <Re K, Pr> + <Im K, Pi> (elementwise; Im K and Pi antisymmetric): add the second term to the nf
+    // entries that carry m.  mL is free scratch until run_sum_mL below.
+    h->trial_im = dalloc(h, (size_t)M * Nt);
+    double* mtmp = dalloc(h, h->nf);
+    if (!h->trial_im || !mtmp) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex trial)");
+    cudaMemcpyAsync(h->trial_im, ti.data(), ti.size() * 8, cudaMemcpyHostToDevice, h->st);
+    cudaMemcpyAsync(mL, Pi.data(), MM * 8, cudaMemcpyHostToDevice, h->st);
+    h->launches += run_mean_field(h->L + (size_t)h->nf * MM, mL, mtmp, M, h->nf, h->st);
+    h->launches += run_add(h->m, h->m, mtmp, h->nf, h->st);
+    cudaStreamSynchronize(h->st);           // Pi (host vector) and mtmp are released below
+    dfree_one(h, mtmp);
+  }
   h->launches += run_sum_mL(h->L, h->m, mL, M, nc, h->st);
   // sum_g L_g L_g = L2d^T L2d with L2d = L viewed as [(g,k)][M] (L_g symmetric), split over K
   {
@@ -857,6 +904,23 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
       GemmArgs gg = g;
       gg.B = g.B + (size_t)b0 * MM; gg.C = g.C + (size_t)b0 * Nt * M; gg.batch = std::min(32768, nc - b0);
       h->launches += run_gemm(GEMM_KN, gg, h->st);
+    }
+    if (ctrial) {
+      // psi^+ K = (Re psi^T Kr + Im psi^T Ki) + i (Re psi^T Ki - Im psi^T Kr): the same batched GEMM with the plane
+      // -Im psi^T, then the planes are combined in place (Lrot[0:nf] real part, Lrot[nf:2nf] imaginary part)
+      double* t2 = dalloc(h, (size_t)nc * Nt * M);
+      if (!t2) return bail(AFQMC_ERR_ALLOC, "device allocation failed (complex trial half rotation)");
+      for (int b0 = 0; b0 < nc; b0 += 32768) {
+        GemmArgs gg = g;
+        gg.A = h->trialT + (size_t)Nt * M;
+        gg.B = g.B + (size_t)b0 * MM; gg.C = t2 + (size_t)b0 * Nt * M; gg.batch = std::min(32768, nc - b0);
+        h->launches += run_gemm(GEMM_KN, gg, h->st);
+      }
+      const long half = (long)h->nf * Nt * M;
+      h->launches += run_add_scaled(h->Lrot, h->Lrot, t2 + half, -1.0, half, h->st);
+      h->launches += run_add_scaled(h->Lrot + half, h->Lrot + half, t2, 1.0, half, h->st);
+      cudaStreamSynchronize(h->st);
+      dfree_one(h, t2);
     }
     GemmArgs g2 = gemm_args();
     g2.A = h->trialT; g2.lda = M; g2.B = h->h1; g2.ldb = M; g2.C = h->hrot; g2.ldc = M;
@@ -911,6 +975,16 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     g2.A = h->trialT; g2.lda = M; g2.B = h->Xs; g2.ldb = M; g2.C = h->hrot_i; g2.ldc = M;
     g2.M = Nt; g2.N = M; g2.K = M;
     h->launches += run_gemm(GEMM_KN, g2, h->st);
+    if (ctrial) {
+      // psi^+ h = (Re psi^T hr + Im psi^T hi) + i (Re psi^T hi - Im psi^T hr); Pa, Pb are free scratch here
+      GemmArgs g3 = g2;
+      g3.A = h->trialT + (size_t)Nt * M; g3.C = h->Pa;                  // -Im psi^T hi
+      h->launches += run_gemm(GEMM_KN, g3, h->st);
+      g3.B = h->h1; g3.C = h->Pb;                                       // -Im psi^T hr
+      h->launches += run_gemm(GEMM_KN, g3, h->st);
+      h->launches += run_add_scaled(h->hrot, h->hrot, h->Pa, -1.0, (long)Nt * M, h->st);
+      h->launches += run_add_scaled(h->hrot_i, h->hrot_i, h->Pb, 1.0, (long)Nt * M, h->st);
+    }
     h->launches += run_add(h->Lrot_sum, h->Lrot, h->Lrot + (size_t)nf * Nt * M, (long)nf * Nt * M, h->st);
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
       return bail(AFQMC_ERR_CUDA, "complex setup kernels failed");
@@ -1114,7 +1188,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   // ---- E_shift = trial energy ---------------------------------------------------------------
   {
     std::vector<double> wt((size_t)M * Nt * 2, 0.0);
-    for (size_t i = 0; i < th.size(); ++i) wt[2 * i] = th[i];
+    for (size_t i = 0; i < th.size(); ++i) { wt[2 * i] = th[i]; if (ctrial) wt[2 * i + 1] = ti[i]; }
     cudaMemcpyAsync(h->stW, wt.data(), wt.size() * 8, cudaMemcpyHostToDevice, h->st);
     if (local_energy_device(h, h->stW, h->stE, 1) != AFQMC_OK) return bail(AFQMC_ERR_CUDA, h->err);
     double e[6];

@@ -42,6 +42,11 @@ __global__ void axpy_kernel(double* dst, const double* a, const double* b, long 
   if (i < n) dst[i] = a[i] + b[i];
 }
 
+__global__ void axpy_scaled_kernel(double* dst, const double* a, const double* b, double sb, long n) {
+  const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) dst[i] = a[i] + sb * b[i];
+}
+
 __global__ void add_antisym_kernel(double* A, const double* B, long MM, int M, long total) {
   const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= total) return;
@@ -106,7 +111,11 @@ __global__ void __launch_bounds__(256) field_shift_cplx_kernel(CShiftArgs a) {
     a.X[(size_t)(2 * w) * nf + g] = Xr;
     a.X[(size_t)(2 * w + 1) * nf + g] = Xi;
     const double mg = a.m[g], x = a.x[(size_t)w * nf + g];
-    const double br = -sq * Xi, bi = sq * (Xr - mg);     // xbar = i sqrt(dt) (X - m)
+    double br = -sq * Xi, bi = sq * (Xr - mg);           // xbar = i sqrt(dt) (X - m)
+    if (a.xbar_bound > 0.0) {                            // reading S8b: cap the modulus, keep the phase
+      const double mag = hypot(br, bi);
+      if (mag > a.xbar_bound) { const double sc = a.xbar_bound / mag; br *= sc; bi *= sc; }
+    }
     const double sr = x - br, si = -bi;                  // xs = x - xbar
     v[0] += x * br - 0.5 * (br * br - bi * bi);
     v[1] += x * bi - br * bi;
@@ -181,6 +190,10 @@ int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStr
 }
 int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st) {
   axpy_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(dst, a, b, n);
+  return 1;
+}
+int run_add_scaled(double* dst, const double* a, const double* b, double sb, long n, cudaStream_t st) {
+  axpy_scaled_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(dst, a, b, sb, n);
   return 1;
 }
 int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st) {

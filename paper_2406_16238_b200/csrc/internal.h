@@ -91,7 +91,9 @@ int run_gemm(GemmKind kind, GemmArgs a, cudaStream_t st);
 // small.cu ---------------------------------------------------------------------------------
 struct OTArgs {                 // overlap / Theta / one-body energy, one CTA per (block, walker)
   const double* W;              // walkers as doubles [nw][M][2*Nt]
-  const double* trial;          // [M][Nt]
+  const double* trial;          // [M][Nt] (real part)
+  const double* trial_im = nullptr;   // [M][Nt] imaginary part of a complex trial, else null; trialT then holds
+                                      // the planes (Re psi^T, -Im psi^T), [2][Nt][M]
   const double* hrot;           // [Nt][M] (only with want_e1)
   double* det;                  // [nw][nblk] complex: det(psi_s^T phi_s)
   double* ThT;                  // [nw][2][Nt][M] planar transpose of Theta (want_theta)
@@ -118,6 +120,7 @@ struct ShiftArgs {              // a4: force bias -> shifted fields and scalars,
   double* cmf;                  // [nw] complex
   int n_chol;
   double spin_factor, sqrt_dt;
+  double xbar_bound = 0.0;      // > 0: |xbar_g| capped (afqmc_params::xbar_bound)
 };
 int run_field_shift(const ShiftArgs& a, int nw, cudaStream_t st);
 
@@ -130,6 +133,7 @@ struct WeightArgs {
   double* ovlp;                 // [nw] complex out: overlap of the new walkers
   int nblk, rhf;
   double expo;                  // -dt (E_const - E_shift)
+  double dt = 0.0, ehyb_bound = 0.0;   // > 0: |I| bounded (afqmc_params::ehyb_bound)
 };
 int run_weight_update(const WeightArgs& a, int nw, cudaStream_t st);
 
@@ -247,6 +251,7 @@ struct CShiftArgs {
   double *X, *Cf, *cfb, *cmf;                 // X [nw][2][nf]; Cf [nw][2][nv]
   int nf;
   double spin_factor, sqrt_dt;
+  double xbar_bound = 0.0;
 };
 struct CEnergyArgs {
   const double* Xr; const double* Xi;         // tr(T) of the Re / Im plane runs, [nf][nw] complex
@@ -259,6 +264,7 @@ struct CEnergyArgs {
 };
 int run_hermitian_planes(const double* L_cplx, double* Ks, int M, int n, cudaStream_t st);
 int run_add(double* dst, const double* a, const double* b, long n, cudaStream_t st);
+int run_add_scaled(double* dst, const double* a, const double* b, double sb, long n, cudaStream_t st);   // dst = a + sb b
 // A[r][p][q] += sign(q - p) * B[r][p][q] for `rows` matrices of M x M (B: an antisymmetric sum computed by the
 // symmetric-half V_HS kernel, i.e. correct above the diagonal and mirrored with the wrong sign below)
 int run_add_antisym(double* A, const double* B, int rows, int M, cudaStream_t st);

@@ -63,12 +63,13 @@ __global__ void __launch_bounds__(256) overlap_theta_kernel(OTArgs a) {
   double2* fcol = sphi + (size_t)kRows * ldp;                   // [ns]
   double* spsi = reinterpret_cast<double*>(fcol + ns);          // [kRows][ns]
   double* red = spsi + (size_t)kRows * ns;                      // [32] reduction scratch
+  double* spsi_i = red + 32;                                    // [kRows][ns], complex trial only
   __shared__ int s_piv;
   __shared__ double2 s_det;
 
   const double2* Wc = reinterpret_cast<const double2*>(a.W) + (size_t)w * M * Nt;
 
-  // ---- O = psi^T phi ---------------------------------------------------------------
+  // ---- O = psi^+ phi (psi^T for a real trial) ------------------------------------------
   const int nout = ns * ns;
   double2 acc[16];
 #pragma unroll
@@ -80,6 +81,7 @@ __global__ void __launch_bounds__(256) overlap_theta_kernel(OTArgs a) {
       int pl = c / ns, j = c % ns;
       sphi[pl * ldp + j] = Wc[(size_t)(p0 + pl) * Nt + off + j];
       spsi[pl * ns + j] = a.trial[(size_t)(p0 + pl) * Nt + off + j];
+      if (a.trial_im) spsi_i[pl * ns + j] = a.trial_im[(size_t)(p0 + pl) * Nt + off + j];
     }
     __syncthreads();
 #pragma unroll
@@ -94,6 +96,13 @@ __global__ void __launch_bounds__(256) overlap_theta_kernel(OTArgs a) {
           s.x = fma(ps, z.x, s.x);
           s.y = fma(ps, z.y, s.y);
         }
+        if (a.trial_im)                       // conj(psi) z = (pr - i pi)(zr + i zi)
+          for (int pl = 0; pl < pr; ++pl) {
+            const double pi = spsi_i[pl * ns + i];
+            const double2 z = sphi[pl * ldp + j];
+            s.x = fma(pi, z.y, s.x);
+            s.y = fma(-pi, z.x, s.y);
+          }
         acc[k] = s;
       }
     }
@@ -331,7 +340,11 @@ __global__ void __launch_bounds__(256) field_shift_kernel(ShiftArgs a) {
     a.X[(size_t)(2 * w + 1) * nc + g] = xi;
     const double mg = a.m[g], x = a.x[(size_t)w * nc + g];
     // xbar = i sqrt(dt) (X - m)
-    const double br = -sq * xi, bi = sq * (xr - mg);
+    double br = -sq * xi, bi = sq * (xr - mg);
+    if (a.xbar_bound > 0.0) {                           // reading S8b: cap the modulus, keep the phase
+      const double mag = hypot(br, bi);
+      if (mag > a.xbar_bound) { const double sc = a.xbar_bound / mag; br *= sc; bi *= sc; }
+    }
     const double sr = x - br, si = -bi;                 // xs = x - xbar
     // c_fb = sum x xbar - 1/2 sum xbar^2 (bilinear)
     v[0] += x * br - 0.5 * (br * br - bi * bi);
@@ -378,7 +391,11 @@ __global__ void weight_update_kernel(WeightArgs a, int nw) {
   sincos(cmi, &sn, &cs);
   const double2 S = cmul(r, make_double2(em * cs, em * sn));        // Eq. (17)
   const double absS = hypot(S.x, S.y);
-  const double absI = absS * exp(a.cfb[2 * w]) * exp(a.expo);        // |I|, Eq. (16) + reading S7
+  double absI = absS * exp(a.cfb[2 * w]) * exp(a.expo);              // |I|, Eq. (16) + reading S7
+  if (a.ehyb_bound > 0.0 && absI > 0.0) {                            // reading S8b: clip D = -log|I| / dt
+    const double D = -log(absI) / a.dt;
+    if (fabs(D) > a.ehyb_bound) absI = exp(-a.dt * copysign(a.ehyb_bound, D));
+  }
   const bool ok = isfinite(S.x) && isfinite(S.y) && isfinite(absI) && absS > 0.0 &&
                   (oo.x != 0.0 || oo.y != 0.0) && isfinite(on.x) && isfinite(on.y) &&
                   isfinite(a.cfb[2 * w + 1]);
@@ -526,16 +543,17 @@ __global__ void fill_kernel(double* p, double v, long n) {
 
 static size_t ot_smem(int ns) {
   const int ldp = ns | 1;
-  return (size_t)ns * 2 * ns * 16 + (size_t)kRows * ldp * 16 + (size_t)ns * 16 + (size_t)kRows * ns * 8 + 32 * 8 + 64;
+  return (size_t)ns * 2 * ns * 16 + (size_t)kRows * ldp * 16 + (size_t)ns * 16 + (size_t)2 * kRows * ns * 8 + 32 * 8 + 64;
 }
 
 // the DMMA route; returns launches or -1 if a GEMM cannot be served (caller falls back to the one-kernel route)
 static int run_overlap_theta_gemm(const OTArgs& a, int nw, cudaStream_t st) {
   const int M = a.M, Nt = a.Nt, K2 = 2 * Nt;
   int launches = 0;
-  // O[w] = trial^T (Nt x M, shared) * W[w] (M x 2 Nt)
-  int r = run_gemm_ws_kn(a.trialT, M, 0, 0, false, a.W, K2, (long)M * K2, a.Obuf, nullptr, K2, (long)Nt * K2, Nt, K2, M,
-                         nw, 1.0, 0, st);
+  // O[w] = trial^T (Nt x M, shared) * W[w] (M x 2 Nt); complex trial: conj(trial)^T as the planar pair
+  // (Re psi^T, -Im psi^T) of the planar-complex GEMM
+  int r = run_gemm_ws_kn(a.trialT, M, a.trial_im ? (long)Nt * M : 0, 0, a.trial_im != nullptr, a.W, K2, (long)M * K2, a.Obuf,
+                         nullptr, K2, (long)Nt * K2, Nt, K2, M, nw, 1.0, 0, st);
   if (r < 0) return -1;
   launches += r;
   int nsmax = a.ns[0];

@@ -178,10 +178,11 @@ def make_problem_host(name, seed=0, nw=None, literal=False, **overrides):
     return cfg, h1, L, trial, walkers
 
 
-def make_complex_problem(M, n_alpha, n_beta, n_pairs, walker_kind, seed=0, nw=4, noise=1e-2):
+def make_complex_problem(M, n_alpha, n_beta, n_pairs, walker_kind, seed=0, nw=4, noise=1e-2, complex_trial=False):
     """Complex Cholesky vectors: complex Hermitian h1, vectors {C_k, C_k^+} (a set closed under
     the adjoint factorises a (ps|qr) = (qr|ps) symmetric tensor), k < n_pairs, i.e. n_chol = 2 n_pairs vectors and
-    4 n_pairs auxiliary fields; real trial = lowest eigenvectors of Re h1; walkers = trial + complex noise.  The amplitude follows
+    4 n_pairs auxiliary fields; real trial = lowest eigenvectors of Re h1 (complex_trial: complex128 lowest
+    eigenvectors of the Hermitian h1 itself); walkers = trial + complex noise.  The amplitude follows
     reading R1: E[sum_g |L_g|^2] such that ||A||_2 ~ 0.4 at dt = 0.005.
     Returns (h1, L [2 n_pairs, M, M] complex, trial [M, Nt], walkers [nw, M, Nt])."""
     r = _rng(seed, 11)
@@ -190,7 +191,7 @@ def make_complex_problem(M, n_alpha, n_beta, n_pairs, walker_kind, seed=0, nw=4,
     amp = np.sqrt(10.0 / (M * 4.0 * n_pairs))
     C = (r.standard_normal((n_pairs, M, M)) + 1j * r.standard_normal((n_pairs, M, M))) * amp
     L = np.ascontiguousarray(np.concatenate([C, C.conj().transpose(0, 2, 1)], axis=0))
-    _, v = np.linalg.eigh(h.real)                # real trial: lowest eigenvectors of Re h1 (as c1's recipe)
+    _, v = np.linalg.eigh(h if complex_trial else h.real)   # lowest eigenvectors (as c1's recipe)
     blocks = [v[:, :n_alpha]]
     if walker_kind == 1:
         blocks.append(v[:, :n_beta])

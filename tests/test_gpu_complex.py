@@ -21,15 +21,17 @@ def _torch():
     return torch
 
 
-def _pair(M, na, nb, npairs, kind, nw, seed=0):
+def _pair(M, na, nb, npairs, kind, nw, seed=0, complex_trial=False, kernel_path=0, xbar_bound=0.0, ehyb_bound=0.0):
     torch = _torch()
     from oracle.complex_chol_oracle import ComplexCholOracle
     from paper_2406_16238_b200 import afqmc
-    h, L, trial, walkers = inputs.make_complex_problem(M, na, nb, npairs, kind, seed, nw)
-    o = ComplexCholOracle(h, L, trial, na, nb, kind)
+    h, L, trial, walkers = inputs.make_complex_problem(M, na, nb, npairs, kind, seed, nw, complex_trial=complex_trial)
+    assert np.iscomplexobj(trial) == complex_trial
+    o = ComplexCholOracle(h, L, trial, na, nb, kind, xbar_bound=xbar_bound, ehyb_bound=ehyb_bound)
     Ld = torch.from_numpy(L).cuda()
     g = afqmc.AFQMC(h, Ld, trial, M=M, n_alpha=na, n_beta=nb, n_chol=L.shape[0], max_walkers=nw, walker_kind=kind,
-                    complex_chol=True)
+                    complex_chol=True, complex_trial=complex_trial, kernel_path=kernel_path,
+                    xbar_bound=xbar_bound, ehyb_bound=ehyb_bound)
     Ld.fill_(float("nan"))                 # the caller's tensor is not referenced after afqmc_create
     torch.cuda.synchronize()
     return o, g, walkers
@@ -61,9 +63,10 @@ def _energy(g, W):
 CASES = [(24, 5, 5, 12, 0, 8), (40, 9, 6, 10, 1, 5), (37, 7, 7, 9, 0, 3), (64, 16, 14, 20, 1, 6)]
 
 
+@pytest.mark.parametrize("ctrial", [False, True])
 @pytest.mark.parametrize("M,na,nb,npairs,kind,nw", CASES)
-def test_setup_and_stages(M, na, nb, npairs, kind, nw):
-    o, g, walkers = _pair(M, na, nb, npairs, kind, nw)
+def test_setup_and_stages(M, na, nb, npairs, kind, nw, ctrial):
+    o, g, walkers = _pair(M, na, nb, npairs, kind, nw, complex_trial=ctrial)
     c = g.constants()
     assert abs(c["E_const"] - o.E_const) <= 1e-12 * abs(o.E_const)
     assert abs(c["e_trial"] - o.e_shift) <= 1e-11 * abs(o.e_shift)
@@ -82,9 +85,10 @@ def test_setup_and_stages(M, na, nb, npairs, kind, nw):
     g.close()
 
 
+@pytest.mark.parametrize("ctrial", [False, True])
 @pytest.mark.parametrize("M,na,nb,npairs,kind,nw", CASES)
-def test_local_energy(M, na, nb, npairs, kind, nw):
-    o, g, walkers = _pair(M, na, nb, npairs, kind, nw)
+def test_local_energy(M, na, nb, npairs, kind, nw, ctrial):
+    o, g, walkers = _pair(M, na, nb, npairs, kind, nw, complex_trial=ctrial)
     Eo = o.local_energy(walkers)
     Eg = _energy(g, walkers)
     X = o.force_bias_X(o.theta(walkers))
@@ -96,8 +100,11 @@ def test_local_energy(M, na, nb, npairs, kind, nw):
     g.close()
 
 
-def test_free_running():
-    o, g, walkers = _pair(40, 9, 6, 10, 1, 8)
+@pytest.mark.parametrize("ctrial,kpath", [(False, 0), (True, 0), (True, 1), (True, 2)])
+def test_free_running(ctrial, kpath):
+    """10 free-running steps + energy; with a complex trial (oracle pins PC6-PC9) also on the
+    cp.async kernels (kernel_path 1) and the one-kernel overlap route (kernel_path 2)."""
+    o, g, walkers = _pair(40, 9, 6, 10, 1, 8, complex_trial=ctrial, kernel_path=kpath)
     Wo, wo = walkers, np.ones(8)
     Wg, wg = walkers.copy(), np.ones(8)
     for s in range(10):
@@ -110,6 +117,25 @@ def test_free_running():
     Eo, Eg = o.local_energy(Wo), _energy(g, Wg)
     assert rel_max(Eg[:, 0], Eo[:, 0], scale=np.abs(Eo[:, 1]) + np.abs(Eo[:, 2])) < TOL_RUN
     assert wo.min() > 0.05
+    g.close()
+
+
+def test_bounds_complex():
+    """Optional bounds (S8b, pin P17) in the complex mode with a complex trial; both set so that they
+    trigger on part of the components / walkers."""
+    o0, g0, walkers = _pair(40, 9, 6, 10, 1, 8, complex_trial=True)
+    x = inputs.make_complex_fields(0, 0, 8, o0.n_fields)
+    _, info = o0.propagate(walkers, x, 0.005)
+    g0.close()
+    b = float(np.median(np.abs(info["xbar"])))
+    B = float(np.median(np.abs(np.log(np.abs(info["I"])) / 0.005)))
+    o, g, walkers = _pair(40, 9, 6, 10, 1, 8, complex_trial=True, xbar_bound=b, ehyb_bound=B)
+    Wo, wo, ovo = o.step(walkers, np.ones(8), x, 0.005)
+    Wg, wg, ovg = _step(g, walkers, np.ones(8), x, 0.005)
+    assert rel_fro(Wg, Wo) < TOL_STEP and rel_max(ovg, ovo) < TOL_STEP
+    assert rel_max(wg, wo, scale=np.maximum(np.abs(wo), 1e-3)) < TOL_STEP
+    W1, w1, _ = o0.step(walkers, np.ones(8), x, 0.005)
+    assert rel_fro(Wo, W1) > 1e-6 and np.abs(wo - w1).max() > 1e-6          # the bounds did something
     g.close()
 
 

@@ -420,7 +420,7 @@ def test_dead_walkers_get_zero_weight():
 
 
 # --------------------------------------------------------------------------- literal amplitudes (stress case)
-def test_c1_literal_amplitudes():
+def _literal_stress(xbar_bound=0.0, ehyb_bound=0.0):
     """SURVEY 8(d) R1 / BASELINE.md 5: c1 with BASELINE.json's LITERAL N(0,1) exp(-g/24) amplitudes (no global
     rescale).  ||A||_2 = 2..9, |xbar| up to 50, Taylor-6 is no exponential there and every weight is exactly 0
     by step 7 - but one step is still a deterministic map, so per-step parity (GPU re-seeded from the oracle
@@ -430,11 +430,12 @@ def test_c1_literal_amplitudes():
     |c_fb| + |c_mf| (2.2e3 at step 7 here, where |xbar| reaches 50): 1e-10 relative on the exponent's terms is
     1e-10 max(1, |c_fb| + |c_mf|) relative on the weight."""
     _torch()
-    pr = Pair("c1", literal=True)
+    pr = Pair("c1", literal=True, xbar_bound=xbar_bound, ehyb_bound=ehyb_bound)
     o, cfg, nw = pr.oracle, pr.cfg, pr.nw
     Wo, wo = pr.walkers0.copy(), np.ones(nw)
     zeros_seen = 0
     borderline = []
+    stats = dict(xbar_hits=0, ehyb_hits=0, xbar_max=0.0)
     for s in range(cfg.steps):
         x = pr.fields(s)
         _, info = o.propagate(Wo, x, cfg.dt)
@@ -442,6 +443,14 @@ def test_c1_literal_amplitudes():
         if s == 0:
             assert nA > 1.5                                   # this IS the stress regime
         cos = info["S"].real / np.abs(info["S"])
+        stats["xbar_max"] = max(stats["xbar_max"], float(np.abs(info["xbar"]).max()))
+        if xbar_bound > 0:
+            raw = 1j * np.sqrt(cfg.dt) * (info["X"] - o.m[None, :])
+            stats["xbar_hits"] += int((np.abs(raw) > xbar_bound).sum())
+        if ehyb_bound > 0:
+            with np.errstate(all="ignore"):
+                D = -np.log(np.abs(info["I"])) / cfg.dt
+            stats["ehyb_hits"] += int((np.abs(D) > ehyb_bound).sum())
         w_in = wo.copy() if s > 0 else np.ones(nw)
         w_in = np.where(w_in > 0, w_in, 1.0)                  # keep every walker's weight rule exercised
         Wg, wg, ovg = gpu_step(pr, Wo, w_in, x, cfg.dt)
@@ -472,10 +481,29 @@ def test_c1_literal_amplitudes():
                 assert abs(wg[k] - wn[k]) < TOL_STEP * amp * wn[k], (s, k, wg[k], wn[k], amp)
         _, wo, _ = Wn, wo * (wn / w_in), ovn
         Wo = Wn
+    pr.close()
+    assert not borderline, borderline
+    return zeros_seen, wo, stats
+
+
+
+
+def test_c1_literal_amplitudes():
+    """The literal c1 inputs without bounds: see _literal_stress."""
+    zeros_seen, wo, _ = _literal_stress()
     assert zeros_seen >= 10, zeros_seen                       # the phaseless cut really fired
     assert np.all(wo == 0.0)                                  # R1: all 16 walkers are dead by the last step
-    assert not borderline, borderline
-    pr.close()
+
+
+def test_bounds_trigger_on_literal_amplitudes():
+    """SURVEY 8f NEXT-1 / DESIGN.md S8b (oracle pin P17): the optional force-bias and hybrid-energy bounds, on inputs
+    where both DO trigger (literal c1 amplitudes: raw |xbar| up to 50, hybrid energies far outside +-sqrt(2/dt)).
+    Same per-step parity as above; with the bounds the shifts stay <= 1 and the weights stay finite."""
+    dt = 0.005
+    zeros_seen, wo, st = _literal_stress(xbar_bound=1.0, ehyb_bound=float(np.sqrt(2.0 / dt)))
+    assert st["xbar_hits"] > 50 and st["ehyb_hits"] > 5, st
+    assert st["xbar_max"] <= 1.0 + 1e-12
+    assert np.all(np.isfinite(wo))
 
 
 def test_error_codes():

@@ -442,21 +442,10 @@ def test_P15_estimator_and_block_loop():
 
 
 # --------------------------------------------------------------------------- P16 weight rule, L != 0
-@pytest.mark.parametrize("kind,na,nb,seed", [(1, 2, 1, 21), (0, 2, 2, 22)])
-def test_P16_weight_rule_many_body(kind, na, nb, seed):
-    """Eqs. (13), (15)-(18) (PAPER.md:102-128) with L != 0, from explicit many-body matrices only.
-
-    In the 256-dimensional Fock space the one-sample propagator is built WITHOUT any of the oracle's one-body
-    formulas: with m_g = <Psi_T|L_g|Psi_T>, E_c = -1/2 sum m_g^2 and V0 = H - E_c - 1/2 sum_g (L_g - m_g)^2
-    (the operator the Trotter split of Eq. 7 calls v0 after the mean-field shift, PAPER.md:108),
-        B(x - xbar) = e^{-dt E_c} e^{-dt/2 V0} e^{-i sqrt(dt) sum_g (x - xbar)_g (L_g - m_g)} e^{-dt/2 V0},
-    xbar_g = i sqrt(dt) (<L_g>_mixed - m_g).  Then S = <Psi_T|B|phi>/<Psi_T|phi> e^{+dt E_c} (Eq. 17; real
-    positive factors do not enter theta), I = <Psi_T|B|phi>/<Psi_T|phi> e^{x.xbar - xbar.xbar/2} e^{dt E_shift}
-    (Eq. 16 with the energy shift of reading S7) and w' = w |I| max(0, Re S/|S|) (Eqs. 13, 15, 18).  The oracle's
-    `step` (Taylor order 24, i.e. the exact exponential to 1e-15) must give the same weights and overlaps."""
-    M, ng, dt = 4, 3, 0.04
-    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, seed, lscale=0.45, noise=0.35, nw=6)
-    o = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24)
+def _many_body_step(o, h, L, trial, walkers, x, w0, dt, xbar_bound=0.0, ehyb_bound=0.0):
+    """Weights and new overlaps of one step from explicit many-body matrices only (see P16's docstring); the optional
+    bounds are applied as DESIGN.md reading S8b states them."""
+    M, ng = h.shape[0], L.shape[0]
     F = Fock(M)
     dim = 2 ** F.n
     Id = np.eye(dim)
@@ -474,28 +463,105 @@ def test_P16_weight_rule_many_body(kind, na, nb, seed):
         d = Lop[g] - m[g] * Id
         V0 = V0 - 0.5 * d @ d
     half = sla.expm(-0.5 * dt * V0)
-    x = np.random.default_rng(seed).standard_normal((walkers.shape[0], ng))
-    w0 = np.linspace(0.5, 2.0, walkers.shape[0])
-    expect_w, expect_ov, phases = [], [], []
+    expect_w, expect_ov, phases, xbars, absI = [], [], [], [], []
     for k in range(walkers.shape[0]):
         wa, wb = spin_blocks(o, walkers[k])
         ket = F.det_state(wa, wb)
         ov = bra @ ket
         X = np.array([(bra @ Lop[g] @ ket) / ov for g in range(ng)])
         xbar = 1j * np.sqrt(dt) * (X - m)
+        if xbar_bound > 0:
+            xbar = np.array([z * min(1.0, xbar_bound / abs(z)) if abs(z) > 0 else z for z in xbar])
         xs = x[k] - xbar
         two = sla.expm(-1j * np.sqrt(dt) * sum(xs[g] * (Lop[g] - m[g] * Id) for g in range(ng)))
         Bket = np.exp(-dt * E_c) * (half @ (two @ (half @ ket)))
         ratio = (bra @ Bket) / ov
         S = ratio * np.exp(dt * E_c)
         I = ratio * np.exp(np.sum(x[k] * xbar) - 0.5 * np.sum(xbar * xbar)) * np.exp(dt * e_shift)
-        expect_w.append(w0[k] * abs(I) * max(0.0, S.real / abs(S)))
+        mod = abs(I)
+        if ehyb_bound > 0:
+            D = -np.log(mod) / dt
+            mod = np.exp(-dt * min(max(D, -ehyb_bound), ehyb_bound))
+        expect_w.append(w0[k] * mod * max(0.0, S.real / abs(S)))
         expect_ov.append(bra @ Bket * np.exp(dt * E_c) / np.exp(1j * np.sqrt(dt) * (xs @ m)))
         phases.append(np.angle(S))
+        xbars.append(xbar)
+        absI.append(abs(I))
+    return dict(w=np.array(expect_w), ov=np.array(expect_ov), phases=np.array(phases), xbar=np.array(xbars),
+                absI=np.array(absI), e_shift=e_shift, E_c=E_c)
+
+
+@pytest.mark.parametrize("kind,na,nb,seed", [(1, 2, 1, 21), (0, 2, 2, 22)])
+def test_P16_weight_rule_many_body(kind, na, nb, seed):
+    """Eqs. (13), (15)-(18) (PAPER.md:102-128) with L != 0, from explicit many-body matrices only.
+
+    In the 256-dimensional Fock space the one-sample propagator is built WITHOUT any of the oracle's one-body
+    formulas: with m_g = <Psi_T|L_g|Psi_T>, E_c = -1/2 sum m_g^2 and V0 = H - E_c - 1/2 sum_g (L_g - m_g)^2
+    (the operator the Trotter split of Eq. 7 calls v0 after the mean-field shift, PAPER.md:108),
+        B(x - xbar) = e^{-dt E_c} e^{-dt/2 V0} e^{-i sqrt(dt) sum_g (x - xbar)_g (L_g - m_g)} e^{-dt/2 V0},
+    xbar_g = i sqrt(dt) (<L_g>_mixed - m_g).  Then S = <Psi_T|B|phi>/<Psi_T|phi> e^{+dt E_c} (Eq. 17; real
+    positive factors do not enter theta), I = <Psi_T|B|phi>/<Psi_T|phi> e^{x.xbar - xbar.xbar/2} e^{dt E_shift}
+    (Eq. 16 with the energy shift of reading S7) and w' = w |I| max(0, Re S/|S|) (Eqs. 13, 15, 18).  The oracle's
+    `step` (Taylor order 24, i.e. the exact exponential to 1e-15) must give the same weights and overlaps."""
+    M, ng, dt = 4, 3, 0.04
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, seed, lscale=0.45, noise=0.35, nw=6)
+    o = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24)
+    x = np.random.default_rng(seed).standard_normal((walkers.shape[0], ng))
+    w0 = np.linspace(0.5, 2.0, walkers.shape[0])
+    mb = _many_body_step(o, h, L, trial, walkers, x, w0, dt)
+    expect_w, expect_ov, phases, e_shift, E_c = mb["w"], mb["ov"], mb["phases"], mb["e_shift"], mb["E_c"]
     new, w, ov_new = o.step(walkers, w0, x, dt)
     assert abs(o.e_shift - e_shift) < 1e-12 and abs(o.E_const - E_c) < 1e-12
-    assert np.max(np.abs(w - np.array(expect_w))) < 1e-10 * max(expect_w)
+    assert np.max(np.abs(w - expect_w)) < 1e-10 * max(expect_w)
     # the propagated determinant itself: <Psi_T|phi'> = <Psi_T|B|phi> without the scalars B carries
-    assert np.max(np.abs(ov_new - np.array(expect_ov)) / np.abs(expect_ov)) < 1e-10
+    assert np.max(np.abs(ov_new - expect_ov) / np.abs(expect_ov)) < 1e-10
     assert np.max(np.abs(phases)) > 1e-2          # theta is not trivially zero: the cos factor is exercised
-    assert np.all(np.array(expect_w) > 0)
+    assert np.all(expect_w > 0)
+
+
+# --------------------------------------------------------------------------- P17 (optional bounds, reading S8b)
+def test_P17_bounds():
+    """SURVEY 8f NEXT-1 / DESIGN.md S8b: (a) bounds that never trigger leave every bit unchanged; (b) a force-bias
+    bound that does trigger caps |xbar_g| at the bound, keeps the phases and the untouched components, and the step
+    still equals the many-body step with THAT xbar (Eqs. 12, 16 hold for any xbar: the estimator stays exact);
+    (c) a hybrid-energy bound that triggers replaces |I| by exp(-/+ dt b) and leaves max(0, cos theta) alone."""
+    M, ng, dt, kind, na, nb = 4, 3, 0.04, 1, 2, 1
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, 31, lscale=0.45, noise=0.35, nw=6)
+    x = np.random.default_rng(31).standard_normal((walkers.shape[0], ng))
+    w0 = np.linspace(0.5, 2.0, walkers.shape[0])
+    plain = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24)
+    W0, wt0, ov0 = plain.step(walkers, w0, x, dt)
+    _, info0 = plain.propagate(walkers, x, dt)
+    # (a)
+    loose = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24, xbar_bound=1e6, ehyb_bound=1e6)
+    W1, wt1, ov1 = loose.step(walkers, w0, x, dt)
+    assert np.array_equal(W0, W1) and np.array_equal(wt0, wt1) and np.array_equal(ov0, ov1)
+    # (b)
+    mags = np.abs(info0["xbar"])
+    b = float(np.median(mags))                      # about half of the components get capped
+    capped = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24, xbar_bound=b)
+    _, info = capped.propagate(walkers, x, dt)
+    hit = mags > b
+    assert hit.any() and (~hit).any()
+    assert np.all(np.abs(info["xbar"]) <= b * (1 + 1e-15))
+    assert np.array_equal(info["xbar"][~hit], info0["xbar"][~hit])
+    assert np.abs(info["xbar"][hit] / np.abs(info["xbar"][hit]) - info0["xbar"][hit] / mags[hit]).max() < 1e-15
+    mb = _many_body_step(capped, h, L, trial, walkers, x, w0, dt, xbar_bound=b)
+    W2, wt2, ov2 = capped.step(walkers, w0, x, dt)
+    assert np.abs(mb["xbar"] - info["xbar"]).max() < 1e-12
+    assert np.max(np.abs(wt2 - mb["w"])) < 1e-10 * mb["w"].max()
+    assert np.max(np.abs(ov2 - mb["ov"]) / np.abs(mb["ov"])) < 1e-10
+    assert np.abs(wt2 - wt0).max() > 1e-6           # the bound did change the sample
+    # (c)
+    D = -np.log(np.abs(info0["I"])) / dt
+    B = float(np.median(np.abs(D)))
+    eb = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24, ehyb_bound=B)
+    W3, wt3, ov3 = eb.step(walkers, w0, x, dt)
+    assert np.array_equal(W3, W0) and np.array_equal(ov3, ov0)      # the bound touches the weights only
+    cos = np.maximum(0.0, info0["S"].real / np.abs(info0["S"]))
+    trig = np.abs(D) > B
+    assert trig.any() and (~trig).any()
+    expect = np.where(trig, w0 * np.exp(-dt * np.sign(D) * B) * cos, wt0)
+    assert np.max(np.abs(wt3 - expect)) < 1e-14 * expect.max()
+    mb3 = _many_body_step(eb, h, L, trial, walkers, x, w0, dt, ehyb_bound=B)
+    assert np.max(np.abs(wt3 - mb3["w"])) < 1e-10 * mb3["w"].max()
