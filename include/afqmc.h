@@ -196,6 +196,17 @@ int64_t afqmc_set_block_graph(afqmc_handle* h, int32_t on);
  *   ovlp_out EITHER complex128 [nw of that step]. */
 int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out);
 
+/* Row a10 on its own ("stabilization"; reading S9): every walker block phi_sigma = Q R with R_ii
+ * real > 0 is replaced by Q, in place - what afqmc_step does on the ortho_every schedule.  Repeated Cholesky-QR
+ * passes with a shifted pass when the Gram matrix is numerically singular (cond(phi) up to ~1e15).
+ *   walkers  EITHER complex128 [nw][M][Nt], in/out.
+ *   detR_out EITHER double [nw][n_blocks] = prod_i R_ii per block (n_blocks = 1 RHF, 2 UHF), or NULL.
+ * If nw equals the nw of the last afqmc_step the stored overlaps (afqmc_get_overlaps) are divided by
+ * prod_sigma det R_sigma (squared for RHF), as on the schedule. */
+int32_t afqmc_reorthonormalise(afqmc_handle* h, void* walkers, double* detR_out, int32_t nw);
+/* Number of shifted Cholesky-QR passes (numerically singular Gram matrices) since afqmc_create; synchronises. */
+int64_t afqmc_qr_shifted_passes(afqmc_handle* h);
+
 /* Scalars fixed at create: out[0] = E_const, out[1] = E_shift in use, out[2] = trial energy
  * (NaN if never computed).  HOST pointer. */
 int32_t afqmc_get_constants(afqmc_handle* h, double* out3);

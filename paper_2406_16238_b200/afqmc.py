@@ -22,7 +22,8 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_set_block_graph", "afqmc_shard_setup_partial", "afqmc_shard_setup_finish",
            "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
            "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
-           "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce", "afqmc_exchange_plan", "afqmc_exchange_plan_pin"]
+           "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce", "afqmc_exchange_plan", "afqmc_exchange_plan_pin",
+           "afqmc_reorthonormalise", "afqmc_qr_shifted_passes"]
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
           "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
@@ -91,6 +92,10 @@ def _load():
     lib.afqmc_shard_setup_reduce.restype = i32
     lib.afqmc_measure_fp64_peak.argtypes = [dbl, vp]
     lib.afqmc_measure_fp64_peak.restype = i32
+    lib.afqmc_reorthonormalise.argtypes = [vp, vp, vp, i32]
+    lib.afqmc_reorthonormalise.restype = i32
+    lib.afqmc_qr_shifted_passes.argtypes = [vp]
+    lib.afqmc_qr_shifted_passes.restype = i64
     lib.afqmc_exchange_plan.argtypes = [i32, i32, i32, C.c_char_p, i32]
     lib.afqmc_exchange_plan.restype = i32
     lib.afqmc_exchange_plan_pin.argtypes = [i32] * 9
@@ -189,6 +194,16 @@ class AFQMC:
     def local_energy(self, walkers, E_out, nw=None):
         nw = int(walkers.shape[0]) if nw is None else nw
         self._check(lib.afqmc_local_energy(self._h, _ptr(walkers), _ptr(E_out), nw))
+
+    def reorthonormalise(self, walkers, detR_out=None, nw=None):
+        nw = int(walkers.shape[0]) if nw is None else nw
+        self._check(lib.afqmc_reorthonormalise(self._h, _ptr(walkers), _ptr(detR_out), nw))
+
+    def qr_shifted_passes(self):
+        v = int(lib.afqmc_qr_shifted_passes(self._h))
+        if v < 0:
+            self._check(v)
+        return v
 
     def population_control(self, walkers, weights, xi, map_out=None, nw=None):
         """xi: array/tensor holding one double in [0, 1) (host or device)."""

@@ -39,6 +39,7 @@ struct afqmc_handle {
   // population control / estimators
   double *cum = nullptr, *xi_dev = nullptr, *est_dev = nullptr, *ovlp_tmp = nullptr;
   int* pmap = nullptr;
+  int* qr_shifted = nullptr;     // device counter: shifted Cholesky-QR passes (ill-conditioned walkers) so far
   // CUDA graphs of whole blocks (afqmc_run_block on device buffers), keyed by the call's arguments
   struct BlockGraph {
     const void *W, *wt, *x, *xi, *E, *est;
@@ -459,6 +460,18 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   return propagate_device(h, W, wt, h->cfb, h->cmf, dt, nw);
 }
 
+// a10: thin QR with R_ii > 0 of every walker block, in place; h->detR [nw][nblk] = prod diag R per block
+void reortho_device(afqmc_handle* h, double* W, int nw, bool fix_overlaps) {
+  StageTimer tm(h, AFQMC_STAGE_REORTHO);
+  QRArgs q;
+  q.W = W; q.detR = h->detR; q.M = h->M; q.Nt = h->Nt; q.nblk = h->nblk;
+  for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
+  q.shifted = h->qr_shifted;
+  h->launches += run_fill(h->detR, 1.0, (long)nw * h->nblk, h->st);
+  h->launches += run_cholqr_pass(q, nw, h->st);       // all passes in one launch (small.cu)
+  if (fix_overlaps) h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
+}
+
 // a9-a10: overlap of the propagated walkers, phaseless weight update, re-orthonormalisation on schedule
 int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw) {
   const int M = h->M, Nt = h->Nt;
@@ -479,16 +492,7 @@ int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb
   // a10: re-orthonormalisation
   h->step_count += 1;
   h->last_nw = nw;
-  if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) {
-    StageTimer tm(h, AFQMC_STAGE_REORTHO);
-    QRArgs q;
-    q.W = W; q.detR = h->detR; q.M = M; q.Nt = Nt; q.nblk = h->nblk;
-    for (int b = 0; b < 2; ++b) { q.off[b] = h->off[b]; q.ns[b] = h->ns[b]; }
-    h->launches += run_fill(h->detR, 1.0, (long)nw * h->nblk, h->st);
-    h->launches += run_cholqr_pass(q, nw, h->st);
-    h->launches += run_cholqr_pass(q, nw, h->st);
-    h->launches += run_ovlp_div_detR(h->ovlp, h->detR, h->nblk, h->rhf, nw, h->st);
-  }
+  if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) reortho_device(h, W, nw, true);
   return AFQMC_OK;
 }
 
@@ -1100,7 +1104,9 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->stW = dalloc(h, wsz); h->stWt = dalloc(h, mw); h->stX = dalloc(h, (size_t)mw * nc); h->stE = dalloc(h, (size_t)mw * 6);
   h->cum = dalloc(h, mw); h->xi_dev = dalloc(h, 4); h->est_dev = dalloc(h, 4); h->ovlp_tmp = dalloc(h, 2 * mw);
   h->pmap = (int*)dalloc(h, (mw + 1) / 2 + 1);
-  if (!h->cum || !h->xi_dev || !h->est_dev || !h->ovlp_tmp || !h->pmap)
+  h->qr_shifted = (int*)dalloc(h, 1);
+  if (h->qr_shifted) cudaMemsetAsync(h->qr_shifted, 0, 8, h->st);
+  if (!h->cum || !h->xi_dev || !h->est_dev || !h->ovlp_tmp || !h->pmap || !h->qr_shifted)
     return bail(AFQMC_ERR_ALLOC, "device allocation failed (population control)");
   if (!h->det_old || !h->det_new || !h->ThT || !h->Xp || !h->X || !h->Cf || !h->cfb || !h->cmf || !h->A ||
       !h->T0 || !h->T1 || !h->Acc || !h->ovlp || !h->detR || !h->expart[0] || (h->nblk > 1 && !h->expart[1]) ||
@@ -1386,6 +1392,35 @@ int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out) {
   cudaMemcpyAsync(ovlp_out, h->ovlp, (size_t)h->last_nw * 16, cudaMemcpyDefault, h->st);
   if (host && cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_get_overlaps");
   return check_cuda(h, "afqmc_get_overlaps");
+}
+
+int32_t afqmc_reorthonormalise(afqmc_handle* h, void* walkers, double* detR_out, int32_t nw) {
+  if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
+  if (!walkers) return fail(h, AFQMC_ERR_INVALID, "null argument");
+  if (nw <= 0 || nw > h->maxw) return fail(h, AFQMC_ERR_DIMS, "nw out of range");
+  const size_t wlen = (size_t)nw * h->M * 2 * h->Nt;
+  const bool hostW = !is_device_ptr(walkers);
+  double* W = (double*)walkers;
+  if (hostW) { to_device(h, h->stW, walkers, wlen); W = h->stW; }
+  reortho_device(h, W, nw, h->last_nw == nw);
+  bool sync = false;
+  if (hostW) { cudaMemcpyAsync(walkers, W, wlen * 8, cudaMemcpyDeviceToHost, h->st); sync = true; }
+  if (detR_out) {
+    cudaMemcpyAsync(detR_out, h->detR, (size_t)nw * h->nblk * 8, cudaMemcpyDefault, h->st);
+    sync = sync || !is_device_ptr(detR_out);
+  }
+  if (sync && cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_reorthonormalise");
+  return check_cuda(h, "afqmc_reorthonormalise");
+}
+
+int64_t afqmc_qr_shifted_passes(afqmc_handle* h) {
+  if (!h) return AFQMC_ERR_INVALID;
+  DevGuard dg_(h->dev);
+  int v = 0;
+  cudaMemcpyAsync(&v, h->qr_shifted, sizeof(int), cudaMemcpyDeviceToHost, h->st);
+  if (cudaStreamSynchronize(h->st) != cudaSuccess) return check_cuda(h, "afqmc_qr_shifted_passes");
+  return v;
 }
 
 int32_t afqmc_get_constants(afqmc_handle* h, double* out3) {

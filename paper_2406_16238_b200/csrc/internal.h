@@ -137,11 +137,12 @@ struct WeightArgs {
 };
 int run_weight_update(const WeightArgs& a, int nw, cudaStream_t st);
 
-struct QRArgs {                 // one Cholesky-QR pass per (block, walker), in place
+struct QRArgs {                 // thin QR per (block, walker), in place: Cholesky-QR passes until orthonormal
   double* W;                    // [nw][M][2*Nt]
   double* detR;                 // [nw][nblk] real: multiplied by prod diag(R) of this pass
   int M, Nt, nblk;
   int off[2], ns[2];
+  int* shifted = nullptr;       // device counter of shifted (breakdown) passes, may be null
 };
 int run_cholqr_pass(const QRArgs& a, int nw, cudaStream_t st);
 int run_ovlp_div_detR(double* ovlp, const double* detR, int nblk, int rhf, int nw, cudaStream_t st);

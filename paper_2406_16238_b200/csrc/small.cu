@@ -410,8 +410,15 @@ __global__ void weight_update_kernel(WeightArgs a, int nw) {
 }
 
 // ------------------------------------------------------------------------------ a10
-// One Cholesky-QR pass: G = phi^H phi = R^H R, phi <- phi R^-1.  Two passes give Q to machine
-// precision with R = R2 R1 upper triangular, R_ii > 0 (the unique thin QR).
+// Thin QR with R_ii > 0 by repeated Cholesky-QR passes inside ONE kernel (a CTA owns its walker-block):
+//     G = phi^H phi = R^H R,  phi <- phi R^-1,  detR *= prod R_ii
+// until the Gram matrix found at the start of a pass is within 0.05 of the identity: that pass then leaves
+// ||Q^H Q - 1|| = O(eps).  Well-conditioned walkers take the two passes of Cholesky-QR2.  When the Cholesky
+// factorisation breaks down (a pivot <= 1e-11 of its diagonal entry, or not finite: cond(phi)^2 reached 1/eps) the
+// pass is redone on G + s 1 with s = 11 (M n + n (n + 1)) eps tr(G) - shifted Cholesky-QR (Fukaya et al., SIAM J. Sci.
+// Comput. 42 (2020)): it brings cond(phi) ~ 1e12 down to ~1e7, which the next two passes finish.  R is the product
+// of the passes' triangles, so its diagonal stays real positive: the unique thin QR, as the oracle's (S9).
+// A walker that is not finite stays not finite (its weight is already 0, S10).  shifted[0] counts shifted passes.
 __global__ void __launch_bounds__(256) cholqr_kernel(QRArgs a) {
   extern __shared__ __align__(16) unsigned char smraw[];
   const int blk = blockIdx.x, w = blockIdx.y;
@@ -419,110 +426,150 @@ __global__ void __launch_bounds__(256) cholqr_kernel(QRArgs a) {
   const int tid = threadIdx.x;
   const int ldp = ns | 1;
   double2* G = reinterpret_cast<double2*>(smraw);     // [ns][ns]
-  double2* Ri = G + (size_t)ns * ns;                  // [ns][ns] inverse of R
+  double2* Ri = G + (size_t)ns * ns;                  // [ns][ns] inverse of R (backup of G during the Cholesky)
   double2* sphi = Ri + (size_t)ns * ns;               // [kRows][ldp]
   double2* Wc = reinterpret_cast<double2*>(a.W) + (size_t)w * M * Nt;
-
+  __shared__ double s_red[8];
+  __shared__ double s_diag0[kMaxOcc];
+  __shared__ int s_bad;
   const int nout = ns * ns;
-  double2 acc[16];
+  double detR = 1.0;
+
+  for (int pass = 0; pass < 8; ++pass) {
+    double2 acc[16];
 #pragma unroll
-  for (int k = 0; k < 16; ++k) acc[k] = make_double2(0.0, 0.0);
-  for (int p0 = 0; p0 < M; p0 += kRows) {
-    const int pr = min(kRows, M - p0);
-    __syncthreads();
-    for (int c = tid; c < pr * ns; c += blockDim.x) {
-      int pl = c / ns, j = c % ns;
-      sphi[pl * ldp + j] = Wc[(size_t)(p0 + pl) * Nt + off + j];
+    for (int k = 0; k < 16; ++k) acc[k] = make_double2(0.0, 0.0);
+    for (int p0 = 0; p0 < M; p0 += kRows) {
+      const int pr = min(kRows, M - p0);
+      __syncthreads();
+      for (int c = tid; c < pr * ns; c += blockDim.x) {
+        int pl = c / ns, j = c % ns;
+        sphi[pl * ldp + j] = Wc[(size_t)(p0 + pl) * Nt + off + j];
+      }
+      __syncthreads();
+#pragma unroll
+      for (int k = 0; k < 16; ++k) {
+        const int idx = tid + k * 256;
+        if (idx < nout) {
+          const int i = idx / ns, j = idx % ns;
+          double2 s = acc[k];
+          for (int pl = 0; pl < pr; ++pl) {
+            const double2 u = sphi[pl * ldp + i], z = sphi[pl * ldp + j];
+            s.x += u.x * z.x + u.y * z.y;               // conj(u) z
+            s.y += u.x * z.y - u.y * z.x;
+          }
+          acc[k] = s;
+        }
+      }
     }
     __syncthreads();
+    // G, its backup, and max |G - 1| (NaN counts as far from the identity)
+    double dev = 0.0;
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
       const int idx = tid + k * 256;
       if (idx < nout) {
+        G[idx] = acc[k];
+        Ri[idx] = acc[k];
         const int i = idx / ns, j = idx % ns;
-        double2 s = acc[k];
-        for (int pl = 0; pl < pr; ++pl) {
-          const double2 u = sphi[pl * ldp + i], z = sphi[pl * ldp + j];
-          s.x += u.x * z.x + u.y * z.y;               // conj(u) z
-          s.y += u.x * z.y - u.y * z.x;
-        }
-        acc[k] = s;
+        const double e = fmax(fabs(acc[k].x - (i == j ? 1.0 : 0.0)), fabs(acc[k].y));
+        dev = (e > dev || !(e == e)) ? (e == e ? e : 1e300) : dev;
+        if (i == j) s_diag0[i] = acc[k].x;
       }
     }
-  }
-  __syncthreads();
 #pragma unroll
-  for (int k = 0; k < 16; ++k) {
-    const int idx = tid + k * 256;
-    if (idx < nout) {
-      G[idx] = acc[k];
-      Ri[idx] = make_double2(0.0, 0.0);
-    }
-  }
-  __syncthreads();
-  // Cholesky G = R^H R, R upper, in place
-  for (int k = 0; k < ns; ++k) {
-    const double d = sqrt(G[k * ns + k].x);
+    for (int o = 16; o > 0; o >>= 1) dev = fmax(dev, __shfl_down_sync(0xffffffffu, dev, o));
+    if ((tid & 31) == 0) s_red[tid >> 5] = dev;
+    if (tid == 0) s_bad = 0;
     __syncthreads();
-    for (int j = k + tid; j < ns; j += blockDim.x) {
-      double2 v = G[k * ns + j];
-      G[k * ns + j] = (j == k) ? make_double2(d, 0.0) : make_double2(v.x / d, v.y / d);
-    }
-    __syncthreads();
-    const int rem = ns - k - 1;
-    for (int idx = tid; idx < rem * rem; idx += blockDim.x) {
-      const int i = k + 1 + idx / rem, j = k + 1 + idx % rem;
-      if (j >= i) {
-        const double2 u = G[k * ns + i], z = G[k * ns + j];
-        double2 v = G[i * ns + j];
-        v.x -= u.x * z.x + u.y * z.y;
-        v.y -= u.x * z.y - u.y * z.x;
-        G[i * ns + j] = v;
-      }
-    }
-    __syncthreads();
-  }
-  // R^-1 by back substitution, one column per thread
-  if (tid < ns) {
-    const int c = tid;
-    for (int i = c; i >= 0; --i) {
-      double2 s = make_double2(i == c ? 1.0 : 0.0, 0.0);
-      for (int k = i + 1; k <= c; ++k) {
-        const double2 r = G[i * ns + k], x = Ri[k * ns + c];
-        s.x -= r.x * x.x - r.y * x.y;
-        s.y -= r.x * x.y + r.y * x.x;
-      }
-      const double rii = G[i * ns + i].x;
-      Ri[i * ns + c] = make_double2(s.x / rii, s.y / rii);
-    }
-  }
-  if (tid == 0) {
-    double dr = 1.0;
-    for (int k = 0; k < ns; ++k) dr *= G[k * ns + k].x;
-    a.detR[(size_t)w * a.nblk + blk] *= dr;
-  }
-  __syncthreads();
-  // phi <- phi R^-1, rows are independent
-  const int lane = tid & 31, rw = tid >> 5;
-  for (int q0 = 0; q0 < M; q0 += kRows) {
-    const int qr = min(kRows, M - q0);
-    __syncthreads();
-    for (int c = tid; c < qr * ns; c += blockDim.x) {
-      int pl = c / ns, j = c % ns;
-      sphi[pl * ldp + j] = Wc[(size_t)(q0 + pl) * Nt + off + j];
-    }
-    __syncthreads();
-    for (int pl = rw; pl < qr; pl += 8)
-      for (int i = lane; i < ns; i += 32) {
-        double2 s = make_double2(0.0, 0.0);
-        for (int j = 0; j <= i; ++j) {
-          const double2 z = sphi[pl * ldp + j], o = Ri[j * ns + i];
-          s.x += z.x * o.x - z.y * o.y;
-          s.y += z.x * o.y + z.y * o.x;
+    dev = 0.0;
+    for (int k = 0; k < 8; ++k) dev = fmax(dev, s_red[k]);
+    const bool last = dev <= 0.05;
+
+    // Cholesky G = R^H R, R upper, in place; one retry on the shifted matrix
+    for (int attempt = 0; attempt < 2; ++attempt) {
+      bool bad = false;
+      for (int k = 0; k < ns; ++k) {
+        const double d2 = G[k * ns + k].x;
+        if (attempt == 0 && !(d2 > 1e-11 * s_diag0[k])) { bad = true; break; }     // uniform: every thread reads the same
+        const double d = sqrt(d2);
+        __syncthreads();
+        for (int j = k + tid; j < ns; j += blockDim.x) {
+          double2 v = G[k * ns + j];
+          G[k * ns + j] = (j == k) ? make_double2(d, 0.0) : make_double2(v.x / d, v.y / d);
         }
-        Wc[(size_t)(q0 + pl) * Nt + off + i] = s;
+        __syncthreads();
+        const int rem = ns - k - 1;
+        for (int idx = tid; idx < rem * rem; idx += blockDim.x) {
+          const int i = k + 1 + idx / rem, j = k + 1 + idx % rem;
+          if (j >= i) {
+            const double2 u = G[k * ns + i], z = G[k * ns + j];
+            double2 v = G[i * ns + j];
+            v.x -= u.x * z.x + u.y * z.y;
+            v.y -= u.x * z.y - u.y * z.x;
+            G[i * ns + j] = v;
+          }
+        }
+        __syncthreads();
       }
+      if (!bad) break;
+      // breakdown: restore G from the backup with the shift on the diagonal
+      __syncthreads();
+      double tr = 0.0;
+      for (int k = 0; k < ns; ++k) tr += s_diag0[k];
+      const double shift = 11.0 * ((double)M * ns + (double)ns * (ns + 1)) * 1.1102230246251565e-16 * tr;
+      for (int idx = tid; idx < nout; idx += blockDim.x) {
+        double2 v = Ri[idx];
+        if (idx / ns == idx % ns) v.x += shift;
+        G[idx] = v;
+      }
+      if (tid == 0) { s_bad = 1; if (a.shifted) atomicAdd(a.shifted, 1); }
+      __syncthreads();
+    }
+    for (int idx = tid; idx < nout; idx += blockDim.x) Ri[idx] = make_double2(0.0, 0.0);
+    __syncthreads();
+    // R^-1 by back substitution, one column per thread
+    if (tid < ns) {
+      const int c = tid;
+      for (int i = c; i >= 0; --i) {
+        double2 s = make_double2(i == c ? 1.0 : 0.0, 0.0);
+        for (int k = i + 1; k <= c; ++k) {
+          const double2 r = G[i * ns + k], x = Ri[k * ns + c];
+          s.x -= r.x * x.x - r.y * x.y;
+          s.y -= r.x * x.y + r.y * x.x;
+        }
+        const double rii = G[i * ns + i].x;
+        Ri[i * ns + c] = make_double2(s.x / rii, s.y / rii);
+      }
+    }
+    for (int k = 0; k < ns; ++k) detR *= G[k * ns + k].x;
+    __syncthreads();
+    // phi <- phi R^-1, rows are independent
+    const int lane = tid & 31, rw = tid >> 5;
+    for (int q0 = 0; q0 < M; q0 += kRows) {
+      const int qr = min(kRows, M - q0);
+      __syncthreads();
+      for (int c = tid; c < qr * ns; c += blockDim.x) {
+        int pl = c / ns, j = c % ns;
+        sphi[pl * ldp + j] = Wc[(size_t)(q0 + pl) * Nt + off + j];
+      }
+      __syncthreads();
+      for (int pl = rw; pl < qr; pl += 8)
+        for (int i = lane; i < ns; i += 32) {
+          double2 s = make_double2(0.0, 0.0);
+          for (int j = 0; j <= i; ++j) {
+            const double2 z = sphi[pl * ldp + j], o = Ri[j * ns + i];
+            s.x += z.x * o.x - z.y * o.y;
+            s.y += z.x * o.y + z.y * o.x;
+          }
+          Wc[(size_t)(q0 + pl) * Nt + off + i] = s;
+        }
+    }
+    __syncthreads();
+    // stop after the pass that started within 0.05 of orthonormal, or when the walker is not finite
+    if (last || !(detR == detR) || !(fabs(detR) < 1e308)) break;
   }
+  if (tid == 0) a.detR[(size_t)w * a.nblk + blk] *= detR;
 }
 
 __global__ void ovlp_div_detR_kernel(double* ovlp, const double* detR, int nblk, int rhf, int nw) {

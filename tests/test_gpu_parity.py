@@ -506,6 +506,97 @@ def test_bounds_trigger_on_literal_amplitudes():
     assert np.all(np.isfinite(wo))
 
 
+# --------------------------------------------------------------------------- a10 on ill-conditioned walkers
+def _reortho_gpu(pr, W):
+    torch = _torch()
+    Wd = torch.from_numpy(np.ascontiguousarray(W)).cuda()
+    nblk = 1 if pr.cfg.walker_kind == 0 else 2
+    dR = torch.empty((W.shape[0], nblk), dtype=torch.float64, device="cuda")
+    torch.cuda.synchronize()
+    pr.gpu.reorthonormalise(Wd, dR)
+    pr.gpu.sync()
+    return Wd.cpu().numpy(), dR.cpu().numpy()
+
+
+def _check_qr(pr, W, Q, dR, kappa):
+    """Q against the definition (orthonormal, same span, R = Q^H phi upper triangular with a real positive diagonal)
+    to rounding, and against the oracle's Householder QR to the FORWARD accuracy the factorisation allows: Q and R of
+    a matrix with condition number kappa are only determined to ~kappa * eps by ANY backward-stable algorithm, so the
+    1e-10 of the well-conditioned case widens to max(1e-10, 50 kappa eps)."""
+    cfg = pr.cfg
+    blocks = [(0, cfg.n_alpha)] if cfg.walker_kind == 0 else [(0, cfg.n_alpha), (cfg.n_alpha, cfg.n_alpha + cfg.n_beta)]
+    Qo, detRo = pr.oracle.reorthonormalise(W)
+    tol = max(1e-10, 50 * kappa * 2.2e-16)
+    for w in range(W.shape[0]):
+        for b, (a0, a1) in enumerate(blocks):
+            q, phi = Q[w][:, a0:a1], W[w][:, a0:a1]
+            n = a1 - a0
+            assert np.abs(q.conj().T @ q - np.eye(n)).max() < 1e-13
+            R = q.conj().T @ phi
+            assert np.linalg.norm(phi - q @ R) < 1e-13 * np.linalg.norm(phi)
+            assert np.abs(np.tril(R, -1)).max() < 1e-13 * np.abs(R).max()
+            d = np.diag(R)
+            assert np.all(d.real > 0) and np.abs(d.imag).max() < 1e-13 * np.abs(R).max()
+            assert abs(np.prod(d.real) / dR[w, b] - 1.0) < tol * 10
+            assert np.linalg.norm(q - Qo[w][:, a0:a1]) < tol * np.sqrt(n)
+        det_g = dR[w, 0] ** 2 if cfg.walker_kind == 0 else dR[w, 0] * dR[w, 1]
+        assert abs(det_g / detRo[w] - 1.0) < tol * 20
+
+
+@pytest.mark.parametrize("name,nw", [("c1", 6), ("c2", 6)])
+@pytest.mark.parametrize("kappa", [1e4, 1e8, 1e12])
+def test_reortho_ill_conditioned(name, nw, kappa):
+    """Row a10 on walkers with nearly parallel columns: phi = U diag(sigma) V^H with singular
+    values from 1 down to 1 / kappa.  Cholesky-QR alone breaks down at kappa ~ 1e8 (Gram matrix not positive
+    definite in FP64); the kernel's shifted pass must take over (and only then)."""
+    _torch()
+    pr = Pair(name, nw=nw)
+    cfg = pr.cfg
+    r = np.random.default_rng(int(np.log10(kappa)))
+    W = np.empty((nw, cfg.M, cfg.Nt), dtype=np.complex128)
+    blocks = [(0, cfg.n_alpha)] if cfg.walker_kind == 0 else [(0, cfg.n_alpha), (cfg.n_alpha, cfg.n_alpha + cfg.n_beta)]
+    for w in range(nw):
+        for a0, a1 in blocks:
+            n = a1 - a0
+            U = np.linalg.qr(r.standard_normal((cfg.M, n)) + 1j * r.standard_normal((cfg.M, n)))[0]
+            V = np.linalg.qr(r.standard_normal((n, n)) + 1j * r.standard_normal((n, n)))[0]
+            sig = kappa ** (-np.arange(n) / (n - 1.0))
+            W[w][:, a0:a1] = (U * sig) @ V.conj().T
+    n0 = pr.gpu.qr_shifted_passes()
+    Q, dR = _reortho_gpu(pr, W)
+    _check_qr(pr, W, Q, dR, kappa)
+    shifted = pr.gpu.qr_shifted_passes() - n0
+    assert (shifted == 0) if kappa <= 1e4 else (shifted >= nw), shifted
+    pr.close()
+
+
+def test_reortho_after_long_free_projection():
+    """300 c1 steps without any re-orthonormalisation, then ONE QR: the library against the oracle's QR of the very
+    same walkers; the stored overlaps are divided by (det R)^2 and must equal the overlaps recomputed from Q."""
+    torch = _torch()
+    pr = Pair("c1", ortho_every=0)
+    cfg, nw = pr.cfg, pr.nw
+    Wd = torch.from_numpy(pr.walkers0.copy()).cuda()
+    wd = torch.ones(nw, dtype=torch.float64, device="cuda")
+    for s in range(300):
+        xd = torch.from_numpy(pr.fields(s)).cuda()
+        torch.cuda.synchronize()
+        pr.gpu.step(Wd, wd, xd, cfg.dt)
+    pr.gpu.sync()
+    W = Wd.cpu().numpy()
+    assert np.all(np.isfinite(W))
+    kappa = max(np.linalg.cond(W[k]) for k in range(nw))
+    dR = torch.empty((nw, 1), dtype=torch.float64, device="cuda")
+    ov = torch.empty(nw, dtype=torch.complex128, device="cuda")
+    pr.gpu.reorthonormalise(Wd, dR)
+    pr.gpu.get_overlaps(ov)
+    pr.gpu.sync()
+    Q = Wd.cpu().numpy()
+    _check_qr(pr, W, Q, dR.cpu().numpy(), kappa)
+    assert rel_max(ov.cpu().numpy(), pr.oracle.overlap(Q)) < 1e-10 * max(1.0, 1e-4 * kappa)
+    pr.close()
+
+
 def test_error_codes():
     torch = _torch()
     from paper_2406_16238_b200 import afqmc, inputs
