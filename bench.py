@@ -32,18 +32,23 @@ if ROOT not in sys.path:
 
 METRIC = "walker-steps/s (propagate + local energy)"
 UNIT = "walker-steps/s"
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the
-# `ncu --set full` captures summarised under profiles/ (file named beside each number).
-NCU_TRAFFIC = {
-    ("c5", "exchange"): 3.234e9,   # profiles/r1v4_full_c5.md (exchange_ws_kernel<4,3,4,7>, 3.220 GB rd + 0.014 GB wr)
-    ("c5", "vhs"): 30.48e9,        # profiles/r1v4_full_c5.md (vhs_ws_kernel<0>, 29.02 GB rd + 1.46 GB wr; upper tiles of L)
-}
+
+
+def ncu_traffic(workload, stage):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of a stage's kernel from profiles/ncu_traffic.json
+    (one `ncu --set full` capture per entry; the file names the capture and the commit it was taken on), or None."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            e = json.load(f).get(f"{workload}:{stage}")
+        return None if e is None else {"bytes": e["bytes"], "capture": e.get("capture"), "commit": e.get("commit")}
+    except (OSError, ValueError, KeyError):
+        return None
 
 
 def flops_model(cfg, nw, complex_fields=0):
     """Algorithmic real FP64 flops per launch of each contraction stage.
     complex_fields > 0: complex Cholesky vectors with that many Hermitian matrices (complex x complex products,
-    8 real flops per multiply-add; the exchange stage EXECUTES 1.5x this: three real-plane runs)."""
+    8 real flops per multiply-add; the exchange stage runs ONE pass over the two planes of Lrot)."""
     M, ng, K = cfg.M, cfg.n_chol, cfg.taylor_order
     blocks = [cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta]
     Nt = sum(blocks)
@@ -312,6 +317,9 @@ def main():
     ap.add_argument("--complex-chol", action="store_true",
                     help="complex Cholesky vectors (afqmc_params.complex_chol) on the workload's shapes: "
                          "n_chol / 2 complex vectors = n_chol Hermitian matrices = n_chol fields (c1-c3)")
+    ap.add_argument("--complex-trial", action="store_true",
+                    help="with --complex-chol: complex trial (afqmc_params.complex_trial), the lowest eigenvectors of "
+                         "the complex Hermitian h1")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
     ap.add_argument("--group", type=int, default=0,
@@ -354,13 +362,15 @@ def main():
         if cfg.n_chol * cfg.M * cfg.M * 8 > (2 << 30):
             raise SystemExit("--complex-chol: workloads c1-c3 only (the tensor is generated on the host)")
         hc, Lc, trial, walkers_c = inputs.make_complex_problem(cfg.M, cfg.n_alpha, cfg.n_beta, cfg.n_chol // 4,
-                                                               cfg.walker_kind, seed, nw)
+                                                               cfg.walker_kind, seed, nw,
+                                                               complex_trial=args.complex_trial)
         cx = dict(h=hc, L=Lc, walkers=walkers_c, nf=2 * Lc.shape[0])
         h1 = hc
         Ld = torch.from_numpy(Lc).cuda()
         g = afqmc.AFQMC(hc, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=Lc.shape[0],
                         max_walkers=nw, walker_kind=cfg.walker_kind, taylor_order=cfg.taylor_order,
-                        ortho_every=cfg.ortho_every, stream=stream.cuda_stream, complex_chol=True)
+                        ortho_every=cfg.ortho_every, stream=stream.cuda_stream, complex_chol=True,
+                        complex_trial=args.complex_trial)
         args.no_block = True
     else:
         Ld, _ = make_L(cfg, 0, False, True)
@@ -512,7 +522,11 @@ def main():
             "share_of_step": per_stage[dom]["ms_per_step"] / (ms_prof / K),
             "timing": "CUDA events of the library's own stage brackets on the launch stream, in a separate pass "
                       "over the same K steps (%.3f ms per step with the brackets on, %.3f without)" % (ms_prof / K, ms / K),
-            "traffic": NCU_TRAFFIC.get((cfg.name, dom))}
+            "traffic": None}
+    tr = ncu_traffic(cfg.name + ("+complex" if cx else ""), dom)
+    if tr:
+        roof["traffic"] = tr["bytes"]
+        roof["traffic_source"] = f"{tr['capture']} (commit {tr['commit']})"
     # the profiling guide's rule for a dtype without a measured peak: another dtype's measured peak x the
     # nominal ratio (bf16 burst figure of MEASURED_PEAKS.json x 40 / 2250 for FP64); a weaker denominator
     # than the DMMA rate measured above, kept beside it for comparison
@@ -535,7 +549,10 @@ def main():
                    "taylor_order": cfg.taylor_order, "ortho_every": cfg.ortho_every,
                    "local_energy": "every step", "parallelism": f"replicas x{world}",
                    "pack_chol": bool(args.pack_chol), "mixed_precision": bool(args.mixed_precision),
-                   "complex_chol": bool(args.complex_chol), "hbm_resident_gb": round(hbm_resident_gb, 1),
+                   "complex_chol": bool(args.complex_chol), "complex_trial": bool(args.complex_trial),
+                   "exchange_plan": [afqmc.exchange_plan(ns, cfg.M, bool(cx))[1] for ns in
+                                     ([cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta])],
+                   "hbm_resident_gb": round(hbm_resident_gb, 1),
                    "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "stages": per_stage, "block": block,
