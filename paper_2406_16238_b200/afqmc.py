@@ -98,7 +98,7 @@ def _load():
     lib.afqmc_qr_shifted_passes.restype = i64
     lib.afqmc_exchange_plan.argtypes = [i32, i32, i32, C.c_char_p, i32]
     lib.afqmc_exchange_plan.restype = i32
-    lib.afqmc_exchange_plan_pin.argtypes = [i32] * 9
+    lib.afqmc_exchange_plan_pin.argtypes = [i32] * 10
     lib.afqmc_exchange_plan_pin.restype = i32
     return lib
 
@@ -145,10 +145,10 @@ def exchange_plan(ns, M, pair=False):
     return rc * 1e-6, buf.value.decode()
 
 
-def exchange_plan_pin(ns, M, pair, warps, mi, ni, wm, G, Wn):
+def exchange_plan_pin(ns, M, pair, warps, mi, ni, wm, G, Wn, epi_warps=3):
     """Pin the exchange kernel's tile plan for (ns, M, pair); call before creating handles.  False if it does not fit."""
     return lib.afqmc_exchange_plan_pin(int(ns), int(M), int(bool(pair)), int(warps), int(mi), int(ni), int(wm),
-                                       int(G), int(Wn)) == 0
+                                       int(G), int(Wn), int(epi_warps)) == 0
 
 
 class AFQMC:

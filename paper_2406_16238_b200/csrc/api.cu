@@ -1223,9 +1223,9 @@ int32_t afqmc_exchange_plan(int32_t ns, int32_t M, int32_t pair, char* out, int3
 }
 
 int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t warps, int32_t mi, int32_t ni, int32_t wm,
-                                int32_t G, int32_t Wn) {
+                                int32_t G, int32_t Wn, int32_t epi_warps) {
   if (ns < 1 || ns > afq::kMaxOcc || M < ns) return AFQMC_ERR_INVALID;
-  return afq::exchange_ws_pin(ns, M, pair != 0, warps, mi, ni, wm, G, Wn) ? AFQMC_OK : AFQMC_ERR_UNSUPPORTED;
+  return afq::exchange_ws_pin(ns, M, pair != 0, warps, mi, ni, wm, G, Wn, epi_warps) ? AFQMC_OK : AFQMC_ERR_UNSUPPORTED;
 }
 
 int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {

@@ -30,8 +30,7 @@ namespace afq {
 namespace {
 
 constexpr int kProducerThreads = 128;     // one warpgroup (setmaxnreg is warpgroup-wide)
-constexpr int kEpiWarps = 3;              // warps 1..3 of the producer's warpgroup
-constexpr int kEpiThreads = kEpiWarps * 32;
+// epilogue warps: 3 (warps 1..3 of the producer's warpgroup) or 7 (a second warpgroup of them; 8 consumer warps only)
 constexpr int kSmemMax = 232448;          // 227 KB opt-in limit per CTA
 constexpr int kMaxTasks = 512;            // (gamma, walker, row pair) lane tasks per tile: 16 KB of partial sums
 constexpr int kMaxWarps = 12;
@@ -51,19 +50,20 @@ struct XwsArgs {
   unsigned rect[kMaxWarps];   // r0 | mi << 8 | c0 << 16 | ni << 24, in 8 x 8 blocks
 };
 
-template <int NCW, int MI, int NI>
+template <int NCW, int MI, int NI, int EW>
 struct XwsCfg {
   static constexpr int NCT = NCW * 32;
-  static constexpr int THREADS = NCT + kProducerThreads;
+  static constexpr int OTHER = (EW + 1) * 32;           // producer warp + epilogue warps
+  static constexpr int THREADS = NCT + OTHER;
+  static constexpr int EPT = EW * 32;
   // register file: THREADS * R0 at launch (R0 from __launch_bounds__), then PREGS for the producer's
   // warpgroup and CREGS for the consumers
   static constexpr int R0 = (65536 / THREADS) / 8 * 8;
   static constexpr int PREGS = NCW == 12 ? 40 : 56;
-  static constexpr int CREGS_ = ((THREADS * R0 - kProducerThreads * PREGS) / NCT) / 8 * 8;
+  static constexpr int CREGS_ = ((THREADS * R0 - OTHER * PREGS) / NCT) / 8 * 8;
   static constexpr int CREGS = CREGS_ > 232 ? 232 : CREGS_;
 };
 
-__device__ __forceinline__ void named_bar_sync_epi() { named_bar_sync(2, kEpiThreads); }
 
 // K = M loop of one tile for a warp rectangle of MU x NU blocks known at compile time (no predicates in the DMMA
 // stream); GENERIC: rectangle sizes from registers (small or odd problems), predicated.
@@ -105,12 +105,12 @@ __device__ __forceinline__ void xws_kloop(double (&acc)[MI][NI][2], uint32_t ful
   }
 }
 
-template <int NCW, int MI, int NI>
-__global__ void __launch_bounds__(XwsCfg<NCW, MI, NI>::THREADS, 1)
+template <int NCW, int MI, int NI, int EW>
+__global__ void __launch_bounds__(XwsCfg<NCW, MI, NI, EW>::THREADS, 1)
 exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__ TensorMap tmB,
                    const __grid_constant__ XwsArgs a) {
-  using Cfg = XwsCfg<NCW, MI, NI>;
-  constexpr int NCT = Cfg::NCT;
+  using Cfg = XwsCfg<NCW, MI, NI, EW>;
+  constexpr int NCT = Cfg::NCT, kEpiThreads = Cfg::EPT, kEpiWarps = EW;
   // SWIZZLE_128B tiles need a 1024-byte aligned base
   extern __shared__ __align__(1024) unsigned char smem[];
   if (smem_u32(smem) & 1023u) __trap();
@@ -255,7 +255,7 @@ exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant_
         }
       // fixed-order sums over the tile's vectors and row pairs, between two barriers of the epilogue warps (the
       // second one frees the table for the next tile)
-      named_bar_sync_epi();
+      named_bar_sync(2, kEpiThreads);
       // one warp per walker of the tile; a group of hp lanes (hp = h rounded up to a power of two) sums the row
       // pairs of one vector, 32 / hp vectors at a time, in a fixed order
       for (int wl = ew; wl < a.Wn; wl += kEpiWarps) {
@@ -291,7 +291,7 @@ exchange_ws_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant_
           eo[0] = sr; eo[1] = si;
         }
       }
-      named_bar_sync_epi();
+      named_bar_sync(2, kEpiThreads);
     }
     return;
   }
@@ -381,8 +381,9 @@ struct Plan {
   double bpf = 1e30;    // operand bytes per useful flop (shared-memory fill traffic out of L2)
 };
 
-struct Inst { int NCW, MI, NI; };
-constexpr Inst kInst[] = {{8, 5, 7}, {8, 7, 5}, {8, 6, 6}, {12, 4, 7}, {12, 7, 4}, {12, 5, 5}, {12, 5, 4}, {12, 4, 5}};
+struct Inst { int NCW, MI, NI, EW; };
+constexpr Inst kInst[] = {{8, 5, 7, 3}, {8, 7, 5, 3}, {8, 6, 6, 3}, {12, 4, 7, 3}, {12, 7, 4, 3}, {12, 5, 5, 3},
+                          {12, 5, 4, 3}, {12, 4, 5, 3}, {8, 5, 7, 7}, {8, 7, 5, 7}, {8, 6, 6, 7}};
 constexpr int kNumInst = sizeof(kInst) / sizeof(kInst[0]);
 
 // staging row stride: stride mod 16 in {6, 10} spreads the accumulator dump (8 rows x 4 columns per store
@@ -434,10 +435,14 @@ size_t fixed_smem(int ns, int nitems) {
 // 21 B/clk/SM at 92 % of the DMMA peak; 30 taken as the ceiling); every pass costs the DMMA warps a dump; the
 // epilogue warps need about 150 + 30 (ns - 1) clocks per round of 96 lane tasks and stall the consumers when a tile
 // has more passes than staging buffers, or when they cannot keep up with a short K loop.
+// clocks per pair of an epilogue lane while the DMMA pipe is saturated (its FP64 operations queue behind the DMMAs);
+// c2: 224 lane tasks of 15 pairs on 96 lanes held a 25 k-clock main loop up at 37 k clocks per tile
+constexpr double kEpiTrip = 150.0;
+
 std::vector<Plan> enumerate_plans(int ns, bool pair, int KT) {
   const int planes = pair ? 2 : 1;
   const int h = (ns + 1) / 2;
-  auto t_epi = [&](int items) { return 300.0 + ((items * h + kEpiThreads - 1) / kEpiThreads) * (150.0 + 30.0 * (ns - 1)); };
+  auto t_epi = [&](int items, int ew) { return 300.0 + ((items * h + 32 * ew - 1) / (32 * ew)) * kEpiTrip * (ns - 1); };
   std::vector<Plan> cands;
   for (int c = 0; c < kNumInst; ++c) {
     const Inst& I = kInst[c];
@@ -481,7 +486,7 @@ std::vector<Plan> enumerate_plans(int ns, bool pair, int KT) {
             // 12 consumer warps run on 152 registers (a few spills in the k loop), 8 on 224: measured 2 % apart
             double main = KT * std::max(64.0 * maxload, bytes / 30.0) * (S == 2 ? 1.03 : 1.0) * (I.NCW == 12 ? 1.02 : 1.0);
             const double dump = bp * (I.NCW / 4) * (6.0 * I.MI * I.NI + 150.0);
-            const double epi_pass = t_epi(q.Gp * q.Wp);
+            const double epi_pass = t_epi(q.Gp * q.Wp, I.EW);
             const double stall = std::max(0, bp - q.nbuf) * epi_pass;
             const double epi_all = bp * epi_pass + 300.0;
             // rectangles other than (MI | MI - 1) x (NI | NI - 1) run the predicated k loop
@@ -491,6 +496,9 @@ std::vector<Plan> enumerate_plans(int ns, bool pair, int KT) {
               generic = generic || mi < I.MI - 1 || ni < I.NI - 1;
             }
             if (generic) main *= 1.15;
+            // measured: seven epilogue warps pay off while the K loop is short (c2, c3), cost 5 % at c5 (200
+            // instead of 224 consumer registers)
+            if (I.EW == 7) main *= KT <= 32 ? 0.98 : 1.05;
             const double t_tile = std::max(main + 800.0 + dump + stall, epi_all);
             q.score = useful * KT / t_tile;
             cands.push_back(q);
@@ -501,8 +509,29 @@ std::vector<Plan> enumerate_plans(int ns, bool pair, int KT) {
   return cands;
 }
 
+// Plans found by sweeping every candidate on a B200 (afqmc_exchange_plan_pin; profiles/r2_exchange.md), for the
+// shapes of BASELINE.json's configs; any other shape takes the model's choice.
+struct Tuned { int ns, KT, pair, ncw, mi, ni, wm, G, Wn, ew; };
+constexpr Tuned kTuned[] = {
+    {16, 7, 0, 8, 5, 7, 4, 9, 3, 7},    // c2 alpha block: 144 x 96 tiles, 7 epilogue warps (short K loop)
+    {14, 7, 0, 8, 7, 5, 1, 4, 8, 7},    // c2 beta block: 56 x 224 tiles
+    {50, 19, 0, 8, 5, 7, 4, 3, 1, 7},   // c3
+    {40, 44, 0, 12, 5, 4, 4, 4, 1, 3},  // c4: 160 x 80 tiles in one pass
+    {42, 75, 0, 12, 4, 7, 4, 3, 2, 3},  // c5: 126 x 168 tiles, three passes through two buffers
+    {50, 19, 1, 12, 4, 5, 4, 1, 1, 3},  // complex c3 shapes
+};
+
 Plan make_plan(int ns, bool pair, int KT) {
   const std::vector<Plan> cands = enumerate_plans(ns, pair, KT);
+  for (const Tuned& t : kTuned) {
+    if (t.ns != ns || t.KT != KT || (t.pair != 0) != pair) continue;
+    const Plan* pick = nullptr;
+    for (const Plan& p : cands)
+      if (p.ncw == t.ncw && kInst[p.inst].MI == t.mi && kInst[p.inst].NI == t.ni && kInst[p.inst].EW == t.ew &&
+          p.WM == t.wm && p.G == t.G && p.Wn == t.Wn && (!pick || p.stages > pick->stages))
+        pick = &p;
+    if (pick) return *pick;
+  }
   // the most useful work per cycle; among plans within 1 % of it the one that moves the fewest bytes per flop (the
   // squarest tile), then the deeper ring
   Plan best;
@@ -515,10 +544,10 @@ Plan make_plan(int ns, bool pair, int KT) {
   return best;
 }
 
-template <int NCW, int MI, int NI>
+template <int NCW, int MI, int NI, int EW>
 int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
-  using Cfg = XwsCfg<NCW, MI, NI>;
-  auto kern = exchange_ws_kernel<NCW, MI, NI>;
+  using Cfg = XwsCfg<NCW, MI, NI, EW>;
+  auto kern = exchange_ws_kernel<NCW, MI, NI, EW>;
   static uint64_t attr = 0;
   if (auto once_ = first_use_on_device(&attr)) {
     cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kSmemMax);
@@ -580,12 +609,13 @@ double exchange_ws_efficiency(int ns, int M, bool pair) { return cached_plan(ns,
 
 // Tuning hook: replace the plan of (ns, M, pair) by the candidate with this warp count, rectangle bound, warp grid
 // and tile (the deepest ring that fits); false if there is no such candidate.
-bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn) {
+bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn, int ew) {
   const int KT = (M + 15) / 16;
   const std::vector<Plan> cands = enumerate_plans(ns, pair, KT);
   const Plan* pick = nullptr;
   for (const Plan& p : cands)
-    if (p.ncw == ncw && kInst[p.inst].MI == mi && kInst[p.inst].NI == ni && p.WM == wm && p.G == G && p.Wn == Wn &&
+    if (p.ncw == ncw && kInst[p.inst].MI == mi && kInst[p.inst].NI == ni && kInst[p.inst].EW == ew && p.WM == wm &&
+        p.G == G && p.Wn == Wn &&
         (!pick || p.stages > pick->stages))
       pick = &p;
   if (!pick) return false;
@@ -599,8 +629,8 @@ bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, 
 void exchange_ws_describe(int ns, int M, bool pair, char* out, int n) {
   const Plan& p = cached_plan(ns, pair, M);
   if (p.inst < 0) { snprintf(out, n, "no plan"); return; }
-  snprintf(out, n, "warps %d grid %dx%d (<=%dx%d blocks each) G %d Wn %d tile %dx%d eff %.3f stages %d passes %dx%d nbuf %d ldt %d smem %zu",
-           p.ncw, p.WM, p.ncw / p.WM, kInst[p.inst].MI, kInst[p.inst].NI, p.G, p.Wn, p.rowsA, p.rowsB, p.eff, p.stages,
+  snprintf(out, n, "warps %d+%d grid %dx%d (<=%dx%d blocks each) G %d Wn %d tile %dx%d eff %.3f stages %d passes %dx%d nbuf %d ldt %d smem %zu",
+           p.ncw, kInst[p.inst].EW, p.WM, p.ncw / p.WM, kInst[p.inst].MI, kInst[p.inst].NI, p.G, p.Wn, p.rowsA, p.rowsB, p.eff, p.stages,
            (p.G + p.Gp - 1) / p.Gp, (p.Wn + p.Wp - 1) / p.Wp, p.nbuf, p.ldt, p.smem);
 }
 
@@ -609,14 +639,17 @@ int run_exchange_ws(const ExArgs& e, cudaStream_t st) {
   const Plan& p = cached_plan(e.ns, e.plane_stride != 0, e.M);
   if (p.inst < 0) return -1;
   switch (p.inst) {
-    case 0: return launch_xws<8, 5, 7>(e, p, st);
-    case 1: return launch_xws<8, 7, 5>(e, p, st);
-    case 2: return launch_xws<8, 6, 6>(e, p, st);
-    case 3: return launch_xws<12, 4, 7>(e, p, st);
-    case 4: return launch_xws<12, 7, 4>(e, p, st);
-    case 5: return launch_xws<12, 5, 5>(e, p, st);
-    case 6: return launch_xws<12, 5, 4>(e, p, st);
-    case 7: return launch_xws<12, 4, 5>(e, p, st);
+    case 0: return launch_xws<8, 5, 7, 3>(e, p, st);
+    case 1: return launch_xws<8, 7, 5, 3>(e, p, st);
+    case 2: return launch_xws<8, 6, 6, 3>(e, p, st);
+    case 3: return launch_xws<12, 4, 7, 3>(e, p, st);
+    case 4: return launch_xws<12, 7, 4, 3>(e, p, st);
+    case 5: return launch_xws<12, 5, 5, 3>(e, p, st);
+    case 6: return launch_xws<12, 5, 4, 3>(e, p, st);
+    case 7: return launch_xws<12, 4, 5, 3>(e, p, st);
+    case 8: return launch_xws<8, 5, 7, 7>(e, p, st);
+    case 9: return launch_xws<8, 7, 5, 7>(e, p, st);
+    case 10: return launch_xws<8, 6, 6, 7>(e, p, st);
   }
   return -1;
 }

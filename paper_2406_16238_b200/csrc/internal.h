@@ -167,7 +167,7 @@ bool exchange_ws_usable(int M, const void* Lrot, const void* ThT);
 int exchange_ws_group_size(int ns, int M, bool pair = false);      // the plan depends on the K = M loop length
 double exchange_ws_efficiency(int ns, int M, bool pair = false);
 void exchange_ws_describe(int ns, int M, bool pair, char* out, int n);
-bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn);
+bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn, int ew);
 int run_exchange_ws(const ExArgs& a, cudaStream_t st);
 
 struct EnergyArgs {
