@@ -56,7 +56,8 @@ def flops_model(cfg, nw, complex_fields=0):
         nf = complex_fields
         return {
             "exchange": nw * sum(8.0 * nf * ns * ns * M + 8.0 * nf * ns * ns for ns in blocks),
-            "vhs": nw * 8.0 * nf * M * M,
+            # two runs of the symmetric-half kernel: Re planes (symmetric sum), Im planes (antisymmetric sum)
+            "vhs": nw * 4.0 * nf * M * (M + 1),
             "taylor": nw * 8.0 * K * M * M * Nt,
             "force_bias": nw * 8.0 * nf * Nt * M,
             "one_body": 2 * nw * 8.0 * M * M * Nt,

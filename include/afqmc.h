@@ -95,7 +95,9 @@ typedef struct {
   int32_t kernel_path;  /* 0: the TMA warp-specialised kernels wherever the shapes allow (even M), the cp.async    */
                         /* kernels otherwise.  1: force the cp.async kernels (what odd M runs; lets a test cover   */
                         /* them at even M on the same inputs).  2: the one-kernel overlap / Theta route instead of */
-                        /* the batched DMMA GEMMs.  Results agree to rounding; ignored for group_size > 1.         */
+                        /* the batched DMMA GEMMs.  3: as 0 but without the one-kernel step / local energy that 0  */
+                        /* picks for systems whose walker fits one CTA's shared memory (M <= 64, occupied blocks   */
+                        /* <= 16, n_chol <= 2048; c1).  Results agree to rounding; ignored for group_size > 1.     */
   int32_t complex_trial; /* 1: `trial` is complex128 [M][Nt] (PAPER.md:219 gives the trial no dtype; PAPER.md:328:   */
                         /* magnetic fields, spin-orbit coupling, Bloch orbitals).  <Psi_T| carries conj(psi):       */
                         /* O = psi^+ phi, Lrot = psi^+ K, hrot = psi^+ h, P = psi psi^+, m_g = tr(K_g P) (real).    */
@@ -246,7 +248,9 @@ int64_t afqmc_launch_count(const afqmc_handle* h);
 #define AFQMC_STAGE_ESTIMATORS 14    /* weighted sums of Code Snippet 9                       */
 #define AFQMC_STAGE_SHARD_EXCHANGE 15 /* distributed Hamiltonian: pushes into peer slots (copies)  */
 #define AFQMC_STAGE_SHARD_REDUCE 16   /* distributed Hamiltonian: fixed-order sums of the slots    */
-#define AFQMC_STAGE_COUNT 17
+#define AFQMC_STAGE_FUSED_STEP 17     /* small systems: rows a1-a9 in one kernel (fused_small.cu)   */
+#define AFQMC_STAGE_FUSED_ENERGY 18   /* small systems: row a11 in one kernel                       */
+#define AFQMC_STAGE_COUNT 19
 int32_t afqmc_set_profiling(afqmc_handle* h, int32_t on);
 /*   ms_out HOST double [AFQMC_STAGE_COUNT]; count_out HOST int64 [AFQMC_STAGE_COUNT] or NULL. */
 int32_t afqmc_get_stage_times(afqmc_handle* h, double* ms_out, int64_t* count_out, int32_t reset);

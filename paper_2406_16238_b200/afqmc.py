@@ -27,7 +27,7 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
           "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
-          "shard_exchange", "shard_reduce"]
+          "shard_exchange", "shard_reduce", "fused_step", "fused_energy"]
 
 
 class AfqmcParams(C.Structure):

@@ -62,6 +62,7 @@ struct afqmc_handle {
   double *Obuf = nullptr, *Aop = nullptr;       // overlap / inverse operands of the DMMA overlap-Theta route
   bool ot_gemm = false;
   int fb_split = 1;
+  bool small = false;   // whole step / local energy in one kernel each (fused_small.cu)
   bool ws = false;      // warp-specialised TMA kernels (even M); else the cp.async kernels
   bool ws_vhs = false;
   int* vhs_tiles = nullptr;
@@ -274,6 +275,16 @@ OTArgs ot_args(afqmc_handle* h, const double* W, double* det, int want_theta, in
   return a;
 }
 
+SmallArgs small_args(afqmc_handle* h, double* W) {
+  SmallArgs a{};
+  a.W = W; a.trial = h->trial; a.Lrot = h->Lrot; a.hrot = h->hrot; a.m = h->m; a.L = h->L; a.E1 = h->E1;
+  a.ovlp = h->ovlp; a.Xdbg = h->X; a.Adbg = h->A;
+  a.M = h->M; a.Nt = h->Nt; a.nblk = h->nblk; a.n_chol = h->n_chol; a.K = h->K; a.rhf = h->rhf;
+  for (int b = 0; b < 2; ++b) { a.off[b] = h->off[b]; a.ns[b] = h->ns[b]; }
+  a.sf = h->sf; a.xbar_bound = h->p.xbar_bound; a.ehyb_bound = h->p.ehyb_bound;
+  return a;
+}
+
 // exchange + Coulomb + final sums for the nw walkers whose Theta^T sits in h->ThT; e1 [nw][nblk]
 int energy_from_theta(afqmc_handle* h, const double* e1, double* E_out, int nw) {
   for (int b = 0; b < h->nblk; ++b) {
@@ -358,6 +369,13 @@ int local_energy_complex_device(afqmc_handle* h, const double* W, double* E_out,
 
 int local_energy_device(afqmc_handle* h, const double* W, double* E_out, int nw) {
   if (h->cplx) return local_energy_complex_device(h, W, E_out, nw);
+  if (h->small) {
+    StageTimer tm(h, AFQMC_STAGE_FUSED_ENERGY);
+    SmallArgs a = small_args(h, const_cast<double*>(W));
+    a.E_out = E_out;
+    h->launches += run_small_energy(a, nw, h->st);
+    return AFQMC_OK;
+  }
   {
     StageTimer tm(h, AFQMC_STAGE_E_THETA);
     h->launches += run_overlap_theta(ot_args(h, W, h->det_old, 1, 1), nw, h->st);
@@ -409,6 +427,7 @@ int force_bias_shift_device(afqmc_handle* h, const double* x, double dt, int nw)
   return AFQMC_OK;
 }
 
+void reortho_device(afqmc_handle* h, double* W, int nw, bool fix_overlaps);
 int finish_step_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
 int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, const double* cmf, double dt, int nw);
 
@@ -416,6 +435,19 @@ int step_device(afqmc_handle* h, double* W, double* wt, const double* x, double 
   const int M = h->M, nc = h->n_chol;
   const long MM = (long)M * M;
   if (!(h->dt_cached == dt)) build_E1(h, dt);
+  if (h->small) {
+    {
+      StageTimer tm(h, AFQMC_STAGE_FUSED_STEP);
+      SmallArgs a = small_args(h, W);
+      a.x = x; a.weights = wt;
+      a.sqrt_dt = sqrt(dt); a.dt = dt; a.expo = -dt * (h->E_const - h->e_shift);
+      h->launches += run_small_step(a, nw, h->st);
+    }
+    h->step_count += 1;
+    h->last_nw = nw;
+    if (h->p.ortho_every > 0 && h->step_count % h->p.ortho_every == 0) reortho_device(h, W, nw, true);
+    return AFQMC_OK;
+  }
 
   // a1/a2: overlap, Theta
   {
@@ -720,7 +752,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->n_alpha > kMaxOcc || p->n_beta > kMaxOcc) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "occupied block > 64 columns");
   // the per-walker kernels put the walker index in gridDim.y / gridDim.z (limit 65535)
   if (p->max_walkers > 65535) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "max_walkers > 65535");
-  if (p->kernel_path < 0 || p->kernel_path > 2) return fail(nullptr, AFQMC_ERR_INVALID, "kernel_path must be 0, 1 or 2");
+  if (p->kernel_path < 0 || p->kernel_path > 3) return fail(nullptr, AFQMC_ERR_INVALID, "kernel_path must be 0, 1, 2 or 3");
   const bool cplx = p->complex_chol == 1;
   const bool ctrial = p->complex_trial == 1;
   if (ctrial && !cplx) return fail(nullptr, AFQMC_ERR_UNSUPPORTED, "complex_trial needs complex_chol = 1");
@@ -1086,6 +1118,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->Obuf = dalloc(h, (size_t)mw * Nt * 2 * Nt); h->Aop = dalloc(h, (size_t)mw * 4 * Nt * Nt);
   if (!h->Obuf || !h->Aop) return bail(AFQMC_ERR_ALLOC, "device allocation failed (overlap operands)");
   h->ot_gemm = h->ws && p->kernel_path != 2;   // kernel_path = 2: the one-kernel overlap / Theta route (tests)
+  h->small = p->kernel_path == 0 && !cplx && !p->mixed_precision && !p->pack_chol && G == 1 &&
+             small_path_fits(M, Nt, std::max(h->ns[0], h->ns[1]), nc);
   if (G > 1) {
     h->theta_buf = h->ThT;
     h->a_slots = dalloc(h, (size_t)G * mw * 2 * MM);

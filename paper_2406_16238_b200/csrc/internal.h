@@ -275,6 +275,29 @@ int run_field_shift_cplx(const CShiftArgs& a, int nw, cudaStream_t st);
 int run_energy_cplx(const CEnergyArgs& a, cudaStream_t st);
 int run_e1(const OTArgs& a, int nw, cudaStream_t st);    // small.cu: one-body energy sum only
 
+// fused_small.cu: whole step / whole local energy in one kernel per call for small systems (c1-sized)
+struct SmallArgs {
+  double* W;                    // [nw][M][Nt] complex, in/out (step), in (energy)
+  const double* trial;          // [M][Nt]
+  const double* Lrot;           // [n_chol][Nt][M]
+  const double* hrot;           // [Nt][M]
+  const double* m;              // [n_chol]
+  const double* x;              // [nw][n_chol]
+  const double* L;              // [n_chol][M][M]
+  const double* E1;             // [M][M]
+  double* weights;              // [nw]
+  double* ovlp;                 // [nw] complex
+  double* Xdbg;                 // [nw][2][n_chol] or null (afqmc_debug_read 0)
+  double* Adbg;                 // [nw][2][M][M] or null (afqmc_debug_read 1)
+  double* E_out;                // [nw][3] complex
+  int M, Nt, nblk, n_chol, K, rhf, gchunk, lchunk;
+  int off[2], ns[2];
+  double sf, sqrt_dt, dt, expo, xbar_bound, ehyb_bound;
+};
+bool small_path_fits(int M, int Nt, int nsmax, int n_chol);
+int run_small_step(SmallArgs a, int nw, cudaStream_t st);
+int run_small_energy(SmallArgs a, int nw, cudaStream_t st);
+
 // setup.cu ---------------------------------------------------------------------------------
 int run_mean_field(const double* L, const double* P, double* m, int M, int n_chol, cudaStream_t st);
 int run_sum_mL(const double* L, const double* m, double* out, int M, int n_chol, cudaStream_t st);

@@ -42,9 +42,12 @@ def main():
         dmma, dfma, mhz = afqmc.measure_fp64_peak(ms)
         stop.set()
         t.join()
-        rec[name] = {"dmma_tflops": dmma, "dfma_tflops": dfma, "sm_mhz_from_clock64": mhz,
-                     "flop_per_clk_per_sm_dmma": dmma * 1e12 / (rec["sms"] * mhz * 1e6) if mhz else None,
-                     "nvidia_smi": {"sm_mhz": sorted(s[0] for s in samples)[len(samples) // 2] if samples else None,
+        smi_mhz = sorted(s[0] for s in samples)[len(samples) // 2] if samples else None
+        rec[name] = {"dmma_tflops": dmma, "dfma_tflops": dfma,
+                     # per SM and clock at the SM clock nvidia-smi reports under this load (128 = one DMMA.8x8x4 per
+                     # 4 clocks per SM)
+                     "flop_per_clk_per_sm_dmma": dmma * 1e12 / (rec["sms"] * smi_mhz * 1e6) if smi_mhz else None,
+                     "nvidia_smi": {"sm_mhz": smi_mhz,
                                     "sm_max_mhz": samples[0][1] if samples else None,
                                     "power_w_max": max((s[2] for s in samples), default=None),
                                     "sw_power_cap_seen": any(s[3] == "Active" for s in samples),

@@ -169,13 +169,14 @@ def test_free_running_parity(name, nw):
 
 
 # --------------------------------------------------------------------------- the other kernel paths at even M
-@pytest.mark.parametrize("path", [1, 2])
+@pytest.mark.parametrize("path", [1, 2, 3])
 @pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 24, {}),
                                           ("c1", 3, dict(M=90, n_alpha=42, n_beta=42, n_chol=38))])
 def test_kernel_paths_at_even_M(name, nw, over, path):
     """afqmc_params.kernel_path: 1 = the cp.async kernels (what odd M runs), 2 = the one-kernel overlap / Theta
-    route, both at EVEN M where the default is the TMA path: a step with QR and the local energy against the
-    oracle, and against the default path to rounding."""
+    route, both at EVEN M where the default is the TMA path; 3 = the multi-kernel path for a system small enough for
+    the one-kernel step / local energy that the default (0) picks (c1): a step with QR and the local energy against
+    the oracle, and against the default path to rounding."""
     _torch()
     pr = Pair(name, nw=nw, ortho_every=1, kernel_path=path, **over)
     ref = Pair(name, nw=nw, ortho_every=1, oracle=False, **over)
@@ -311,7 +312,7 @@ def test_pack_chol_gives_the_same_bits_and_releases_L(name, nw, over):
     longer reads the caller's dense tensor after afqmc_create (it is overwritten with NaN here);
     steps and energies are bit-identical to the dense-tensor handle and match the oracle."""
     torch = _torch()
-    dense = Pair(name, nw=nw, **over)
+    dense = Pair(name, nw=nw, kernel_path=3, **over)      # the multi-kernel path also at c1 (same V_HS kernel as packed)
     packed = Pair(name, nw=nw, oracle=False, pack_chol=True, **over)
     packed.L_dev.fill_(float("nan"))
     torch.cuda.synchronize()
