@@ -102,3 +102,26 @@ def test_shard_setup_reduce_adds_in_member_order():
         ref = ref + parts[k]
     assert np.array_equal(out, ref)
     assert afqmc.lib.afqmc_shard_setup_reduce(None, 2, 3, None) == -1
+
+
+def test_exchange_plan_exists_for_every_block_size():
+    """Host logic of the exchange kernel's tile plan (exchange_ws.cu: make_plan): every occupied-block size the
+    library accepts (1..64), short and long K loops, real and pair mode gets a plan that fits shared memory and wastes
+    less than half of the issued DMMA blocks; the shapes of BASELINE.json's configs take their tuned entries."""
+    from paper_2406_16238_b200 import afqmc
+    for pair in (False, True):
+        for M in (64, 108, 300, 1200):
+            for ns in range(1, 65):
+                if ns > M:
+                    continue
+                eff, desc = afqmc.exchange_plan(ns, M, pair)
+                smem = int(re.search(r"smem (\d+)", desc).group(1))
+                assert 0.5 < eff <= 1.0 + 1e-9, (ns, M, pair, desc)
+                assert smem <= 232448, (ns, M, pair, desc)
+    assert "warps 12+3" in afqmc.exchange_plan(42, 1200)[1] and "tile 126x168" in afqmc.exchange_plan(42, 1200)[1]
+    assert "warps 8+7" in afqmc.exchange_plan(50, 300)[1] and "tile 150x100" in afqmc.exchange_plan(50, 300)[1]
+    assert "warps 8+7" in afqmc.exchange_plan(16, 108)[1]
+    # pinning: a candidate that cannot exist is refused, one that exists replaces the plan
+    assert not afqmc.exchange_plan_pin(50, 300, False, 12, 4, 7, 4, 30, 30)
+    assert afqmc.exchange_plan_pin(50, 302, False, 12, 4, 7, 6, 3, 1)
+    assert "grid 6x2" in afqmc.exchange_plan(50, 302)[1]

@@ -507,6 +507,44 @@ def test_bounds_trigger_on_literal_amplitudes():
     assert np.all(np.isfinite(wo))
 
 
+# --------------------------------------------------------------------------- every exchange-kernel instantiation
+_INSTS = [(8, 5, 7, 3), (8, 7, 5, 3), (8, 6, 6, 3), (12, 4, 7, 3), (12, 7, 4, 3), (12, 5, 5, 3), (12, 5, 4, 3),
+          (12, 4, 5, 3), (8, 5, 7, 7), (8, 7, 5, 7), (8, 6, 6, 7)]
+
+
+@pytest.mark.parametrize("name,nw,over", [("c1", 7, dict(M=90, n_alpha=42, n_beta=42, n_chol=41)),
+                                          ("c2", 9, dict(M=60, n_alpha=16, n_beta=14, n_chol=50)),
+                                          ("c1", 5, dict(M=64, n_alpha=5, n_beta=5, n_chol=77))])
+def test_every_exchange_plan_gives_the_same_energy(name, nw, over):
+    """The local energy must not depend on the exchange kernel's tile plan (afqmc_exchange_plan_pin): for every
+    instantiation (consumer warps, rectangle bound, epilogue warps), every warp grid and a spread of tile sizes -
+    full and ragged tiles in both directions, one and several epilogue passes, compile-time and predicated warp
+    rectangles - the energies equal the oracle's.  (The tuned plans of the configs only ever run a few of these.)"""
+    _torch()
+    from paper_2406_16238_b200 import afqmc
+    base = Pair(name, nw=nw, **over)
+    cfg, o = base.cfg, base.oracle
+    W = base.walkers0
+    E_o = o.local_energy(W)
+    sc = energy_scale(o, W, E_o)
+    base.close()
+    blocks = [cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta]
+    tried = 0
+    for (ncw, mi, ni, ew) in _INSTS:
+        for wm in [d for d in range(1, ncw + 1) if ncw % d == 0]:
+            for G, Wn in ((1, 1), (2, 3), (3, 2), (5, 4), (9, 7), (13, 2)):
+                ok = [afqmc.exchange_plan_pin(ns, cfg.M, False, ncw, mi, ni, wm, G, Wn, ew) for ns in blocks]
+                if not all(ok):
+                    continue
+                pr = Pair(name, nw=nw, oracle=False, kernel_path=3, **over)
+                E_g = gpu_energy(pr, W)
+                pr.close()
+                for k in range(3):
+                    assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10, (ncw, mi, ni, ew, wm, G, Wn, k)
+                tried += 1
+    assert tried >= 20, tried
+
+
 # --------------------------------------------------------------------------- a10 on ill-conditioned walkers
 def _reortho_gpu(pr, W):
     torch = _torch()
