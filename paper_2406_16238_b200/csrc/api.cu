@@ -39,6 +39,7 @@ struct afqmc_handle {
   // population control / estimators
   double *cum = nullptr, *xi_dev = nullptr, *est_dev = nullptr, *ovlp_tmp = nullptr;
   int* pmap = nullptr;
+  KnStreamK sk = {nullptr, 0, nullptr, 0};   // stream-K scratch of the batched KN GEMMs (gemm_ws.cu)
   int* qr_shifted = nullptr;     // device counter: shifted Cholesky-QR passes (ill-conditioned walkers) so far
   // CUDA graphs of whole blocks (afqmc_run_block on device buffers), keyed by the call's arguments
   struct BlockGraph {
@@ -576,12 +577,12 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
       g.A = h->E1c; g.A2 = h->E1c + MM;
       if (h->ws)
         r = run_gemm_ws_kn(h->E1c, M, MM, 0, true, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
-                           nw, 1.0, 2, h->st);
+                           nw, 1.0, 2, h->st, &h->sk);
       h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
     } else {
       if (h->ws)
         r = run_gemm_ws_kn(h->E1, M, 0, 0, false, W, 2 * Nt, wstride, h->T0, h->Acc, 2 * Nt, wstride, M, 2 * Nt, M,
-                           nw, 1.0, 2, h->st);
+                           nw, 1.0, 2, h->st, &h->sk);
       h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
     }
   }
@@ -597,7 +598,7 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
       int r = -1;
       if (h->ws)
         r = run_gemm_ws_kn(h->A, M, MM, 2 * MM, true, Tp, 2 * Nt, wstride, Tn, h->Acc, 2 * Nt, wstride, M, 2 * Nt,
-                           M, nw, 1.0 / n, 1, h->st);
+                           M, nw, 1.0 / n, 1, h->st, &h->sk);
       h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
       std::swap(Tp, Tn);
     }
@@ -613,12 +614,12 @@ int propagate_device(afqmc_handle* h, double* W, double* wt, const double* cfb, 
       g.A = h->E1c; g.A2 = h->E1c + MM;
       if (h->ws)
         r = run_gemm_ws_kn(h->E1c, M, MM, 0, true, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
-                           nw, 1.0, 0, h->st);
+                           nw, 1.0, 0, h->st, &h->sk);
       h->launches += r > 0 ? r : run_gemm(GEMM_CPLX_KN, g, h->st);
     } else {
       if (h->ws)
         r = run_gemm_ws_kn(h->E1, M, 0, 0, false, h->Acc, 2 * Nt, wstride, W, nullptr, 2 * Nt, wstride, M, 2 * Nt, M,
-                           nw, 1.0, 0, h->st);
+                           nw, 1.0, 0, h->st, &h->sk);
       h->launches += r > 0 ? r : run_gemm(GEMM_KN, g, h->st);
     }
   }
@@ -1139,6 +1140,15 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->cum = dalloc(h, mw); h->xi_dev = dalloc(h, 4); h->est_dev = dalloc(h, 4); h->ovlp_tmp = dalloc(h, 2 * mw);
   h->pmap = (int*)dalloc(h, (mw + 1) / 2 + 1);
   h->qr_shifted = (int*)dalloc(h, 1);
+  if (h->ws) {
+    const int nsm = sm_count_current();
+    h->sk.part_doubles = (size_t)nsm * 2 * 2 * ((2 * Nt + 7) / 8 + 1) * 2 * 256;
+    h->sk.part = dalloc(h, h->sk.part_doubles);
+    h->sk.flag = (int*)dalloc(h, (nsm + 1) / 2 + 1);
+    h->sk.flags = nsm;
+    if (!h->sk.part || !h->sk.flag) return bail(AFQMC_ERR_ALLOC, "device allocation failed (stream-K scratch)");
+    cudaMemsetAsync(h->sk.flag, 0, (size_t)nsm * sizeof(int), h->st);
+  }
   if (h->qr_shifted) cudaMemsetAsync(h->qr_shifted, 0, 8, h->st);
   if (!h->cum || !h->xi_dev || !h->est_dev || !h->ovlp_tmp || !h->pmap || !h->qr_shifted)
     return bail(AFQMC_ERR_ALLOC, "device allocation failed (population control)");

@@ -34,7 +34,39 @@ struct KnArgs {
   int a_shared;        // A is the same matrix for every batch entry
   int stages;
   int nb16;            // 16-column boxes of B per n tile
+  // stream-K (sk_w > 0): CTA c works on the k iterations [c sk_w, (c + 1) sk_w) of the tile-major iteration space, so
+  // every SM gets the same amount of work whatever the tile count; a tile cut by a chunk boundary is finished by
+  // the CTA holding its LAST part, which adds the first part's accumulators out of sk_part[c - 1]
+  int sk_w;
+  double* sk_part;     // [grid][PL * MI * NI * 2][256]
+  int* sk_flag;        // [grid], zero between launches
 };
+
+// Work of one CTA as a short list of segments (tile, k range, mode): 0 whole tile, 1 first part of a tile whose rest
+// belongs to CTA c + 1 (accumulators go to sk_part[c]), 2 last part of a tile started by CTA c - 1.  The first part
+// comes FIRST so that the neighbour never waits long.
+struct KnSeg { int tile, kb, ke, mode; };
+__device__ __forceinline__ bool kn_segment(const KnArgs& a, int KT, int ntiles, int idx, KnSeg& s) {
+  if (a.sk_w <= 0) {
+    s.tile = blockIdx.x + idx * gridDim.x; s.kb = 0; s.ke = KT; s.mode = 0;
+    return s.tile < ntiles;
+  }
+  const long total = (long)ntiles * KT;
+  const long begin = (long)blockIdx.x * a.sk_w, end = min(begin + a.sk_w, total);
+  if (begin >= end) return false;
+  const int ft = (int)(begin / KT), kb = (int)(begin % KT);
+  const int lt = (int)((end - 1) / KT), ke = (int)((end - 1) % KT) + 1;
+  const bool head = ke < KT, tail = kb > 0;
+  if (head) {
+    if (idx == 0) { s.tile = lt; s.kb = 0; s.ke = ke; s.mode = 1; return true; }
+    idx -= 1;
+  }
+  const int f0 = ft + (tail ? 1 : 0), l0 = lt - (head ? 1 : 0);
+  if (idx <= l0 - f0) { s.tile = f0 + idx; s.kb = 0; s.ke = KT; s.mode = 0; return true; }
+  idx -= (l0 - f0 + 1);
+  if (tail && idx == 0) { s.tile = ft; s.kb = kb; s.ke = KT; s.mode = 2; return true; }
+  return false;
+}
 
 template <int MI, int NI, bool CPLX>
 struct KnCfg {
@@ -74,10 +106,12 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
       prefetch_tensormap(&tmA);
       prefetch_tensormap(&tmB);
       uint32_t it = 0;
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      KnSeg sg;
+      for (int si = 0; kn_segment(a, KT, ntiles, si, sg); ++si) {
+        const int tile = sg.tile;
         const int b = tile / per_b, rem = tile % per_b;
         const int mt = rem / a.ntiles_n, nt = rem % a.ntiles_n;
-        for (int kt = 0; kt < KT; ++kt, ++it) {
+        for (int kt = sg.kb; kt < sg.ke; ++kt, ++it) {
           const int s = it % S;
           mbar_wait(&empty[s], ((it / S) & 1) ^ 1);
           mbar_expect_tx(&full[s], Cfg::STAGE_BYTES);
@@ -109,7 +143,9 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
   const uint32_t aoff = (uint32_t)(warp * MI) * 1024u;
 
   uint32_t it = 0;
-  for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+  KnSeg sg;
+  for (int si = 0; kn_segment(a, KT, ntiles, si, sg); ++si) {
+    const int tile = sg.tile;
     const int b = tile / per_b, rem = tile % per_b;
     const int mt = rem / a.ntiles_n, nt = rem % a.ntiles_n;
 
@@ -121,7 +157,7 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
 #pragma unroll
         for (int j = 0; j < NI; ++j) acc[pl][i][j][0] = acc[pl][i][j][1] = 0.0;
 
-    for (int kt = 0; kt < KT; ++kt, ++it) {
+    for (int kt = sg.kb; kt < sg.ke; ++kt, ++it) {
       const int s = it % S;
       mbar_wait(&full[s], (it / S) & 1);
       consumer_release_prev(empty, it, S, lane);
@@ -151,6 +187,38 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
       }
     }
 
+    if (sg.mode != 0) {
+      constexpr int NACC = PL * MI * NI * 2;
+      if (sg.mode == 1) {                      // first part: park the accumulators, tell the neighbour, go on
+        double* dst = a.sk_part + (size_t)blockIdx.x * NACC * 256 + tid;
+        int q = 0;
+#pragma unroll
+        for (int pl = 0; pl < PL; ++pl)
+#pragma unroll
+          for (int i = 0; i < MI; ++i)
+#pragma unroll
+            for (int j = 0; j < NI; ++j) { dst[(q++) * 256] = acc[pl][i][j][0]; dst[(q++) * 256] = acc[pl][i][j][1]; }
+        __threadfence();
+        named_bar_sync(1, 256);
+        if (tid == 0) atomicExch(a.sk_flag + blockIdx.x, 1);
+        continue;
+      }
+      // last part: wait for the neighbour's first part (written as the very first thing it did), add it
+      if (tid == 0) {
+        while (atomicAdd(a.sk_flag + blockIdx.x - 1, 0) == 0) {}
+        atomicExch(a.sk_flag + blockIdx.x - 1, 0);      // ready for the next launch
+        __threadfence();
+      }
+      named_bar_sync(1, 256);
+      const double* src = a.sk_part + (size_t)(blockIdx.x - 1) * NACC * 256 + tid;
+      int q = 0;
+#pragma unroll
+      for (int pl = 0; pl < PL; ++pl)
+#pragma unroll
+        for (int i = 0; i < MI; ++i)
+#pragma unroll
+          for (int j = 0; j < NI; ++j) { acc[pl][i][j][0] += __ldcg(src + (q++) * 256); acc[pl][i][j][1] += __ldcg(src + (q++) * 256); }
+    }
     double* C = a.C + (size_t)b * a.sC;
     double* C2 = a.C2 ? a.C2 + (size_t)b * a.sC : nullptr;
 #pragma unroll
@@ -185,7 +253,7 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
 }
 
 template <int MI, int NI, bool CPLX>
-int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, cudaStream_t st) {
+int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, const KnStreamK* sk, cudaStream_t st) {
   using Cfg = KnCfg<MI, NI, CPLX>;
   auto kern = gemm_ws_kn_kernel<MI, NI, CPLX>;
   static uint64_t attr = 0;
@@ -199,14 +267,27 @@ int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, cudaStream_t
   const size_t smem = (size_t)S * Cfg::STAGE_BYTES + 1024 + 256;
   const long nt = (long)a.mtiles * a.ntiles_n * a.batch;
   const int grid = nt < sm_count() ? (int)nt : sm_count();
+  a.sk_w = 0; a.sk_part = nullptr; a.sk_flag = nullptr;
+  if (sk && sk->part && sk->flag && nt > grid && nt % grid != 0) {
+    // stream-K when the tile count leaves a partial last wave (c5 Taylor: 1216 tiles = 8.2 waves on 148 SMs)
+    const int KT = (a.K + 15) / 16;
+    const long w = (nt * KT + grid - 1) / grid;
+    const size_t need = (size_t)grid * Cfg::PL * MI * NI * 2 * 256;
+    // parking and fetching a tile's accumulators costs about 8 k iterations per CTA (c2, c3: no gain, measured)
+    const long plain = ((nt + grid - 1) / grid) * KT;
+    if (w >= KT && (double)(w + 8) < 0.99 * plain && need <= sk->part_doubles && grid <= sk->flags) {
+      a.sk_w = (int)w; a.sk_part = sk->part; a.sk_flag = sk->flag;
+    }
+  }
   kern<<<grid, Cfg::THREADS, smem, st>>>(tmA, tmB, a);
   return 1;
 }
 
 template <bool CPLX>
-int dispatch_kn(int MI, int NI, const TensorMap& tmA, const TensorMap& tmB, const KnArgs& a, cudaStream_t st) {
+int dispatch_kn(int MI, int NI, const TensorMap& tmA, const TensorMap& tmB, const KnArgs& a, const KnStreamK* sk,
+                cudaStream_t st) {
 #define KN_CASE(mi, ni) \
-  if (MI == mi && NI == ni) return launch_kn<mi, ni, CPLX>(tmA, tmB, a, st);
+  if (MI == mi && NI == ni) return launch_kn<mi, ni, CPLX>(tmA, tmB, a, sk, st);
   KN_CASE(1, 2) KN_CASE(1, 4) KN_CASE(1, 6) KN_CASE(1, 8) KN_CASE(1, 10) KN_CASE(1, 11) KN_CASE(1, 12)
   KN_CASE(1, 13) KN_CASE(1, 14) KN_CASE(1, 16)
   KN_CASE(2, 2) KN_CASE(2, 4) KN_CASE(2, 6) KN_CASE(2, 8) KN_CASE(2, 10) KN_CASE(2, 11) KN_CASE(2, 12)
@@ -342,7 +423,7 @@ bool al16(const void* p) { return ((uintptr_t)p & 15) == 0; }
 // shapes cannot be served (caller falls back to the cp.async GEMM).
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
                    double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,
-                   int mode, cudaStream_t st) {
+                   int mode, cudaStream_t st, const KnStreamK* sk) {
   if (!(even(lda) && even(sPlane) && even(sA) && even(ldb) && even(sB) && even(ldc) && even(sC) && even(N)))
     return -1;
   if (!(al16(A) && al16(B) && al16(C) && (C2 == nullptr || al16(C2)))) return -1;
@@ -382,7 +463,7 @@ int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, c
   a.M = M; a.N = N; a.K = K; a.batch = batch;
   a.mtiles = (M + 64 * MI - 1) / (64 * MI); a.ntiles_n = ntn;
   a.a_shared = sA == 0; a.stages = 0; a.nb16 = (NI + 1) / 2;
-  return cplx ? dispatch_kn<true>(MI, NI, tmA, tmB, a, st) : dispatch_kn<false>(MI, NI, tmA, tmB, a, st);
+  return cplx ? dispatch_kn<true>(MI, NI, tmA, tmB, a, sk, st) : dispatch_kn<false>(MI, NI, tmA, tmB, a, sk, st);
 }
 
 // split-K choice for the NK GEMM: the slice count whose tile count fills the SM grid best

@@ -226,9 +226,11 @@ int taylor_tc_apply(const void* Aplanes, bool real_shared, const void* Tb, void*
                     const double* Src, double alpha, int nw, int M, int N2, cudaStream_t st);
 
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
+// stream-K scratch of one caller (stream): accumulators of the tiles cut by a chunk boundary + one flag per CTA
+struct KnStreamK { double* part; size_t part_doubles; int* flag; int flags; };
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
                    double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,
-                   int mode, cudaStream_t st);
+                   int mode, cudaStream_t st, const KnStreamK* sk = nullptr);
 int gemm_ws_nk_split(int M, int N, int K, int max_split);
 int run_gemm_ws_nk(const double* A, long lda, const double* B, long ldb, double* C, long ldc, long sCsplit,
                    int M, int N, int K, int split, cudaStream_t st);
