@@ -347,7 +347,8 @@ int32_t afqmc_exchange_plan(int32_t ns, int32_t M, int32_t pair, char* out, int3
 /* Tuning hook (host only): replace the plan chosen for (ns, M, pair) in this process by the candidate with `warps`
  * consumer warps (8 or 12) arranged as wm x (warps / wm), warp rectangles of at most mi x ni DMMA blocks, G vectors x
  * Wn walkers per tile, epi_warps (3, or 7 with 8 consumer warps) epilogue warps.  Results do not depend on the plan beyond the order of the fixed-order sums.  Handles
- * created BEFORE the call keep buffers sized for the old plan: pin first, then create.  AFQMC_ERR_UNSUPPORTED if
+ * created BEFORE the call keep buffers sized for the old plan: pin first, then create (afqmc_local_energy on an older
+ * handle returns AFQMC_ERR_INVALID if the new plan groups the vectors differently).  AFQMC_ERR_UNSUPPORTED if
  * no such candidate exists (does not fit shared memory or registers). */
 int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t warps, int32_t mi, int32_t ni, int32_t wm,
                                 int32_t G, int32_t Wn, int32_t epi_warps);

@@ -293,9 +293,10 @@ int energy_from_theta(afqmc_handle* h, const double* e1, double* E_out, int nw) 
     ExArgs e;
     e.Lrot = h->Lrot; e.ThT = h->ThT; e.expart = h->expart[b]; e.X = h->Xe;
     e.M = h->M; e.Nt = h->Nt; e.n_chol = h->n_chol; e.nw = nw;
-    e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
+    e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0; e.ngroups_cap = h->exgroups[b];
     if (h->ws) {
       const int r = run_exchange_ws(e, h->st);
+      if (r == -2) return fail(h, AFQMC_ERR_INVALID, "exchange: the tile plan was changed (afqmc_exchange_plan_pin) after this handle was created");
       if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
       h->launches += r;
     } else {
@@ -332,8 +333,9 @@ int local_energy_complex_device(afqmc_handle* h, const double* W, double* E_out,
       ExArgs e;
       e.Lrot = h->Lrot; e.plane_stride = (long)lsz; e.ThT = h->ThT; e.expart = h->expart_c[0][b]; e.X = h->Xe;
       e.M = h->M; e.Nt = h->Nt; e.n_chol = nf; e.nw = nw;
-      e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0;
+      e.off = h->off[b]; e.ns = h->ns[b]; e.accumulate = b > 0; e.ngroups_cap = h->exgroups_c[b];
       const int r = run_exchange_ws(e, h->st);
+      if (r == -2) return fail(h, AFQMC_ERR_INVALID, "exchange: the tile plan was changed (afqmc_exchange_plan_pin) after this handle was created");
       if (r < 0) return fail(h, AFQMC_ERR_CUDA, "exchange: tensor map encode failed");
       h->launches += r;
     }

@@ -634,10 +634,12 @@ void exchange_ws_describe(int ns, int M, bool pair, char* out, int n) {
            (p.G + p.Gp - 1) / p.Gp, (p.Wn + p.Wp - 1) / p.Wp, p.nbuf, p.ldt, p.smem);
 }
 
-// returns launches issued, or -1 if the tensor maps could not be encoded
+// returns launches issued, -1 if the tensor maps could not be encoded, -2 if the plan needs more partial-sum rows
+// than the caller allocated
 int run_exchange_ws(const ExArgs& e, cudaStream_t st) {
   const Plan& p = cached_plan(e.ns, e.plane_stride != 0, e.M);
   if (p.inst < 0) return -1;
+  if (e.ngroups_cap > 0 && (e.n_chol + p.G - 1) / p.G != e.ngroups_cap) return -2;   // the reduce sums exactly cap rows
   switch (p.inst) {
     case 0: return launch_xws<8, 5, 7, 3>(e, p, st);
     case 1: return launch_xws<8, 7, 5, 3>(e, p, st);

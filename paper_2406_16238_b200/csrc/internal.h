@@ -157,6 +157,8 @@ struct ExArgs {
   int M, Nt, n_chol, nw;
   int off, ns;                  // spin block
   int accumulate;               // 1: add to expart / X (second spin block)
+  int ngroups_cap = 0;          // > 0: rows of `expart` the caller allocated and sums; exchange_ws refuses (-2) a plan that writes another count
+                                // (a plan pinned after the handle was created)
   long plane_stride = 0;        // != 0 (exchange_ws only): Lrot = Lr + i Li, the imaginary plane starts plane_stride
                                 // doubles after Lrot; T is then the complex product and X = tr(T) of it
 };

@@ -543,6 +543,24 @@ def test_every_exchange_plan_gives_the_same_energy(name, nw, over):
                     assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10, (ncw, mi, ni, ew, wm, G, Wn, k)
                 tried += 1
     assert tried >= 20, tried
+    # a plan pinned AFTER a handle was created would make the kernel write another number of partial-sum rows than
+    # the handle allocated and sums: the library refuses instead
+    pr = Pair(name, nw=nw, oracle=False, kernel_path=3, **over)
+    ns0 = blocks[0]
+    _, before = afqmc.exchange_plan(ns0, cfg.M)
+    G_now = int(before.split(" G ")[1].split()[0])
+    for (ncw, mi, ni, ew) in _INSTS:
+        done = False
+        for wm in [d for d in range(1, ncw + 1) if ncw % d == 0]:
+            if afqmc.exchange_plan_pin(ns0, cfg.M, False, ncw, mi, ni, wm, 1 if G_now != 1 else 2, 1, ew):
+                done = True
+                break
+        if done:
+            break
+    assert done
+    with pytest.raises(afqmc.AfqmcError):
+        gpu_energy(pr, W)
+    pr.close()
 
 
 # --------------------------------------------------------------------------- a10 on ill-conditioned walkers
