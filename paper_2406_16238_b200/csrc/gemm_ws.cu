@@ -139,6 +139,21 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
       const int k = 8 * kp + 2 * t + par;
       lb[kp][par] = (uint32_t)(k * 128 + (((g >> 1) ^ (k & 7)) << 4) + (g & 1) * 8);
     }
+  // Paired blocks: ONE 16-byte load per k row gives a lane the columns (2 g, 2 g + 1) of a 16-column box, i.e. the B
+  // fragments of TWO blocks whose columns are interleaved (block 2 j2 takes the even columns of box j2, block
+  // 2 j2 + 1 the odd ones; the epilogue undoes the interleave).  Half the fragment-load instructions of the 8-byte
+  // loads; an unpaired last block (odd NI) keeps them.
+  uint32_t lbp[2][2];
+#pragma unroll
+  for (int kp = 0; kp < 2; ++kp)
+#pragma unroll
+    for (int par = 0; par < 2; ++par) {
+      const int k = 8 * kp + 2 * t + par;
+      lbp[kp][par] = (uint32_t)(k * 128 + ((g ^ (k & 7)) << 4));
+    }
+  // measured on B200: pairing gains 2.5 % (NI = 11, c5), 5 % (13, c3), 9 % (8, c2) on the Taylor GEMM and loses 4 % for
+  // the planar-complex kernel at NI = 10 (c4), which therefore keeps the 8-byte loads
+  constexpr int NP = (CPLX && NI == 10) ? 0 : NI / 2;           // paired boxes
   const uint32_t smem_u = smem_u32(smem);
   const uint32_t aoff = (uint32_t)(warp * MI) * 1024u;
 
@@ -171,7 +186,27 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
 #pragma unroll
           for (int i = 0; i < MI; ++i) af[pl][i] = lds128(sa + pl * (BM * 128) + i * 1024 + (kp ? la1 : la0));
 #pragma unroll
-        for (int j = 0; j < NI; ++j) {
+        for (int j2 = 0; j2 < NP; ++j2) {
+          const uint32_t bo = sb + j2 * 2048;
+          const double2 q0 = lds128(bo + lbp[kp][0]);       // k even: columns 2 g, 2 g + 1
+          const double2 q1 = lds128(bo + lbp[kp][1]);       // k odd
+#pragma unroll
+          for (int pl = 0; pl < PL; ++pl)
+#pragma unroll
+            for (int i = 0; i < MI; ++i) {
+              dmma884(acc[pl][i][2 * j2][0], acc[pl][i][2 * j2][1], af[pl][i].x, q0.x);
+              dmma884(acc[pl][i][2 * j2 + 1][0], acc[pl][i][2 * j2 + 1][1], af[pl][i].x, q0.y);
+            }
+#pragma unroll
+          for (int pl = 0; pl < PL; ++pl)
+#pragma unroll
+            for (int i = 0; i < MI; ++i) {
+              dmma884(acc[pl][i][2 * j2][0], acc[pl][i][2 * j2][1], af[pl][i].y, q1.x);
+              dmma884(acc[pl][i][2 * j2 + 1][0], acc[pl][i][2 * j2 + 1][1], af[pl][i].y, q1.y);
+            }
+        }
+#pragma unroll
+        for (int j = 2 * NP; j < NI; ++j) {                  // unpaired blocks (an odd last one): 8-byte loads
           const uint32_t bo = sb + (j >> 1) * 2048;
           const double b0 = lds64(bo + (lb[kp][0] ^ ((j & 1) * 64)));
           const double b1 = lds64(bo + (lb[kp][1] ^ ((j & 1) * 64)));
@@ -225,18 +260,8 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
     for (int i = 0; i < MI; ++i) {
       const int r = mt * BM + 8 * (warp * MI + i) + p;
       if (r >= a.M) continue;
-#pragma unroll
-      for (int j = 0; j < NI; ++j) {
-        const int n = (nt * NB16 * 2 + j) * 8 + 2 * t;
-        if (n >= a.N) continue;
-        double v0, v1;
-        if constexpr (CPLX) {
-          v0 = a.alpha * (acc[0][i][j][0] - acc[PL - 1][i][j][1]);
-          v1 = a.alpha * (acc[0][i][j][1] + acc[PL - 1][i][j][0]);
-        } else {
-          v0 = a.alpha * acc[0][i][j][0];
-          v1 = a.alpha * acc[0][i][j][1];
-        }
+      auto put = [&](int n, double v0, double v1) {
+        if (n >= a.N) return;
         const size_t off = (size_t)r * a.ldc + n;
         *reinterpret_cast<double2*>(C + off) = make_double2(v0, v1);
         if (C2) {
@@ -247,6 +272,37 @@ gemm_ws_kn_kernel(const __grid_constant__ TensorMap tmA, const __grid_constant__
             *reinterpret_cast<double2*>(C2 + off) = make_double2(v0, v1);
           }
         }
+      };
+#pragma unroll
+      for (int j2 = 0; j2 < NP; ++j2) {
+        // the lane holds columns 4 t .. 4 t + 3 of box j2: (even block c0, odd block c0, even block c1, odd block c1)
+        const int n = (nt * NB16 + j2) * 16 + 4 * t;
+        const int je = 2 * j2, jo = 2 * j2 + 1;
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+          double v0, v1;
+          if constexpr (CPLX) {      // (re, im) columns: re = P_re - Q_im, im = P_im + Q_re
+            v0 = a.alpha * (acc[0][i][je][h] - acc[PL - 1][i][jo][h]);
+            v1 = a.alpha * (acc[0][i][jo][h] + acc[PL - 1][i][je][h]);
+          } else {
+            v0 = a.alpha * acc[0][i][je][h];
+            v1 = a.alpha * acc[0][i][jo][h];
+          }
+          put(n + 2 * h, v0, v1);
+        }
+      }
+#pragma unroll
+      for (int j = 2 * NP; j < NI; ++j) {
+        const int n = (nt * NB16 * 2 + j) * 8 + 2 * t;
+        double v0, v1;
+        if constexpr (CPLX) {
+          v0 = a.alpha * (acc[0][i][j][0] - acc[PL - 1][i][j][1]);
+          v1 = a.alpha * (acc[0][i][j][1] + acc[PL - 1][i][j][0]);
+        } else {
+          v0 = a.alpha * acc[0][i][j][0];
+          v1 = a.alpha * acc[0][i][j][1];
+        }
+        put(n, v0, v1);
       }
     }
   }
