@@ -164,6 +164,33 @@ int32_t afqmc_local_energy(afqmc_handle* h, const void* walkers, void* E_out, in
 int32_t afqmc_population_control(afqmc_handle* h, void* walkers, double* weights, const double* xi,
                                  int32_t nw, int32_t* map_out);
 
+/* The comb of afqmc_population_control WITHOUT a handle and without any allocation: weights in, resampling map and
+ * equalised weights out - the same map and the same weights, bit for bit, that afqmc_population_control returns for
+ * these weights and this xi (permuting walkers, overlaps or anything else by map_out is left to the caller).
+ * For whom: every other entry point needs an afqmc_handle, and afqmc_create cudaMallocs the workspaces of the whole
+ * step.  A driver that only resamples, or that runs when no device memory is left to hand out (the Cholesky tensor and
+ * the application's own memory pool own the GPU, so cudaMalloc fails), or that must not take the device-wide stall a
+ * cudaMalloc / cudaFree implies while its other streams are busy, calls this instead: the comb's only scratch, the
+ * running sum of the weights, sits in a fixed array inside the library image (8 bytes x
+ * AFQMC_COMB_STATIC_MAX_WALKERS = 512 KiB, held on every GPU that loads the library until the process exits).  The
+ * call makes no cudaMalloc, cudaFree or other allocating call and creates no stream or event.
+ *   weights DEVICE double [nw], in/out: on return every weight is W / nw (unchanged if W is not finite or not > 0).
+ *   xi      DEVICE one double, the caller's uniform draw; clamped into [0, 1) on the device (NaN -> 0).
+ *   map_out DEVICE int32 [nw]: new walker k is a copy of old walker map_out[k] (non-decreasing).
+ *   nw      1 .. AFQMC_COMB_STATIC_MAX_WALKERS; anything larger is refused with AFQMC_ERR_DIMS and a message.
+ *   stream  cudaStream_t of the device that holds the three arrays (they must be plain device memory of ONE GPU;
+ *           host and managed pointers are refused); NULL = that device's default stream.  The call is asynchronous.
+ *   err     HOST char [err_len] or NULL: receives a message when the return value is not AFQMC_OK.
+ * First call on each device: the library looks up the array's address on that device (cudaGetSymbolAddress, which
+ * may load the library's device code there).  Make that first call outside any stream capture.
+ * Sharing: all calls on one device use the same array.  Calls queued on ONE stream are safe back to back (every
+ * call rewrites the part it reads; nothing needs clearing).  Calls that can run at the same time on one GPU - two
+ * streams, two host threads, two handles' drivers - overwrite each other's sums and return garbage maps: order
+ * them yourself.  Different GPUs have different copies and do not interfere. */
+#define AFQMC_COMB_STATIC_MAX_WALKERS 65536
+int32_t afqmc_comb_static(double* weights, const double* xi, int32_t* map_out, int32_t nw, void* stream, char* err,
+                          int32_t err_len);
+
 /* Estimator sums of the paper's Code Snippet 9:
  * est_out[0..3] = (ENumer, EDenom, E1Body, E2Body) = sum_w weights[w] (Re E[w][0], 1, Re E[w][1],
  * Re E[w][2]); the mixed energy estimate of Eq. (11) with Eq. (10)'s weights is ENumer/EDenom.

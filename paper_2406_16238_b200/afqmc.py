@@ -23,7 +23,9 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
            "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
            "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce", "afqmc_exchange_plan", "afqmc_exchange_plan_pin",
-           "afqmc_reorthonormalise", "afqmc_qr_shifted_passes"]
+           "afqmc_reorthonormalise", "afqmc_qr_shifted_passes", "afqmc_comb_static"]
+
+COMB_STATIC_MAX_WALKERS = 65536      # AFQMC_COMB_STATIC_MAX_WALKERS of include/afqmc.h
 
 STAGES = ["overlap_theta", "force_bias", "field_shift", "vhs", "one_body", "taylor", "overlap_new",
           "weight", "reortho", "e_theta", "exchange", "e_reduce", "e1_build", "pop_control", "estimators",
@@ -96,6 +98,8 @@ def _load():
     lib.afqmc_reorthonormalise.restype = i32
     lib.afqmc_qr_shifted_passes.argtypes = [vp]
     lib.afqmc_qr_shifted_passes.restype = i64
+    lib.afqmc_comb_static.argtypes = [vp, vp, vp, i32, vp, C.c_char_p, i32]
+    lib.afqmc_comb_static.restype = i32
     lib.afqmc_exchange_plan.argtypes = [i32, i32, i32, C.c_char_p, i32]
     lib.afqmc_exchange_plan.restype = i32
     lib.afqmc_exchange_plan_pin.argtypes = [i32] * 10
@@ -134,6 +138,19 @@ def measure_fp64_peak(ms=200.0):
     if rc != 0:
         raise AfqmcError(rc, "afqmc_measure_fp64_peak")
     return tuple(out)
+
+
+def comb_static(weights, xi, map_out, nw=None, stream=None):
+    """afqmc_comb_static: the population-control comb for callers that cannot allocate device memory - no handle, no
+    cudaMalloc; the running sum lives in a 512 KiB array built into the library (at most COMB_STATIC_MAX_WALKERS
+    walkers).  `weights` (float64, in/out), `xi` (one float64) and `map_out` (int32) are CUDA tensors on one GPU;
+    `stream` is a raw cudaStream_t of that GPU (None: its default stream).  Asynchronous; calls that may overlap on
+    one GPU share the array and must be ordered by the caller."""
+    n = int(weights.shape[0]) if nw is None else int(nw)
+    buf = C.create_string_buffer(512)
+    rc = lib.afqmc_comb_static(_ptr(weights), _ptr(xi), _ptr(map_out), n, stream, buf, len(buf))
+    if rc != 0:
+        raise AfqmcError(rc, buf.value.decode())
 
 
 def exchange_plan(ns, M, pair=False):

@@ -12,7 +12,7 @@ from concurrent.futures import ThreadPoolExecutor
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libafqmc.so")
-SOURCES = ["api.cu", "gemm.cu", "small.cu", "exchange.cu", "exchange_ws.cu", "vhs_ws.cu", "vhs_tc.cu", "taylor_tc.cu", "gemm_ws.cu", "tmap.cu", "setup.cu", "block.cu", "shard.cu", "cplx.cu", "peak.cu", "fused_small.cu"]
+SOURCES = ["api.cu", "gemm.cu", "small.cu", "exchange.cu", "exchange_ws.cu", "vhs_ws.cu", "vhs_tc.cu", "taylor_tc.cu", "gemm_ws.cu", "tmap.cu", "setup.cu", "block.cu", "shard.cu", "cplx.cu", "peak.cu", "fused_small.cu", "comb_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 
