@@ -321,6 +321,9 @@ def main():
     ap.add_argument("--complex-trial", action="store_true",
                     help="with --complex-chol: complex trial (afqmc_params.complex_trial), the lowest eigenvectors of "
                          "the complex Hermitian h1")
+    ap.add_argument("--min-seconds", type=float, default=0.0,
+                    help="raise K until the timed region lasts at least this long (small workloads: the clock "
+                         "sampler needs >= 1 s for its five samples); the line reports the K that was timed")
     ap.add_argument("--no-block", action="store_true", help="skip the 25-step block timing")
     ap.add_argument("--block-reps", type=int, default=3)
     ap.add_argument("--group", type=int, default=0,
@@ -385,6 +388,9 @@ def main():
         torch.cuda.empty_cache()
     hbm_resident_gb = (torch.cuda.mem_get_info()[1] - torch.cuda.mem_get_info()[0]) / 1e9
     peak_dmma, peak_dfma, _ = afqmc.measure_fp64_peak(200.0)
+    # the same issue loop held for 2 s: the rate the SMs sustain once the power management has settled, which is the
+    # fair denominator for a kernel timed inside a seconds-long step loop (the 200 ms figure is the burst rate)
+    peak_dmma_sustained = afqmc.measure_fp64_peak(2000.0)[0] if rank == 0 else None
 
     if cx:
         walkers_h = cx["walkers"]
@@ -398,13 +404,29 @@ def main():
         xs = torch.from_numpy(xs_h).cuda()
         E = torch.empty((nw, 3), dtype=torch.complex128, device="cuda")
 
+        NX = xs.shape[0]                   # fields of Wm + args.steps steps, reused cyclically beyond that
+
         def one(s):
-            g.step(W, wt, xs[s], cfg.dt)
+            g.step(W, wt, xs[s % NX], cfg.dt)
             g.local_energy(W, E)
 
         for s in range(Wm):
             one(s)
         g.sync()
+        if args.min_seconds > 0.0:
+            # size the timed region from a short untimed probe (same on every rank: the max is taken)
+            q0, q1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            nprobe = max(3, Wm)
+            q0.record(stream)
+            for s in range(nprobe):
+                one(s)
+            q1.record(stream)
+            torch.cuda.synchronize()
+            est = max_over_ranks(q0.elapsed_time(q1) / nprobe, dist, "cuda")
+            K = max(K, int(np.ceil(args.min_seconds * 1e3 / max(est, 1e-4))))
+            W.copy_(torch.from_numpy(walkers_h))
+            wt.fill_(1.0)
+            torch.cuda.synchronize()
         l0 = g.launch_count()
         barrier()
         torch.cuda.synchronize()
@@ -432,13 +454,14 @@ def main():
         g.set_profiling(True)
         g.stage_times(reset=True)
         p0, p1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        Kp = min(K, max(args.steps, 200))       # a raised K (--min-seconds) is not needed for the breakdown
         p0.record(stream)
-        for s in range(Wm, Wm + K):
-            g.step(Wb, wb, xs[s], cfg.dt)
+        for s in range(Wm, Wm + Kp):
+            g.step(Wb, wb, xs[s % NX], cfg.dt)
             g.local_energy(Wb, E)
         p1.record(stream)
         torch.cuda.synchronize()
-        ms_prof = p0.elapsed_time(p1)
+        ms_prof = p0.elapsed_time(p1) * K / Kp   # scaled to K steps: everything below divides by K
         stages = g.stage_times(reset=True)
         g.set_profiling(False)
         del Wb, wb
@@ -461,7 +484,7 @@ def main():
         Wn, wn, En = Wp.numpy(), wp.numpy(), Ep.numpy()
 
         def one_host(s):
-            g.step(Wn, wn, xp[s].numpy(), cfg.dt)
+            g.step(Wn, wn, xp[s % NX].numpy(), cfg.dt)
             g.local_energy(Wn, En)
 
         for s in range(min(Wm, 2)):
@@ -487,7 +510,7 @@ def main():
 
     # ---- roofline of the dominant kernel -------------------------------------------------------
     fl = flops_model(cfg, nw, cx["nf"] if cx else 0)
-    per_stage = {k: {"ms_per_step": v[0] / K, "launches": v[1]} for k, v in stages.items() if v[1]}
+    per_stage = {k: {"ms_per_step": v[0] / Kp, "launches": v[1]} for k, v in stages.items() if v[1]}
     for k, f in fl.items():
         if k in per_stage and per_stage[k]["ms_per_step"] > 0:
             tf = f / (per_stage[k]["ms_per_step"] * 1e-3) / 1e12
@@ -518,6 +541,10 @@ def main():
                            "(register-only mma.sync.m8n8k4.f64 loop, 200 ms); MEASURED_PEAKS.json has "
                            "no FP64 entry",
             "achieved": per_stage[dom].get("tflops"), "frac": per_stage[dom].get("frac_of_dmma_peak"),
+            "peak_sustained": peak_dmma_sustained,
+            "frac_sustained": (per_stage[dom]["tflops"] / peak_dmma_sustained
+                               if per_stage[dom].get("tflops") and peak_dmma_sustained else None),
+            "peak_sustained_source": "the same loop held for 2 s (power management settled)",
             "flops_per_launch": fl.get(dom, 0.0) / nl,
             "ms_per_launch": per_stage[dom]["ms_per_step"] / nl,
             "share_of_step": per_stage[dom]["ms_per_step"] / (ms_prof / K),
@@ -538,6 +565,21 @@ def main():
         roof["peak_by_guide_rule"] = rule
         roof["frac_by_guide_rule"] = (roof["achieved"] / rule) if roof["achieved"] else None
         roof["hbm_gbs_measured"] = mp.get("hbm_gbs")
+        # north_star: achieved HBM GB/s of the streaming kernels against the measured copy bandwidth.  Algorithmic
+        # bytes only (each array once): a4 reads X (complex) and x and writes the shifted fields (complex);
+        # the energy reduction reads X of the energy pass (complex) and the exchange kernel's partial sums
+        # [n_chol / G][nw] (complex) per spin block.  Both are launch-latency sized at these shapes.
+        nf_ = cx["nf"] if cx else cfg.n_chol
+        plan_G = [int(t.split(" G ")[1].split()[0]) if " G " in t else 1
+                  for t in (afqmc.exchange_plan(ns, cfg.M, bool(cx))[1] for ns in
+                            ([cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta]))]
+        stream_bytes = {"field_shift": 40.0 * nf_ * nw,
+                        "e_reduce": 16.0 * nf_ * nw + sum(16.0 * ((nf_ + G_ - 1) // G_) * nw for G_ in plan_G)}
+        for k_, by_ in stream_bytes.items():
+            if k_ in per_stage and per_stage[k_]["ms_per_step"] > 0 and mp.get("hbm_gbs"):
+                gbs = by_ / (per_stage[k_]["ms_per_step"] * 1e-3) / 1e9
+                per_stage[k_].update({"bound": "hbm", "algorithmic_bytes": by_, "gbytes_per_s": gbs,
+                                      "frac_of_hbm_peak": gbs / float(mp["hbm_gbs"])})
     except (OSError, KeyError, ValueError):
         pass
 
@@ -554,6 +596,7 @@ def main():
                    "exchange_plan": [afqmc.exchange_plan(ns, cfg.M, bool(cx))[1] for ns in
                                      ([cfg.n_alpha] if cfg.walker_kind == 0 else [cfg.n_alpha, cfg.n_beta])],
                    "hbm_resident_gb": round(hbm_resident_gb, 1),
+                   "steps_requested": args.steps, "min_seconds": args.min_seconds,
                    "l2": "inputs > L2 (Cholesky tensor %.1f GB)" % (cfg.n_chol * cfg.M * cfg.M * 8 / 1e9)},
         "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
         "roofline": roof, "stages": per_stage, "block": block,
@@ -595,7 +638,9 @@ def main():
         v, sec, thr = oracle_sample(cfg, h1, Lh, trial, nw_s, 2, 1)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": thr, "kind": "oracle",
                                 "sample": f"{nw_s} of {nw} walkers x 2 steps after 1 warm-up step (step + local "
-                                          f"energy), {sec:.1f} s per step"}
+                                          f"energy), {sec:.1f} s per step; the oracle's V_HS and setup stream the whole "
+                                          f"Cholesky tensor for these {nw_s} walkers, the GPU arm amortises that stream "
+                                          f"over {nw}: the oracle's walker-steps/s at full batch would be higher"}
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -32,9 +32,11 @@
  * reading S10).
  *
  * Threads: a handle may be driven by one host thread at a time; different handles may be driven from
- * different host threads concurrently.  The only process-wide state is the per-device bookkeeping of
- * one-off kernel attributes (mutex protected) and the message of a failed afqmc_create, which is kept per
- * host thread (afqmc_last_error(NULL) returns the calling thread's).
+ * different host threads concurrently.  Process-wide state: the per-device bookkeeping of one-off kernel
+ * attributes (mutex protected); the message of a failed afqmc_create, kept per host thread
+ * (afqmc_last_error(NULL) returns the calling thread's); the exchange kernel's plan table, which only the tuning
+ * hooks afqmc_exchange_plan_pin / _unpin write (mutex protected, and it changes what handles created LATER launch:
+ * see there); and the built-in scratch array of afqmc_comb_static (one per GPU, shared by all callers: see there).
  */
 #ifndef AFQMC_H_
 #define AFQMC_H_
@@ -230,8 +232,12 @@ int32_t afqmc_get_overlaps(afqmc_handle* h, void* ovlp_out);
  * passes with a shifted pass when the Gram matrix is numerically singular (cond(phi) up to ~1e15).
  *   walkers  EITHER complex128 [nw][M][Nt], in/out.
  *   detR_out EITHER double [nw][n_blocks] = prod_i R_ii per block (n_blocks = 1 RHF, 2 UHF), or NULL.
- * If nw equals the nw of the last afqmc_step the stored overlaps (afqmc_get_overlaps) are divided by
- * prod_sigma det R_sigma (squared for RHF), as on the schedule. */
+ * SIDE EFFECT on the handle's stored overlaps (afqmc_get_overlaps): the library cannot tell whose walkers it is
+ * given, so whenever nw equals the nw of the last afqmc_step it ASSUMES these are that step's walkers and divides the
+ * stored overlaps by prod_sigma det R_sigma (squared for RHF), as on the schedule.  Passing unrelated walkers of the
+ * same count therefore leaves afqmc_get_overlaps meaningless until the next afqmc_step (which recomputes them from
+ * scratch; nothing else in the library reads them).  Use a second handle, or a different nw, to orthonormalise
+ * walkers that are not the handle's current population. */
 int32_t afqmc_reorthonormalise(afqmc_handle* h, void* walkers, double* detR_out, int32_t nw);
 /* Number of shifted Cholesky-QR passes (numerically singular Gram matrices) since afqmc_create; synchronises. */
 int64_t afqmc_qr_shifted_passes(afqmc_handle* h);
@@ -379,6 +385,12 @@ int32_t afqmc_exchange_plan(int32_t ns, int32_t M, int32_t pair, char* out, int3
  * no such candidate exists (does not fit shared memory or registers). */
 int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t warps, int32_t mi, int32_t ni, int32_t wm,
                                 int32_t G, int32_t Wn, int32_t epi_warps);
+/* Undo afqmc_exchange_plan_pin for (ns, M, pair): the next handle gets the library's own plan again.  ns <= 0 forgets
+ * every pin of the process.  The same ordering rule applies as for pinning: handles that exist keep buffers sized for
+ * the plan they were created under.  The plan table is process-wide and mutex protected; a launch works on its own
+ * copy of the plan, so pinning from one host thread while another thread launches is safe (that launch uses the old
+ * or the new plan, never a mixture). */
+int32_t afqmc_exchange_plan_unpin(int32_t ns, int32_t M, int32_t pair);
 
 #ifdef __cplusplus
 }

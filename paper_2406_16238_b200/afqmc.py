@@ -23,7 +23,8 @@ EXPORTS = ["afqmc_create", "afqmc_step", "afqmc_local_energy", "afqmc_get_overla
            "afqmc_shard_get_buffers", "afqmc_shard_ipc_export", "afqmc_shard_ipc_open", "afqmc_shard_ipc_close",
            "afqmc_shard_set_peers", "afqmc_shard_theta", "afqmc_shard_vhs", "afqmc_shard_propagate",
            "afqmc_shard_energy", "afqmc_shard_energy_finish", "afqmc_shard_setup_reduce", "afqmc_exchange_plan", "afqmc_exchange_plan_pin",
-           "afqmc_reorthonormalise", "afqmc_qr_shifted_passes", "afqmc_comb_static"]
+           "afqmc_reorthonormalise", "afqmc_qr_shifted_passes", "afqmc_comb_static",
+           "afqmc_exchange_plan_unpin"]
 
 COMB_STATIC_MAX_WALKERS = 65536      # AFQMC_COMB_STATIC_MAX_WALKERS of include/afqmc.h
 
@@ -104,6 +105,8 @@ def _load():
     lib.afqmc_exchange_plan.restype = i32
     lib.afqmc_exchange_plan_pin.argtypes = [i32] * 10
     lib.afqmc_exchange_plan_pin.restype = i32
+    lib.afqmc_exchange_plan_unpin.argtypes = [i32, i32, i32]
+    lib.afqmc_exchange_plan_unpin.restype = i32
     return lib
 
 
@@ -166,6 +169,13 @@ def exchange_plan_pin(ns, M, pair, warps, mi, ni, wm, G, Wn, epi_warps=3):
     """Pin the exchange kernel's tile plan for (ns, M, pair); call before creating handles.  False if it does not fit."""
     return lib.afqmc_exchange_plan_pin(int(ns), int(M), int(bool(pair)), int(warps), int(mi), int(ni), int(wm),
                                        int(G), int(Wn), int(epi_warps)) == 0
+
+
+def exchange_plan_unpin(ns=0, M=0, pair=False):
+    """Forget the pinned exchange plan of (ns, M, pair); ns = 0: every pin of this process."""
+    rc = lib.afqmc_exchange_plan_unpin(int(ns), int(M), 1 if pair else 0)
+    if rc != 0:
+        raise AfqmcError(rc, "afqmc_exchange_plan_unpin")
 
 
 class AFQMC:

@@ -1015,14 +1015,18 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     g2.M = Nt; g2.N = M; g2.K = M;
     h->launches += run_gemm(GEMM_KN, g2, h->st);
     if (ctrial) {
-      // psi^+ h = (Re psi^T hr + Im psi^T hi) + i (Re psi^T hi - Im psi^T hr); Pa, Pb are free scratch here
+      // psi^+ h = (Re psi^T hr + Im psi^T hi) + i (Re psi^T hi - Im psi^T hr).  The two Nt x M products go through
+      // Lrot_sum (nf Nt M doubles, nf >= 2, filled only below): Nt exceeds M for UHF walkers past half filling, so an
+      // M x M buffer such as Pa / Pb is too small for them.
+      double* s0 = h->Lrot_sum;
+      double* s1 = h->Lrot_sum + (size_t)Nt * M;
       GemmArgs g3 = g2;
-      g3.A = h->trialT + (size_t)Nt * M; g3.C = h->Pa;                  // -Im psi^T hi
+      g3.A = h->trialT + (size_t)Nt * M; g3.C = s0;                     // -Im psi^T hi
       h->launches += run_gemm(GEMM_KN, g3, h->st);
-      g3.B = h->h1; g3.C = h->Pb;                                       // -Im psi^T hr
+      g3.B = h->h1; g3.C = s1;                                          // -Im psi^T hr
       h->launches += run_gemm(GEMM_KN, g3, h->st);
-      h->launches += run_add_scaled(h->hrot, h->hrot, h->Pa, -1.0, (long)Nt * M, h->st);
-      h->launches += run_add_scaled(h->hrot_i, h->hrot_i, h->Pb, 1.0, (long)Nt * M, h->st);
+      h->launches += run_add_scaled(h->hrot, h->hrot, s0, -1.0, (long)Nt * M, h->st);
+      h->launches += run_add_scaled(h->hrot_i, h->hrot_i, s1, 1.0, (long)Nt * M, h->st);
     }
     h->launches += run_add(h->Lrot_sum, h->Lrot, h->Lrot + (size_t)nf * Nt * M, (long)nf * Nt * M, h->st);
     if (cudaStreamSynchronize(h->st) != cudaSuccess || cudaGetLastError() != cudaSuccess)
@@ -1120,7 +1124,8 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   h->Xe = dalloc(h, (size_t)nc * mwg * 2); h->e1 = dalloc(h, (size_t)mw * 2 * 2);
   h->Obuf = dalloc(h, (size_t)mw * Nt * 2 * Nt); h->Aop = dalloc(h, (size_t)mw * 4 * Nt * Nt);
   if (!h->Obuf || !h->Aop) return bail(AFQMC_ERR_ALLOC, "device allocation failed (overlap operands)");
-  h->ot_gemm = h->ws && p->kernel_path != 2;   // kernel_path = 2: the one-kernel overlap / Theta route (tests)
+  // kernel_path = 2: the one-kernel overlap / Theta route (tests); a group member always takes the GEMM route
+  h->ot_gemm = h->ws && (G > 1 || p->kernel_path != 2);
   h->small = p->kernel_path == 0 && !cplx && !p->mixed_precision && !p->pack_chol && G == 1 &&
              small_path_fits(M, Nt, std::max(h->ns[0], h->ns[1]), nc);
   if (G > 1) {
@@ -1272,6 +1277,12 @@ int32_t afqmc_exchange_plan_pin(int32_t ns, int32_t M, int32_t pair, int32_t war
                                 int32_t G, int32_t Wn, int32_t epi_warps) {
   if (ns < 1 || ns > afq::kMaxOcc || M < ns) return AFQMC_ERR_INVALID;
   return afq::exchange_ws_pin(ns, M, pair != 0, warps, mi, ni, wm, G, Wn, epi_warps) ? AFQMC_OK : AFQMC_ERR_UNSUPPORTED;
+}
+
+int32_t afqmc_exchange_plan_unpin(int32_t ns, int32_t M, int32_t pair) {
+  if (ns > afq::kMaxOcc || (ns > 0 && M < ns)) return AFQMC_ERR_INVALID;
+  afq::exchange_ws_unpin(ns, M, pair != 0);
+  return AFQMC_OK;
 }
 
 int32_t afqmc_step(afqmc_handle* h, void* walkers, double* weights, const double* aux_fields, double dt, int32_t nw) {

@@ -586,15 +586,15 @@ int launch_xws(const ExArgs& e, const Plan& p, cudaStream_t st) {
 std::mutex g_plan_mu;
 std::map<long, Plan> g_plan_cache;
 
-const Plan& cached_plan(int ns, bool pair, int M) {
-  std::mutex& mu = g_plan_mu;
-  std::map<long, Plan>& cache = g_plan_cache;
+// By value, copied under the lock: a pin from another host thread may overwrite the entry at any time, and a launch
+// must see one plan from its first field to its last.
+Plan cached_plan(int ns, bool pair, int M) {
   const int KT = (M + 15) / 16;
   const long key = ((long)KT << 8 | ns) << 1 | (pair ? 1 : 0);
-  std::lock_guard<std::mutex> lk(mu);
-  auto it = cache.find(key);
-  if (it == cache.end()) it = cache.emplace(key, make_plan(ns, pair, KT)).first;
-  return it->second;      // std::map nodes are stable
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  auto it = g_plan_cache.find(key);
+  if (it == g_plan_cache.end()) it = g_plan_cache.emplace(key, make_plan(ns, pair, KT)).first;
+  return it->second;
 }
 
 }  // namespace
@@ -625,9 +625,17 @@ bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, 
   return true;
 }
 
+// Forget the pin of (ns, M, pair), or every pin with ns <= 0: the next use computes the library's own choice again.
+void exchange_ws_unpin(int ns, int M, bool pair) {
+  std::lock_guard<std::mutex> lk(g_plan_mu);
+  if (ns <= 0) { g_plan_cache.clear(); return; }
+  const int KT = (M + 15) / 16;
+  g_plan_cache.erase(((long)KT << 8 | ns) << 1 | (pair ? 1 : 0));
+}
+
 // human-readable plan (bench / tests)
 void exchange_ws_describe(int ns, int M, bool pair, char* out, int n) {
-  const Plan& p = cached_plan(ns, pair, M);
+  const Plan p = cached_plan(ns, pair, M);
   if (p.inst < 0) { snprintf(out, n, "no plan"); return; }
   snprintf(out, n, "warps %d+%d grid %dx%d (<=%dx%d blocks each) G %d Wn %d tile %dx%d eff %.3f stages %d passes %dx%d nbuf %d ldt %d smem %zu",
            p.ncw, kInst[p.inst].EW, p.WM, p.ncw / p.WM, kInst[p.inst].MI, kInst[p.inst].NI, p.G, p.Wn, p.rowsA, p.rowsB, p.eff, p.stages,
@@ -637,7 +645,7 @@ void exchange_ws_describe(int ns, int M, bool pair, char* out, int n) {
 // returns launches issued, -1 if the tensor maps could not be encoded, -2 if the plan needs more partial-sum rows
 // than the caller allocated
 int run_exchange_ws(const ExArgs& e, cudaStream_t st) {
-  const Plan& p = cached_plan(e.ns, e.plane_stride != 0, e.M);
+  const Plan p = cached_plan(e.ns, e.plane_stride != 0, e.M);
   if (p.inst < 0) return -1;
   if (e.ngroups_cap > 0 && (e.n_chol + p.G - 1) / p.G != e.ngroups_cap) return -2;   // the reduce sums exactly cap rows
   switch (p.inst) {

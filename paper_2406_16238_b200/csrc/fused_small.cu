@@ -350,11 +350,12 @@ __global__ void __launch_bounds__(256) small_step_kernel(SmallArgs a) {
     const double2 S = cmul2(r, make_double2(em * cs, em * sn));
     const double absS = hypot(S.x, S.y);
     double absI = absS * exp(cfb_r) * exp(a.expo);
+    const bool finI = isfinite(absI);          // before the bound, as in weight_update_kernel (small.cu)
     if (a.ehyb_bound > 0.0 && absI > 0.0) {
       const double D = -log(absI) / a.dt;
       if (fabs(D) > a.ehyb_bound) absI = exp(-a.dt * copysign(a.ehyb_bound, D));
     }
-    const bool ok = isfinite(S.x) && isfinite(S.y) && isfinite(absI) && absS > 0.0 &&
+    const bool ok = isfinite(S.x) && isfinite(S.y) && finI && absS > 0.0 &&
                     (ov_old.x != 0.0 || ov_old.y != 0.0) && isfinite(ov_new.x) && isfinite(ov_new.y) && isfinite(cfb_i);
     double wt = a.weights[w];
     if (!ok) {

@@ -45,6 +45,14 @@ struct KnArgs {
 // Work of one CTA as a short list of segments (tile, k range, mode): 0 whole tile, 1 first part of a tile whose rest
 // belongs to CTA c + 1 (accumulators go to sk_part[c]), 2 last part of a tile started by CTA c - 1.  The first part
 // comes FIRST so that the neighbour never waits long.
+// Forward progress of the spin wait (CTA c polls the flag CTA c - 1 sets): parking depends on nothing - a CTA parks
+// before it ever waits - so a CTA that has been dispatched always reaches its atomicExch.  CTA c therefore only needs
+// CTA c - 1 to have been DISPATCHED, not to be co-resident with it: the grid is at most one CTA per SM and the
+// hardware hands out CTAs of a grid in increasing blockIdx order, so this holds alone on the device and also when
+// other kernels (another handle's stream, torch, MPS clients) occupy some SMs - a CTA that is running had all its
+// predecessors started before it.  What it does NOT survive is a scheduler that starts CTA c while withholding
+// CTA c - 1 for good; no CUDA device does that today, and a cooperative launch would make it a guarantee at the
+// price of refusing to run beside other work.
 struct KnSeg { int tile, kb, ke, mode; };
 __device__ __forceinline__ bool kn_segment(const KnArgs& a, int KT, int ntiles, int idx, KnSeg& s) {
   if (a.sk_w <= 0) {
@@ -333,6 +341,10 @@ int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, const KnStre
     const long plain = ((nt + grid - 1) / grid) * KT;
     if (w >= KT && (double)(w + 8) < 0.99 * plain && need <= sk->part_doubles && grid <= sk->flags) {
       a.sk_w = (int)w; a.sk_part = sk->part; a.sk_flag = sk->flag;
+      // The kernel leaves every flag at 0 when it completes; a launch that was aborted (sticky error, device reset of
+      // a peer context) may not have, and its stale 1 would let a consumer read accumulators that were never parked.
+      // Clearing on the stream costs one memset node per stream-K launch (8 per step at c5, ~2 us each).
+      cudaMemsetAsync(sk->flag, 0, (size_t)grid * sizeof(int), st);
     }
   }
   kern<<<grid, Cfg::THREADS, smem, st>>>(tmA, tmB, a);

@@ -170,6 +170,7 @@ int exchange_ws_group_size(int ns, int M, bool pair = false);      // the plan d
 double exchange_ws_efficiency(int ns, int M, bool pair = false);
 void exchange_ws_describe(int ns, int M, bool pair, char* out, int n);
 bool exchange_ws_pin(int ns, int M, bool pair, int ncw, int mi, int ni, int wm, int G, int Wn, int ew);
+void exchange_ws_unpin(int ns, int M, bool pair);
 int run_exchange_ws(const ExArgs& a, cudaStream_t st);
 
 struct EnergyArgs {

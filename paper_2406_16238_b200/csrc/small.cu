@@ -392,11 +392,12 @@ __global__ void weight_update_kernel(WeightArgs a, int nw) {
   const double2 S = cmul(r, make_double2(em * cs, em * sn));        // Eq. (17)
   const double absS = hypot(S.x, S.y);
   double absI = absS * exp(a.cfb[2 * w]) * exp(a.expo);              // |I|, Eq. (16) + reading S7
+  const bool finI = isfinite(absI);                                  // judged BEFORE the bound: an overflowed |I| kills
   if (a.ehyb_bound > 0.0 && absI > 0.0) {                            // reading S8b: clip D = -log|I| / dt
     const double D = -log(absI) / a.dt;
     if (fabs(D) > a.ehyb_bound) absI = exp(-a.dt * copysign(a.ehyb_bound, D));
   }
-  const bool ok = isfinite(S.x) && isfinite(S.y) && isfinite(absI) && absS > 0.0 &&
+  const bool ok = isfinite(S.x) && isfinite(S.y) && finI && absS > 0.0 &&
                   (oo.x != 0.0 || oo.y != 0.0) && isfinite(on.x) && isfinite(on.y) &&
                   isfinite(a.cfb[2 * w + 1]);
   double wt = a.weights[w];

@@ -122,6 +122,17 @@ def test_exchange_plan_exists_for_every_block_size():
     assert "warps 8+7" in afqmc.exchange_plan(50, 300)[1] and "tile 150x100" in afqmc.exchange_plan(50, 300)[1]
     assert "warps 8+7" in afqmc.exchange_plan(16, 108)[1]
     # pinning: a candidate that cannot exist is refused, one that exists replaces the plan
+    own = afqmc.exchange_plan(50, 302)[1]
+    own2 = afqmc.exchange_plan(42, 90)[1]
     assert not afqmc.exchange_plan_pin(50, 300, False, 12, 4, 7, 4, 30, 30)
     assert afqmc.exchange_plan_pin(50, 302, False, 12, 4, 7, 6, 3, 1)
-    assert "grid 6x2" in afqmc.exchange_plan(50, 302)[1]
+    assert "grid 6x2" in afqmc.exchange_plan(50, 302)[1] and "grid 6x2" not in own
+    # ... and unpinning gives the library's own choice back (nothing pinned is left behind for later tests)
+    afqmc.exchange_plan_unpin(50, 302)
+    assert afqmc.exchange_plan(50, 302)[1] == own
+    assert afqmc.exchange_plan_pin(50, 302, False, 12, 4, 7, 6, 3, 1)
+    assert any(afqmc.exchange_plan_pin(42, 90, False, 12, 4, 7, wm, 1, 1) for wm in (1, 2, 3, 4, 6, 12))
+    assert afqmc.exchange_plan(42, 90)[1] != own2
+    afqmc.exchange_plan_unpin()                               # ns = 0: every pin
+    assert afqmc.exchange_plan(42, 90)[1] == own2 and afqmc.exchange_plan(50, 302)[1] == own
+    assert afqmc.lib.afqmc_exchange_plan_unpin(65, 100, 0) == -1

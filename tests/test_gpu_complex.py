@@ -60,7 +60,9 @@ def _energy(g, W):
     return E.cpu().numpy()
 
 
-CASES = [(24, 5, 5, 12, 0, 8), (40, 9, 6, 10, 1, 5), (37, 7, 7, 9, 0, 3), (64, 16, 14, 20, 1, 6)]
+# the last case is UHF past half filling: Nt = n_alpha + n_beta = 19 > M = 16 (Nt x M setup products must not go
+# through M x M scratch)
+CASES = [(24, 5, 5, 12, 0, 8), (40, 9, 6, 10, 1, 5), (37, 7, 7, 9, 0, 3), (64, 16, 14, 20, 1, 6), (16, 10, 9, 6, 1, 4)]
 
 
 @pytest.mark.parametrize("ctrial", [False, True])

@@ -8,6 +8,7 @@ from __future__ import annotations
 import numpy as np
 import pytest
 
+from paper_2406_16238_b200 import inputs
 from tests.gpu_util import Pair, energy_scale, planar_to_complex, rel_fro, rel_max
 
 pytestmark = pytest.mark.gpu
@@ -507,6 +508,45 @@ def test_bounds_trigger_on_literal_amplitudes():
     assert np.all(np.isfinite(wo))
 
 
+@pytest.mark.parametrize("kernel_path", [0, 3])
+def test_overflowed_importance_function_is_a_dead_walker_even_with_the_bound(kernel_path):
+    """Reading S10 comes before reading S8b: a walker whose |I| is not finite (here exp(-dt (E_const - E_shift))
+    overflows through an absurd caller-supplied E_shift) gets weight exactly 0; the hybrid-energy bound clips finite
+    values only and must not turn inf into exp(dt b).  Both weight kernels (one-kernel step, kernel_path 0 at c1;
+    weight_update_kernel, kernel_path 3) against the oracle, which judges isfinite(I) before it clips."""
+    torch = _torch()
+    from oracle.afqmc_oracle import AFQMCOracle
+    from paper_2406_16238_b200 import afqmc
+    cfg = inputs.get_config("c1")
+    nw, dt = 6, cfg.dt
+    h1 = inputs.make_h1(cfg, 0)
+    trial = inputs.make_trial(cfg, h1, 0)
+    L = inputs.make_L_host(cfg, 0, False)
+    W0 = inputs.make_walkers(cfg, trial, 0, nw)
+    x = inputs.make_aux_fields(cfg, 0, 0, nw)
+    bound = float(np.sqrt(2.0 / dt))
+    for e_shift, dead in ((1.0e6, True), (0.0, False)):           # dt * 1e6 = 5000 > log(DBL_MAX) = 709.8
+        o = AFQMCOracle(h1, L, trial, cfg.n_alpha, cfg.n_beta, cfg.walker_kind, taylor_order=cfg.taylor_order,
+                        e_shift=e_shift, ehyb_bound=bound)
+        Ld = torch.from_numpy(L).cuda()
+        g = afqmc.AFQMC(h1, Ld, trial, M=cfg.M, n_alpha=cfg.n_alpha, n_beta=cfg.n_beta, n_chol=cfg.n_chol,
+                        max_walkers=nw, walker_kind=cfg.walker_kind, taylor_order=cfg.taylor_order,
+                        e_shift=e_shift, ehyb_bound=bound, kernel_path=kernel_path)
+        Wd = torch.from_numpy(W0.copy()).cuda()
+        wd = torch.ones(nw, dtype=torch.float64, device="cuda")
+        xd = torch.from_numpy(x).cuda()
+        torch.cuda.synchronize()
+        g.step(Wd, wd, xd, dt)
+        g.sync()
+        _, w_o, _ = o.step(W0, np.ones(nw), x, dt)
+        w_g = wd.cpu().numpy()
+        if dead:
+            assert np.all(w_o == 0.0) and np.all(w_g == 0.0), (w_o, w_g)
+        else:
+            assert np.all(w_o > 0.0) and rel_max(w_g, w_o) < TOL_STEP
+        g.close()
+
+
 # --------------------------------------------------------------------------- every exchange-kernel instantiation
 _INSTS = [(8, 5, 7, 3), (8, 7, 5, 3), (8, 6, 6, 3), (12, 4, 7, 3), (12, 7, 4, 3), (12, 5, 5, 3), (12, 5, 4, 3),
           (12, 4, 5, 3), (8, 5, 7, 7), (8, 7, 5, 7), (8, 6, 6, 7)]
@@ -561,6 +601,13 @@ def test_every_exchange_plan_gives_the_same_energy(name, nw, over):
     with pytest.raises(afqmc.AfqmcError):
         gpu_energy(pr, W)
     pr.close()
+    # leave no pinned plan behind: later tests in this process get the library's own plans, whatever the order
+    afqmc.exchange_plan_unpin()
+    pr = Pair(name, nw=nw, oracle=False, kernel_path=3, **over)
+    E_g = gpu_energy(pr, W)
+    pr.close()
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10, k
 
 
 # --------------------------------------------------------------------------- a10 on ill-conditioned walkers

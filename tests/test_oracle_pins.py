@@ -565,3 +565,71 @@ def test_P17_bounds():
     assert np.max(np.abs(wt3 - expect)) < 1e-14 * expect.max()
     mb3 = _many_body_step(eb, h, L, trial, walkers, x, w0, dt, ehyb_bound=B)
     assert np.max(np.abs(wt3 - mb3["w"])) < 1e-10 * mb3["w"].max()
+    # (d) reading S10 before S8b: a walker whose importance function is not finite is dead (weight exactly 0); the
+    # bound clips finite values only and never turns inf into exp(dt b).  E_shift = 1e6: exp(-dt (E_const - E_shift))
+    # overflows, every |I| is inf.
+    dead = AFQMCOracle(h, L, trial, na, nb, kind, taylor_order=24, e_shift=1.0e6, ehyb_bound=B)
+    _, info_d = dead.propagate(walkers, x, dt)
+    assert not np.isfinite(info_d["I"]).any()
+    _, wt4, _ = dead.step(walkers, w0, x, dt)
+    assert np.array_equal(wt4, np.zeros_like(w0))
+
+
+# --------------------------------------------------------------------------- P18 (the slab-provider branch)
+@pytest.mark.parametrize("kind", [0, 1])
+def test_P18_slab_provider_is_the_array_path(kind):
+    """At c4 / c5 the oracle never sees the Cholesky tensor as one array: `_as_slab_iter` takes a callable that
+    yields (g0, slab) pairs, and __init__ (m, h', h_mod, Lrot) and `vhs` accumulate slab by slab.  Pin that branch:
+    UNEVEN slabs (5, 1, 7 vectors - a dropped or doubled slab, a wrong g0 offset into the fields, or a slab mistaken
+    for the whole tensor all fail here) against (i) the array path and (ii) the closed forms that pin the array path
+    itself - the Hartree-Fock energy of P2 and the definition A = -i sqrt(dt) sum_g x_g L_g of Eq. (9)."""
+    na, nb = (3, 3) if kind == 0 else (3, 2)
+    M, ng, dt = 9, 13, 0.01
+    h, L, trial, walkers = small_problem(M, na, nb, ng, kind, 18)
+    cuts = [0, 5, 6, 13]
+    calls = []
+
+    def provider():
+        calls.append(1)
+        for a, b in zip(cuts[:-1], cuts[1:]):
+            yield a, L[a:b].copy()
+
+    o_arr = AFQMCOracle(h, L, trial, na, nb, kind, ortho_every=2)
+    o_slab = AFQMCOracle(h, provider, trial, na, nb, kind, ortho_every=2)
+    assert o_slab.n_chol == ng
+    for name in ("m", "h_mod", "E_const", "e_shift"):
+        a, b = np.asarray(getattr(o_slab, name)), np.asarray(getattr(o_arr, name))
+        assert np.max(np.abs(a - b)) <= 1e-14 * max(1.0, np.max(np.abs(b))), name
+    for a, b in zip(o_slab.Lrot, o_arr.Lrot):
+        assert a.shape == b.shape and np.max(np.abs(a - b)) <= 1e-14 * np.max(np.abs(b))
+    # (ii) P2's closed form through the provider
+    pa = trial[:, :na]
+    pb = pa if kind == 0 else trial[:, na:]
+    Pa, Pb = pa @ pa.T, pb @ pb.T
+    e1 = np.trace(h @ Pa) + np.trace(h @ Pb)
+    ec = 0.5 * sum((np.trace(Lg @ Pa) + np.trace(Lg @ Pb)) ** 2 for Lg in L)
+    ex = -0.5 * sum(np.trace(Lg @ Pa @ Lg @ Pa) + np.trace(Lg @ Pb @ Lg @ Pb) for Lg in L)
+    E = o_slab.local_energy(trial[None].astype(np.complex128))[0]
+    assert abs(E[0] - (e1 + ec + ex)) < 1e-12 * abs(e1 + ec + ex)
+    assert abs(o_slab.e_shift - (e1 + ec + ex)) < 1e-11
+    # V_HS through the provider: the definition, with complex shifted fields, and the array path
+    r = np.random.default_rng(180)
+    xs = r.standard_normal((walkers.shape[0], ng)) + 1j * r.standard_normal((walkers.shape[0], ng))
+    n0 = len(calls)
+    A = o_slab.vhs(xs, dt)
+    assert len(calls) == n0 + 1                                   # the tensor is streamed once per build
+    A_def = -1j * np.sqrt(dt) * np.einsum("wg,gpq->wpq", xs, L)
+    assert np.max(np.abs(A - A_def)) <= 1e-14 * np.max(np.abs(A_def))
+    assert np.max(np.abs(A - o_arr.vhs(xs, dt))) <= 1e-14 * np.max(np.abs(A_def))
+    # two full steps (the second re-orthonormalises) and the local energy
+    x = r.standard_normal((2, walkers.shape[0], ng))
+    Wa, wa = walkers.copy(), np.ones(walkers.shape[0])
+    Wb, wb = walkers.copy(), np.ones(walkers.shape[0])
+    for s in range(2):
+        Wa, wa, ova = o_arr.step(Wa, wa, x[s], dt)
+        Wb, wb, ovb = o_slab.step(Wb, wb, x[s], dt)
+    assert np.max(np.abs(Wa - Wb)) <= 1e-13 * np.max(np.abs(Wa))
+    assert np.max(np.abs(wa - wb)) <= 1e-13 * np.max(np.abs(wa))
+    assert np.max(np.abs(ova - ovb)) <= 1e-13 * np.max(np.abs(ova))
+    Ea, Eb = o_arr.local_energy(Wa), o_slab.local_energy(Wb)
+    assert np.max(np.abs(Ea - Eb)) <= 1e-12 * np.max(np.abs(Ea))
