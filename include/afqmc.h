@@ -105,7 +105,10 @@ typedef struct {
                         /* O = psi^+ phi, Lrot = psi^+ K, hrot = psi^+ h, P = psi psi^+, m_g = tr(K_g P) (real).    */
                         /* Needs complex_chol = 1 (a real tensor is passed as complex vectors with zero imaginary  */
                         /* part; half of the 2 n_chol fields then multiply zero matrices).                          */
-  int32_t reserved0;    /* must be 0 (keeps the doubles below 8-byte aligned)                                       */
+  int32_t tuning_flags; /* 0 (default).  Bit 0: use stream-K in the batched Taylor / one-body GEMMs whenever the tile  */
+                        /* count leaves a partial last wave, also where the library's cost rule would not (lets a     */
+                        /* test reach that code at sizes where every walker is checked; results agree to rounding).   */
+                        /* Other bits must be 0.  (The field also keeps the doubles below 8-byte aligned.)            */
   double xbar_bound;    /* > 0: every component of the force-bias shift is capped in modulus, xbar_g <- xbar_g      */
                         /* min(1, bound / |xbar_g|), BEFORE xs, c_fb and c_mf are formed (Eqs. 12, 16 hold for any  */
                         /* xbar, so the estimator stays exact).  0: no bound (default).  SURVEY 8f NEXT-1, S8.      */

@@ -41,7 +41,7 @@ class AfqmcParams(C.Structure):
                 ("e_shift", C.c_double), ("stream", C.c_void_p), ("pack_chol", C.c_int32),
                 ("group_size", C.c_int32), ("group_rank", C.c_int32), ("mixed_precision", C.c_int32),
                 ("complex_chol", C.c_int32), ("kernel_path", C.c_int32), ("complex_trial", C.c_int32),
-                ("reserved0", C.c_int32), ("xbar_bound", C.c_double), ("ehyb_bound", C.c_double)]
+                ("tuning_flags", C.c_int32), ("xbar_bound", C.c_double), ("ehyb_bound", C.c_double)]
 
 
 def _load():
@@ -184,7 +184,7 @@ class AFQMC:
     def __init__(self, h1, L_chol, trial, *, M, n_alpha, n_beta, n_chol, max_walkers,
                  walker_kind, taylor_order=6, ortho_every=0, e_shift=None, stream=None, pack_chol=False,
                  group_size=0, group_rank=0, mixed_precision=False, complex_chol=False, kernel_path=0,
-                 complex_trial=False, xbar_bound=0.0, ehyb_bound=0.0):
+                 complex_trial=False, xbar_bound=0.0, ehyb_bound=0.0, tuning_flags=0):
         p = AfqmcParams()
         p.struct_size = C.sizeof(AfqmcParams)
         p.M, p.n_alpha, p.n_beta, p.n_chol = M, n_alpha, n_beta, n_chol
@@ -200,6 +200,7 @@ class AFQMC:
         p.kernel_path = int(kernel_path)
         p.complex_trial = 1 if complex_trial else 0
         p.xbar_bound, p.ehyb_bound = float(xbar_bound), float(ehyb_bound)
+        p.tuning_flags = int(tuning_flags)
         # L_chol is borrowed by the library (only during create when pack_chol is set)
         self._keep = (h1, None if (pack_chol or mixed_precision or complex_chol) else L_chol, trial)
         self.M, self.n_chol, self.max_walkers = M, n_chol, max_walkers

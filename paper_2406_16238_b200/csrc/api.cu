@@ -746,7 +746,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
   if (p->struct_size != (int32_t)sizeof(afqmc_params)) return fail(nullptr, AFQMC_ERR_INVALID, "bad struct_size");
   if (p->M <= 0 || p->n_chol <= 0 || p->max_walkers <= 0 || p->n_alpha <= 0 || p->n_beta < 0 ||
       p->ortho_every < 0 || p->taylor_order < 0 || (p->pack_chol != 0 && p->pack_chol != 1) || (p->mixed_precision != 0 && p->mixed_precision != 1) || (p->complex_chol != 0 && p->complex_chol != 1) || (p->walker_kind != 0 && p->walker_kind != 1) ||
-      (p->complex_trial != 0 && p->complex_trial != 1) || p->reserved0 != 0 || !(p->xbar_bound >= 0.0) || !(p->ehyb_bound >= 0.0))
+      (p->complex_trial != 0 && p->complex_trial != 1) || (p->tuning_flags & ~1) != 0 || !(p->xbar_bound >= 0.0) || !(p->ehyb_bound >= 0.0))
     return fail(nullptr, AFQMC_ERR_INVALID, "bad parameter value");
   if (p->walker_kind == 0 && p->n_alpha != p->n_beta) return fail(nullptr, AFQMC_ERR_DIMS, "RHF walkers need n_alpha == n_beta");
   if (p->walker_kind == 1 && p->n_beta <= 0) return fail(nullptr, AFQMC_ERR_DIMS, "UHF walkers need n_beta > 0");
@@ -1153,6 +1153,7 @@ int32_t afqmc_create(const double* h1, const double* L_chol, const double* trial
     h->sk.part = dalloc(h, h->sk.part_doubles);
     h->sk.flag = (int*)dalloc(h, (nsm + 1) / 2 + 1);
     h->sk.flags = nsm;
+    h->sk.force = p->tuning_flags & 1;
     if (!h->sk.part || !h->sk.flag) return bail(AFQMC_ERR_ALLOC, "device allocation failed (stream-K scratch)");
     cudaMemsetAsync(h->sk.flag, 0, (size_t)nsm * sizeof(int), h->st);
   }

@@ -339,7 +339,7 @@ int launch_kn(const TensorMap& tmA, const TensorMap& tmB, KnArgs a, const KnStre
     const size_t need = (size_t)grid * Cfg::PL * MI * NI * 2 * 256;
     // parking and fetching a tile's accumulators costs about 8 k iterations per CTA (c2, c3: no gain, measured)
     const long plain = ((nt + grid - 1) / grid) * KT;
-    if (w >= KT && (double)(w + 8) < 0.99 * plain && need <= sk->part_doubles && grid <= sk->flags) {
+    if (w >= KT && (sk->force || (double)(w + 8) < 0.99 * plain) && need <= sk->part_doubles && grid <= sk->flags) {
       a.sk_w = (int)w; a.sk_part = sk->part; a.sk_flag = sk->flag;
       // The kernel leaves every flag at 0 when it completes; a launch that was aborted (sticky error, device reset of
       // a peer context) may not have, and its stale 1 would let a consumer read accumulators that were never parked.

@@ -230,7 +230,7 @@ int taylor_tc_apply(const void* Aplanes, bool real_shared, const void* Tb, void*
 
 // gemm_ws.cu: warp-specialised TMA GEMMs (return -1 when the shapes/alignment cannot be served)
 // stream-K scratch of one caller (stream): accumulators of the tiles cut by a chunk boundary + one flag per CTA
-struct KnStreamK { double* part; size_t part_doubles; int* flag; int flags; };
+struct KnStreamK { double* part; size_t part_doubles; int* flag; int flags; int force = 0; };
 int run_gemm_ws_kn(const double* A, long lda, long sPlane, long sA, bool cplx, const double* B, long ldb, long sB,
                    double* C, double* C2, long ldc, long sC, int M, int N, int K, int batch, double alpha,
                    int mode, cudaStream_t st, const KnStreamK* sk = nullptr);

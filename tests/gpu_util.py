@@ -37,7 +37,7 @@ class Pair:
     the oracle gets either the very same host array or a slab provider over the device tensor."""
 
     def __init__(self, name, nw=None, seed=0, device_L=False, literal=False, oracle=True,
-                 ortho_every=None, pack_chol=False, kernel_path=0, xbar_bound=0.0, ehyb_bound=0.0, **overrides):
+                 ortho_every=None, pack_chol=False, kernel_path=0, xbar_bound=0.0, ehyb_bound=0.0, tuning_flags=0, **overrides):
         import torch
         from oracle.afqmc_oracle import AFQMCOracle
         from paper_2406_16238_b200 import afqmc
@@ -60,7 +60,7 @@ class Pair:
                                n_beta=cfg.n_beta, n_chol=cfg.n_chol, max_walkers=self.nw,
                                walker_kind=cfg.walker_kind, taylor_order=cfg.taylor_order,
                                ortho_every=oe, pack_chol=pack_chol, kernel_path=kernel_path,
-                               xbar_bound=xbar_bound, ehyb_bound=ehyb_bound)
+                               xbar_bound=xbar_bound, ehyb_bound=ehyb_bound, tuning_flags=tuning_flags)
         self.oracle = None
         if oracle:
             self.oracle = AFQMCOracle(self.h1, L_for_oracle, self.trial, cfg.n_alpha, cfg.n_beta,

@@ -169,6 +169,78 @@ def test_free_running_parity(name, nw):
     pr.close()
 
 
+# --------------------------------------------------------------------------- the one-kernel path at its limits
+@pytest.mark.parametrize("over,fused", [
+    # the frontier of small_path_fits (hard limits M <= 64, block <= 16, Nt <= 32, n_chol <= 2048 AND a walker's
+    # working set within 200 KB of shared memory): the largest M that still fits for each shape
+    (dict(M=61, n_alpha=16, n_beta=16, n_chol=2048, walker_kind=0), True),      # widest RHF block, longest gamma loop
+    (dict(M=47, n_alpha=16, n_beta=16, n_chol=2048, walker_kind=1), True),      # Nt = 32: widest Gauss-Jordan
+    (dict(M=57, n_alpha=16, n_beta=3, n_chol=2047, walker_kind=1), True),       # odd n_chol: the direct-load branch
+    (dict(M=64, n_alpha=5, n_beta=5, n_chol=96, walker_kind=0), True),          # largest M
+    (dict(M=62, n_alpha=16, n_beta=16, n_chol=2048, walker_kind=0), False),     # one past the shared-memory frontier
+    (dict(M=48, n_alpha=16, n_beta=16, n_chol=2048, walker_kind=1), False),     # the same for UHF
+    (dict(M=66, n_alpha=5, n_beta=5, n_chol=96, walker_kind=0), False),         # past M
+    (dict(M=64, n_alpha=17, n_beta=17, n_chol=96, walker_kind=0), False),       # one past the occupied block
+    (dict(M=48, n_alpha=16, n_beta=16, n_chol=2050, walker_kind=0), False),     # past n_chol
+])
+def test_one_kernel_path_at_and_past_its_limits(over, fused):
+    """fused_small.cu serves M <= 64, occupied blocks <= 16, Nt <= 32, n_chol <= 2048 as far as a walker's working
+    set fits one CTA's shared memory (M = 64 only with narrow blocks; 16 columns at n_chol = 2048 up to M = 61, UHF
+    16 + 16 up to M = 47).  At that frontier - the full-width warp-level Gauss-Jordan, the gamma-chunked
+    staging of the energy kernel, the bulk-copy ring with many chunks - a step with QR and the local energy against
+    the oracle; one past each limit the launch count shows that the multi-kernel path took over, same parity."""
+    _torch()
+    nw = 5
+    pr = Pair("c1", nw=nw, ortho_every=1, **over)
+    _run(pr, 1, reseed=True)                        # the first step also builds E1 = expm(-dt/2 h_mod): not counted
+    pr.oracle.n_steps_done = 0
+    l0 = pr.gpu.launch_count()
+    worst, (Wg, wg, ovg), (Wo, wo, ovo) = _run(pr, 2, reseed=True)
+    l1 = pr.gpu.launch_count()
+    assert worst["walkers"] < TOL_STEP and worst["weights"] < TOL_STEP and worst["ovlp"] < TOL_STEP, worst
+    per_step = (l1 - l0) / 2
+    if fused:
+        assert per_step <= 4, per_step               # the step kernel + the QR kernels
+    else:
+        assert per_step >= 10, per_step
+    E_o = pr.oracle.local_energy(Wo)
+    l2 = pr.gpu.launch_count()
+    E_g = gpu_energy(pr, Wo)
+    assert (pr.gpu.launch_count() - l2 == 1) == fused
+    sc = energy_scale(pr.oracle, Wo, E_o)
+    for k in range(3):
+        assert rel_max(E_g[:, k], E_o[:, k], scale=sc) < TOL_STAGE * 10
+    pr.close()
+
+
+# --------------------------------------------------------------------------- stream-K where every walker is checked
+@pytest.mark.parametrize("name,nw,over", [("c2", 640, {})])
+def test_forced_stream_k_every_walker(name, nw, over):
+    """The library switches stream-K on (gemm_ws.cu: tiles cut at chunk boundaries, first parts parked in global
+    memory, cross-CTA flags) only where its cost rule expects a gain - c4 / c5, where the oracle can only check a few
+    sampled walkers.  tuning_flags bit 0 forces it wherever the tile count leaves a partial wave: c2's 640 walkers
+    (640 tiles of 7 k-steps on 148 SMs).  (c3's shape with 64 walkers was tried too: the forced handle returned the
+    plain kernel's bits there, i.e. the launcher's other conditions kept stream-K off - not a case.)  Every walker, weight and
+    overlap of two re-seeded steps against the oracle; against the unforced handle the walkers agree to rounding but
+    NOT bit for bit (the cut tiles add their two parts in another order - which shows the forced path really ran);
+    and 25 repeats of one step are bit-identical (fixed-order sums, no dependence on which CTA arrives first)."""
+    _torch()
+    pr = Pair(name, nw=nw, tuning_flags=1, ortho_every=0, **over)
+    worst, _, _ = _run(pr, 2, reseed=True)
+    assert worst["walkers"] < TOL_STEP and worst["weights"] < TOL_STEP and worst["ovlp"] < TOL_STEP, worst
+    plain = Pair(name, nw=nw, oracle=False, ortho_every=0, **over)
+    x, w0, dt = pr.fields(0), np.ones(nw), pr.cfg.dt
+    Wf, wf, ovf = gpu_step(pr, pr.walkers0, w0, x, dt)
+    Wp, wp, ovp = gpu_step(plain, pr.walkers0, w0, x, dt)
+    assert rel_fro(Wf, Wp) < 1e-13 and rel_max(wf, wp) < 1e-12
+    assert not np.array_equal(Wf, Wp), "forced stream-K gave the plain kernel's bits: it did not run"
+    for _ in range(25):
+        Wr, wr, ovr = gpu_step(pr, pr.walkers0, w0, x, dt)
+        assert np.array_equal(Wr, Wf) and np.array_equal(wr, wf) and np.array_equal(ovr, ovf)
+    plain.close()
+    pr.close()
+
+
 # --------------------------------------------------------------------------- the other kernel paths at even M
 @pytest.mark.parametrize("path", [1, 2, 3])
 @pytest.mark.parametrize("name,nw,over", [("c1", 16, {}), ("c2", 24, {}),
